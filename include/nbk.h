@@ -1,0 +1,191 @@
+/* nbk.h -- C ABI of the B200-native direct N-body force library ("N-Body Kernels").
+ *
+ * The boundary is shaped on the GRAPE-6-style call list of the paper's `kirin` library
+ * (App. A: GPU_open, GPU_close, GPU_npipes, GPU_set_j_particle,
+ * GPU_set_ti, GPUcalc_firsthalf, GPUcalc_lasthalf) and on its statement of the data that
+ * crosses it (L80-L83: in  m, x, v;  out  a, jerk, potential).  Names and signatures are
+ * this build's own.  Differences from the paper's library, all asked for by
+ * BASELINE.json's north_star: j-particle prediction runs on the device (the paper predicts
+ * on the host and uploads all N every block step, L78, L428); split-j partial sums are
+ * reduced on the device (the paper sums them on the host, L118).
+ *
+ * What is computed (Eq. 1; "acceleration, its time derivative (jerk) and
+ * potential ... by direct summation" L68; softening L126, L132; self term L96; DESIGN.md
+ * readings R1-R8), G = 1, r = x_j - x_i, w = v_j - v_i, s = r.r + eps2:
+ *
+ *     acc_i  =  sum_j m_j r s^(-3/2)
+ *     jerk_i =  sum_j m_j [ w s^(-3/2) - 3 (r.w) r s^(-5/2) ]
+ *     pot_i  = -sum_j m_j s^(-1/2)
+ *
+ * over all j in [0, n_j) except the i-particle's own j entry; with NBK_EPS0 pairs with
+ * s == 0 contribute nothing.  Pairwise arithmetic is fp32 (FMA + rsqrt.approx), partial
+ * sums are folded in fp64 on the device, results are returned in fp32.
+ *
+ * Conventions
+ *   - Every function returns NBK_OK (0) or a negative nbk_status; nothing throws or aborts.
+ *     NaN/Inf in results is not an error.  After NBK_ECUDA, nbk_last_cuda_error() gives the
+ *     cudaError_t value.
+ *   - "host" pointers are ordinary host memory (pageable is fine; the library stages through
+ *     its own pinned buffers).  "device" pointers (functions ending in _dev) are device
+ *     memory on the context's device; the library only enqueues work on the context's
+ *     stream and does not synchronise.
+ *   - The caller owns every array it passes.  Host arrays may be reused as soon as the call
+ *     returns; device arrays once the work enqueued on the stream has run.
+ *   - Vectors are row-major [n][3], C order.
+ *   - One context = one device = one stream = one caller thread at a time.
+ */
+#ifndef NBK_H_
+#define NBK_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nbk_ctx nbk_ctx;
+
+typedef enum nbk_status {
+    NBK_OK = 0,
+    NBK_EINVAL = -1,  /* NULL / negative / inconsistent argument */
+    NBK_ERANGE = -2,  /* address, n_j or n_i beyond what the context was opened for */
+    NBK_ENOMEM = -3,  /* host or device allocation failed */
+    NBK_ECUDA = -4,   /* a CUDA call failed: see nbk_last_cuda_error() */
+    NBK_ESTATE = -5   /* call order violated (e.g. lasthalf with no firsthalf in flight) */
+} nbk_status;
+
+/* flags of nbk_calc_firsthalf */
+#define NBK_JERK 1u /* also compute the jerk (needs v of the j-particles)                */
+#define NBK_POT 2u  /* kept for GRAPE-style callers: the potential is always computed    */
+#define NBK_EPS0 4u /* mask pairs with s == 0; forced on if eps2==0 */
+
+/* ---- life cycle (GPU_open / GPU_close / GPU_npipes) ----------------- */
+
+/* Create a context on CUDA device `device` able to hold n_max j-particles and to serve up to
+ * ni_max i-particles per call.  `cuda_stream` is a cudaStream_t (e.g. a torch stream's
+ * .cuda_stream) on which all work is enqueued; NULL = the library creates its own stream.
+ * All device and pinned memory is allocated here, none later. */
+int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cuda_stream);
+
+/* Free everything the context owns (waits for its stream first).  NULL is accepted. */
+int nbk_close(nbk_ctx* ctx);
+
+/* GRAPE callers ask how many i-particles one call takes (48 on GRAPE-6Af, L102; "can be
+ * configured", L426).  Here any n_i <= ni_max is accepted; this returns ni_max clipped to
+ * INT_MAX.  Negative nbk_status on a NULL context. */
+int nbk_npipes(const nbk_ctx* ctx);
+
+/* ---- a1: load j-particles (GPU_set_j_particle, L427; batched) ---------------------------- */
+
+/* Store n particles into the device j-state at addresses addr[k] (NULL: k itself), each
+ * 0 <= addr < n_max.  tj[n] last-update times (NULL: 0), m[n], x[n][3], v[n][3] (NULL: 0),
+ * a[n][3], jerk[n][3] (NULL: 0, i.e. the particle is not moved by the predictor).
+ * Positions are kept in fp64 on the device so the predictor rounds once; the _f64 form takes
+ * double x, v straight from an fp64 integrator.  Host pointers.  The copy is asynchronous on
+ * the context's stream from a pinned staging buffer the library owns. */
+int nbk_set_j_particles(nbk_ctx* ctx, int64_t n, const int32_t* addr, const double* tj,
+                        const float* m, const float* x, const float* v, const float* a,
+                        const float* jerk);
+int nbk_set_j_particles_f64(nbk_ctx* ctx, int64_t n, const int32_t* addr, const double* tj,
+                            const double* m, const double* x, const double* v, const double* a,
+                            const double* jerk);
+/* Same as nbk_set_j_particles with DEVICE pointers; nothing is staged, nothing synchronises. */
+int nbk_set_j_particles_dev(nbk_ctx* ctx, int64_t n, const int32_t* addr, const double* tj,
+                            const float* m, const float* x, const float* v, const float* a,
+                            const float* jerk);
+
+/* ---- a2/a3: set time and predict (GPU_set_ti, L428; predictor L68, reading R8) ---------- */
+
+/* Record the time t to which j-particles are predicted.  Cheap: marks the predicted state
+ * stale; the predictor kernel runs on the device at the next nbk_predict / firsthalf. */
+int nbk_set_ti(nbk_ctx* ctx, double t);
+
+/* Run the predictor now for j in [0, n_j):  dt = t - tj (fp64),
+ *   x_p = x + v dt + a dt^2/2 + jerk dt^3/6,  v_p = v + a dt + jerk dt^2/2,
+ * evaluated in fp64 and rounded once to the fp32 arrays the force kernel reads.
+ * firsthalf calls this itself when the predicted state is stale. */
+int nbk_predict(nbk_ctx* ctx, int64_t n_j);
+
+/* Read back the predicted fp32 state (host pointers, any may be NULL); synchronises.
+ * For tests of a3 and for callers that want the positions the forces were evaluated at. */
+int nbk_get_predicted(nbk_ctx* ctx, int64_t n_j, float* m, float* x, float* v);
+
+/* ---- a4-a6: force on a block of i-particles (GPUcalc_firsthalf, L429) -------------------- */
+
+/* Enqueue prediction (if stale), the i x j force kernel and the split-j reduction for n_i
+ * i-particles against j-particles [0, n_j).  Asynchronous: returns once the work is queued.
+ *   i_index[n_i]  i_index[k] >= 0: i-particle k is j-particle i_index[k]; its predicted
+ *                 state is gathered on the device and its own j entry is left out of the
+ *                 sums.  -1: external test particle (needs xi; no j is left out).
+ *                 NULL: i_index[k] = k.
+ *   xi, vi        optional [n_i][3] explicit i-state overriding the gathered one (vi NULL:
+ *                 gathered velocity, or 0 for external particles).
+ *   eps2          softening length squared (>= 0).
+ *   flags         NBK_JERK | NBK_POT | NBK_EPS0.
+ * Host pointers (copied before return). */
+int nbk_calc_firsthalf(nbk_ctx* ctx, int64_t n_j, int64_t n_i, const int32_t* i_index,
+                       const float* xi, const float* vi, float eps2, uint32_t flags);
+/* Same with DEVICE pointers, which must stay valid until the enqueued work has run. */
+int nbk_calc_firsthalf_dev(nbk_ctx* ctx, int64_t n_j, int64_t n_i, const int32_t* i_index,
+                           const float* xi, const float* vi, float eps2, uint32_t flags);
+
+/* ---- a7: read back (GPUcalc_lasthalf, L430) ----------------------------------------------- */
+
+/* Wait for the last firsthalf and copy acc[n_i][3], jerk[n_i][3], pot[n_i] to HOST arrays
+ * (any may be NULL; jerk is zero if NBK_JERK was not set).  n_i must equal firsthalf's. */
+int nbk_calc_lasthalf(nbk_ctx* ctx, int64_t n_i, float* acc, float* jerk, float* pot);
+/* Same to DEVICE arrays, asynchronous on the stream, no synchronisation. */
+int nbk_calc_lasthalf_dev(nbk_ctx* ctx, int64_t n_i, float* acc, float* jerk, float* pot);
+
+/* ---- a8: host Hermite driver (reading R15) ------------------- */
+
+typedef struct nbk_hermite_stats {
+    int64_t block_steps;      /* force calls made                                    */
+    int64_t particle_steps;   /* sum of n_i over block steps                         */
+    int64_t interactions;     /* sum of n_i * n over block steps                     */
+    double wall_seconds;      /* whole run, host clock                               */
+    double gpu_call_seconds;  /* host time spent inside nbk_* calls (incl. waiting)  */
+    double t_reached;
+    int64_t ni_histogram[32]; /* bucket b counts block steps with 2^b <= n_i < 2^(b+1) */
+} nbk_hermite_stats;
+
+/* Integrate n particles from t = 0 to t_end with the 4th-order Hermite predictor-corrector,
+ * power-of-two block time steps and the Aarseth criterion (eta, dt_max), host arithmetic in
+ * fp64, forces from this context (which must have n_max >= n, ni_max >= n).
+ * m[n], x[n][3], v[n][3] are HOST fp64 arrays, updated in place to the state at t_end
+ * (t_end must be a multiple of dt_max so that all particles are synchronised there).
+ * stats may be NULL. */
+int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, double* x, double* v,
+                       double eps, double t_end, double eta, double dt_max,
+                       nbk_hermite_stats* stats);
+
+/* ---- utilities --------------------------------------------------------------------------- */
+
+/* Block until everything enqueued on the context's stream has run. */
+int nbk_sync(nbk_ctx* ctx);
+
+/* Kernel timing: when enabled, firsthalf/predict record CUDA events around each kernel on
+ * the context's stream.  nbk_get_timing waits for them and returns the durations, in
+ * milliseconds, of the LAST call's kernels: ms[0] scatter (set_j), ms[1] predict,
+ * ms[2] i x j force tile, ms[3] reduce.  A kernel that did not run reports 0. */
+int nbk_set_timing(nbk_ctx* ctx, int enable);
+int nbk_get_timing(nbk_ctx* ctx, float ms[4]);
+
+/* Launch shape of the last firsthalf: out[0] grid (CTAs), out[1] threads per CTA,
+ * out[2] i-particles per thread, out[3] warps splitting each j-tile, out[4] CTAs per SM the
+ * grid was sized for, out[5] SM count, out[6] dynamic shared memory bytes,
+ * out[7] number of kernels launched by the last firsthalf. */
+int nbk_last_launch(const nbk_ctx* ctx, int64_t out[8]);
+
+/* Choose the inner-loop form: 0 = packed f32x2 (FFMA2, two j per instruction; default),
+ * 1 = scalar fp32.  Both compute the same sums; kept for measurement. */
+int nbk_set_variant(nbk_ctx* ctx, int variant);
+
+int nbk_last_cuda_error(const nbk_ctx* ctx);
+const char* nbk_strerror(int status);
+const char* nbk_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NBK_H_ */

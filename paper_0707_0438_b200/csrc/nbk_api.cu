@@ -1,0 +1,598 @@
+// nbk_api.cu -- the C ABI of include/nbk.h: context, workspaces, staging and launch logic.
+// Every step of the path runs in the kernels of nbk_kernels.cu; this file only moves
+// arguments, picks the launch shape and enqueues.  There is no CPU fallback: without a CUDA
+// device nbk_open fails with NBK_ECUDA.
+#include <cuda_runtime.h>
+
+#include <climits>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/nbk.h"
+#include "nbk_kernels.cuh"
+
+using namespace nbk;
+
+namespace {
+
+constexpr int kNumVariants = 24;
+
+inline int variant_key(const Variant& v) {
+    return (v.I == 1 ? 0 : v.I == 2 ? 1 : 2) * 8 + (v.jerk ? 4 : 0) + (v.eps0 ? 2 : 0) +
+           (v.packed ? 1 : 0);
+}
+
+inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
+
+struct DeviceGuard {  // make the context's device current for the call, restore on exit
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != dev) ok = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        int cur = -1;
+        if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+    }
+};
+
+}  // namespace
+
+struct nbk_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    long long n_max = 0, ni_max = 0, n_cap = 0;
+    int num_sms = 0;
+    int occ[kNumVariants];
+
+    RawJ raw{};
+    float* pred = nullptr;  // 7 arrays of n_cap floats: x y z m vx vy vz
+    double t = 0.0;
+    bool pred_valid = false;
+    long long pred_nj = -1;
+
+    int32_t* d_iidx = nullptr;
+    float* d_xi = nullptr;
+    float* d_vi = nullptr;
+    float* d_partial = nullptr;
+    size_t partial_bytes = 0;
+    float* d_result = nullptr;  // acc[3 n_i] | jerk[3 n_i] | pot[n_i] of the last call
+    float* h_result = nullptr;  // pinned
+
+    unsigned char* h_stage = nullptr;  // pinned staging for set_j
+    unsigned char* d_stage = nullptr;
+    size_t stage_bytes = 0;
+    cudaEvent_t stage_free = nullptr;  // recorded after the H2D that reads h_stage
+    unsigned char* h_istage = nullptr;  // pinned staging for i_index / xi / vi
+    cudaEvent_t istage_free = nullptr;
+
+    long long last_ni = -1;
+    bool in_flight = false;
+    int variant_scalar = 0;
+    int force_I = 0;
+    int last_cuda = 0;
+    long long last_launch[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+
+    bool timing = false;
+    cudaEvent_t ev[4][2];
+    bool ev_used[4] = {false, false, false, false};
+};
+
+namespace {
+
+int cuda_fail(nbk_ctx* c, cudaError_t e) {
+    c->last_cuda = static_cast<int>(e);
+    (void)cudaGetLastError();
+    return NBK_ECUDA;
+}
+
+#define NBK_CUDA(c, call)                                   \
+    do {                                                    \
+        cudaError_t e__ = (call);                           \
+        if (e__ != cudaSuccess) return cuda_fail((c), e__); \
+    } while (0)
+
+struct TimeScope {  // CUDA events around one kernel on the context's stream
+    nbk_ctx* c;
+    int slot;
+    TimeScope(nbk_ctx* c_, int slot_) : c(c_), slot(slot_) {
+        if (c->timing) { cudaEventRecord(c->ev[slot][0], c->stream); c->ev_used[slot] = true; }
+    }
+    ~TimeScope() {
+        if (c->timing) cudaEventRecord(c->ev[slot][1], c->stream);
+    }
+};
+
+float* pred_arr(const nbk_ctx* c, int k) { return c->pred + static_cast<size_t>(k) * c->n_cap; }
+
+JPred jpred_of(const nbk_ctx* c) {
+    JPred j;
+    j.x = pred_arr(c, 0); j.y = pred_arr(c, 1); j.z = pred_arr(c, 2); j.m = pred_arr(c, 3);
+    j.vx = pred_arr(c, 4); j.vy = pred_arr(c, 5); j.vz = pred_arr(c, 6);
+    return j;
+}
+
+void free_all(nbk_ctx* c) {
+    cudaFree(c->raw.x); cudaFree(c->raw.v); cudaFree(c->raw.a); cudaFree(c->raw.k);
+    cudaFree(c->raw.m); cudaFree(c->raw.t); cudaFree(c->pred);
+    cudaFree(c->d_iidx); cudaFree(c->d_xi); cudaFree(c->d_vi);
+    cudaFree(c->d_partial); cudaFree(c->d_result); cudaFree(c->d_stage);
+    if (c->h_result) cudaFreeHost(c->h_result);
+    if (c->h_stage) cudaFreeHost(c->h_stage);
+    if (c->h_istage) cudaFreeHost(c->h_istage);
+    if (c->stage_free) cudaEventDestroy(c->stage_free);
+    if (c->istage_free) cudaEventDestroy(c->istage_free);
+    for (int s = 0; s < 4; ++s)
+        for (int e = 0; e < 2; ++e)
+            if (c->ev[s][e]) cudaEventDestroy(c->ev[s][e]);
+    if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
+    (void)cudaGetLastError();
+}
+
+int do_predict(nbk_ctx* c, long long n_j) {
+    const long long n_pad = round_up(n_j, kTileJ);
+    TimeScope ts(c, 1);
+    NBK_CUDA(c, launch_predict(c->raw, c->t, n_j, n_pad, pred_arr(c, 0), pred_arr(c, 1),
+                               pred_arr(c, 2), pred_arr(c, 3), pred_arr(c, 4), pred_arr(c, 5),
+                               pred_arr(c, 6), c->stream));
+    c->pred_valid = true;
+    c->pred_nj = n_j;
+    return NBK_OK;
+}
+
+// Launch shape for (n_i, n_j): which kernel instantiation, how i-tiles and j-tiles are cut.
+void choose_shape(const nbk_ctx* c, long long n_i, long long n_j, uint32_t flags, float eps2,
+                  Variant* v, Decomp* d) {
+    v->jerk = (flags & NBK_JERK) != 0;
+    v->eps0 = (flags & NBK_EPS0) != 0 || eps2 == 0.f;
+    v->packed = c->variant_scalar == 0;
+    int wj = 1, I = 1;
+    if (n_i <= 32) wj = 4;
+    else if (n_i <= 64) wj = 2;
+    else if (n_i >= 4096) I = 2;
+    if (c->force_I > 0 && wj == 1) I = c->force_I;
+    v->I = I;
+    d->n_i = static_cast<int>(n_i);
+    d->wj = wj;
+    d->ti = (kWarps / wj) * 32 * I;
+    d->nit = static_cast<int>((n_i + d->ti - 1) / d->ti);
+    d->njt = static_cast<int>(round_up(n_j, kTileJ) / kTileJ);
+    d->P = static_cast<long long>(d->nit) * d->njt;
+    const long long slots = static_cast<long long>(c->num_sms) * c->occ[variant_key(*v)];
+    d->G = static_cast<int>(d->P < slots ? d->P : slots);
+    const long long W = (d->P + d->G - 1) / d->G;
+    d->maxseg = static_cast<int>((W - 1 + d->njt - 1) / d->njt + 1);
+}
+
+int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iidx,
+                  const float* d_xi, const float* d_vi, float eps2, uint32_t flags) {
+    if (!c->pred_valid || c->pred_nj != n_j) {
+        const int rc = do_predict(c, n_j);
+        if (rc != NBK_OK) return rc;
+    }
+    float* acc = c->d_result;
+    float* jerk = acc + 3 * n_i;
+    float* pot = acc + 6 * n_i;
+    c->last_ni = n_i;
+    c->in_flight = true;
+    if (n_i == 0) return NBK_OK;
+    if (n_j == 0) {
+        NBK_CUDA(c, cudaMemsetAsync(acc, 0, sizeof(float) * 7 * n_i, c->stream));
+        c->last_launch[7] = 0;
+        return NBK_OK;
+    }
+    Variant v;
+    Decomp d;
+    choose_shape(c, n_i, n_j, flags, eps2, &v, &d);
+    const size_t need = static_cast<size_t>(d.G) * d.maxseg * d.wj * d.ti * 8 * sizeof(float);
+    if (need > c->partial_bytes) return NBK_ENOMEM;
+
+    ForceArgs fa;
+    fa.j = jpred_of(c);
+    fa.i_index = d_iidx; fa.xi = d_xi; fa.vi = d_vi;
+    fa.partial = c->d_partial;
+    fa.eps2 = eps2;
+    fa.d = d;
+    {
+        TimeScope ts(c, 2);
+        NBK_CUDA(c, launch_force(v, fa, c->stream));
+    }
+    ReduceArgs ra;
+    ra.j = fa.j;
+    ra.i_index = d_iidx; ra.xi = d_xi; ra.vi = d_vi;
+    ra.partial = c->d_partial;
+    ra.acc = acc; ra.jerk = jerk; ra.pot = pot;
+    ra.eps2 = eps2;
+    ra.d = d;
+    {
+        TimeScope ts(c, 3);
+        NBK_CUDA(c, launch_reduce(v, ra, c->stream));
+    }
+    c->last_launch[0] = d.G;
+    c->last_launch[1] = kThreads;
+    c->last_launch[2] = v.I;
+    c->last_launch[3] = d.wj;
+    c->last_launch[4] = c->occ[variant_key(v)];
+    c->last_launch[5] = c->num_sms;
+    c->last_launch[6] = static_cast<long long>(force_smem_bytes(v));
+    c->last_launch[7] = 2;
+    return NBK_OK;
+}
+
+template <typename T>
+int set_j_host(nbk_ctx* c, long long n, const int32_t* addr, const double* tj, const T* m,
+               const T* x, const T* v, const T* a, const T* jerk) {
+    if (!c || n < 0 || (n > 0 && (!m || !x))) return NBK_EINVAL;
+    if (n > c->n_max) return NBK_ERANGE;
+    if (addr)
+        for (long long k = 0; k < n; ++k)
+            if (addr[k] < 0 || addr[k] >= c->n_max) return NBK_ERANGE;
+    if (n == 0) return NBK_OK;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    NBK_CUDA(c, cudaEventSynchronize(c->stage_free));
+    // pack [tj | m | x | v | a | jerk | addr] into the pinned buffer: one H2D copy
+    size_t off = 0;
+    auto put = [&](const void* src, size_t bytes) -> size_t {
+        const size_t at = off;
+        if (src) std::memcpy(c->h_stage + at, src, bytes);
+        off += (bytes + 15) & ~static_cast<size_t>(15);
+        return at;
+    };
+    const size_t o_t = put(tj, sizeof(double) * n);
+    const size_t o_m = put(m, sizeof(T) * n);
+    const size_t o_x = put(x, sizeof(T) * 3 * n);
+    const size_t o_v = put(v, sizeof(T) * 3 * n);
+    const size_t o_a = put(a, sizeof(T) * 3 * n);
+    const size_t o_k = put(jerk, sizeof(T) * 3 * n);
+    const size_t o_ad = put(addr, sizeof(int32_t) * n);
+    if (off > c->stage_bytes) return NBK_ENOMEM;
+    NBK_CUDA(c, cudaMemcpyAsync(c->d_stage, c->h_stage, off, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaEventRecord(c->stage_free, c->stream));
+    ScatterArgs s;
+    s.n = n;
+    s.addr = addr ? reinterpret_cast<const int32_t*>(c->d_stage + o_ad) : nullptr;
+    s.tj = tj ? reinterpret_cast<const double*>(c->d_stage + o_t) : nullptr;
+    s.m = c->d_stage + o_m;
+    s.x = c->d_stage + o_x;
+    s.v = v ? c->d_stage + o_v : nullptr;
+    s.a = a ? c->d_stage + o_a : nullptr;
+    s.k = jerk ? c->d_stage + o_k : nullptr;
+    s.f64 = sizeof(T) == sizeof(double);
+    s.n_max = c->n_max;
+    {
+        TimeScope ts(c, 0);
+        NBK_CUDA(c, launch_scatter(s, c->raw, c->stream));
+    }
+    c->pred_valid = false;
+    return NBK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cuda_stream) {
+    if (!out || n_max < 1 || ni_max < 1 || n_max > (1LL << 30) || ni_max > (1LL << 30))
+        return NBK_EINVAL;
+    *out = nullptr;
+    nbk_ctx* c = new (std::nothrow) nbk_ctx();
+    if (!c) return NBK_ENOMEM;
+    std::memset(c->ev, 0, sizeof(c->ev));
+    c->device = device;
+    int rc = NBK_OK;
+    auto fail = [&](int code, cudaError_t e) {
+        if (code == NBK_ECUDA) c->last_cuda = static_cast<int>(e);
+        rc = code;
+    };
+    DeviceGuard g(device);
+    cudaError_t e = g.ok ? cudaSuccess : cudaErrorInvalidDevice;
+    do {
+        if (e != cudaSuccess) break;
+        cudaDeviceProp prop;
+        if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) break;
+        if (prop.major < 10) { e = cudaErrorNoKernelImageForDevice; break; }
+        c->num_sms = prop.multiProcessorCount;
+        if (cuda_stream) {
+            c->stream = static_cast<cudaStream_t>(cuda_stream);
+        } else {
+            if ((e = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking)) != cudaSuccess) break;
+            c->own_stream = true;
+        }
+        c->n_max = n_max;
+        c->ni_max = ni_max;
+        c->n_cap = round_up(n_max, kTileJ);
+        c->raw.cap = c->n_cap;
+        int max_occ = 1;
+        for (int I : {1, 2, 4})
+            for (int jk = 0; jk < 2 && e == cudaSuccess; ++jk)
+                for (int e0 = 0; e0 < 2 && e == cudaSuccess; ++e0)
+                    for (int pk = 0; pk < 2 && e == cudaSuccess; ++pk) {
+                        Variant v{I, jk != 0, e0 != 0, pk != 0};
+                        const int o = force_occupancy(v, &e);
+                        if (e == cudaSuccess && o < 1) e = cudaErrorLaunchOutOfResources;
+                        c->occ[variant_key(v)] = o;
+                        if (o > max_occ) max_occ = o;
+                    }
+        if (e != cudaSuccess) break;
+        const size_t cap = static_cast<size_t>(c->n_cap);
+        if ((e = cudaMalloc(&c->raw.x, sizeof(double) * 3 * cap)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->raw.v, sizeof(float) * 3 * cap)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->raw.a, sizeof(float) * 3 * cap)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->raw.k, sizeof(float) * 3 * cap)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->raw.m, sizeof(float) * cap)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->raw.t, sizeof(double) * cap)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->pred, sizeof(float) * 7 * cap)) != cudaSuccess) break;
+        if ((e = cudaMemsetAsync(c->raw.x, 0, sizeof(double) * 3 * cap, c->stream)) != cudaSuccess) break;
+        if ((e = cudaMemsetAsync(c->raw.v, 0, sizeof(float) * 3 * cap, c->stream)) != cudaSuccess) break;
+        if ((e = cudaMemsetAsync(c->raw.a, 0, sizeof(float) * 3 * cap, c->stream)) != cudaSuccess) break;
+        if ((e = cudaMemsetAsync(c->raw.k, 0, sizeof(float) * 3 * cap, c->stream)) != cudaSuccess) break;
+        if ((e = cudaMemsetAsync(c->raw.m, 0, sizeof(float) * cap, c->stream)) != cudaSuccess) break;
+        if ((e = cudaMemsetAsync(c->raw.t, 0, sizeof(double) * cap, c->stream)) != cudaSuccess) break;
+        if ((e = cudaMemsetAsync(c->pred, 0, sizeof(float) * 7 * cap, c->stream)) != cudaSuccess) break;
+        const size_t ni = static_cast<size_t>(ni_max);
+        if ((e = cudaMalloc(&c->d_iidx, sizeof(int32_t) * ni)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_xi, sizeof(float) * 3 * ni)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_vi, sizeof(float) * 3 * ni)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_result, sizeof(float) * 7 * ni)) != cudaSuccess) break;
+        if ((e = cudaMallocHost(&c->h_result, sizeof(float) * 7 * ni)) != cudaSuccess) break;
+        // partial rows: at most (n_i rounded to a tile) + 3 tiles per CTA of slack
+        const size_t g_max = static_cast<size_t>(c->num_sms) * max_occ;
+        c->partial_bytes = 8 * sizeof(float) * (ni + 32 * kMaxI * kWarps * (1 + 3 * g_max));
+        if ((e = cudaMalloc(&c->d_partial, c->partial_bytes)) != cudaSuccess) break;
+        c->stage_bytes = static_cast<size_t>(n_max) * (8 + 8 + 4 * 24 + 4) + 16 * 8;
+        if ((e = cudaMallocHost(&c->h_stage, c->stage_bytes)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_stage, c->stage_bytes)) != cudaSuccess) break;
+        if ((e = cudaMallocHost(&c->h_istage, ni * 28 + 64)) != cudaSuccess) break;
+        if ((e = cudaEventCreateWithFlags(&c->stage_free, cudaEventDisableTiming)) != cudaSuccess) break;
+        if ((e = cudaEventCreateWithFlags(&c->istage_free, cudaEventDisableTiming)) != cudaSuccess) break;
+        if ((e = cudaEventRecord(c->stage_free, c->stream)) != cudaSuccess) break;
+        if ((e = cudaEventRecord(c->istage_free, c->stream)) != cudaSuccess) break;
+        for (int s = 0; s < 4 && e == cudaSuccess; ++s)
+            for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaEventCreate(&c->ev[s][k]);
+        if (e != cudaSuccess) break;
+        e = cudaStreamSynchronize(c->stream);
+    } while (false);
+    if (e != cudaSuccess)
+        fail(e == cudaErrorMemoryAllocation ? NBK_ENOMEM : NBK_ECUDA, e);
+    if (rc != NBK_OK) {
+        free_all(c);
+        delete c;
+        return rc;
+    }
+    *out = c;
+    return NBK_OK;
+}
+
+int nbk_close(nbk_ctx* c) {
+    if (!c) return NBK_OK;
+    DeviceGuard g(c->device);
+    if (c->stream) cudaStreamSynchronize(c->stream);
+    free_all(c);
+    delete c;
+    return NBK_OK;
+}
+
+int nbk_npipes(const nbk_ctx* c) {
+    if (!c) return NBK_EINVAL;
+    return c->ni_max > INT_MAX ? INT_MAX : static_cast<int>(c->ni_max);
+}
+
+int nbk_set_j_particles(nbk_ctx* c, int64_t n, const int32_t* addr, const double* tj,
+                        const float* m, const float* x, const float* v, const float* a,
+                        const float* jerk) {
+    return set_j_host<float>(c, n, addr, tj, m, x, v, a, jerk);
+}
+
+int nbk_set_j_particles_f64(nbk_ctx* c, int64_t n, const int32_t* addr, const double* tj,
+                            const double* m, const double* x, const double* v, const double* a,
+                            const double* jerk) {
+    return set_j_host<double>(c, n, addr, tj, m, x, v, a, jerk);
+}
+
+int nbk_set_j_particles_dev(nbk_ctx* c, int64_t n, const int32_t* addr, const double* tj,
+                            const float* m, const float* x, const float* v, const float* a,
+                            const float* jerk) {
+    if (!c || n < 0 || (n > 0 && (!m || !x))) return NBK_EINVAL;
+    if (n > c->n_max) return NBK_ERANGE;
+    if (n == 0) return NBK_OK;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    ScatterArgs s;
+    s.n = n; s.addr = addr; s.tj = tj; s.m = m; s.x = x; s.v = v; s.a = a; s.k = jerk;
+    s.f64 = 0;
+    s.n_max = c->n_max;
+    {
+        TimeScope ts(c, 0);
+        NBK_CUDA(c, launch_scatter(s, c->raw, c->stream));
+    }
+    c->pred_valid = false;
+    return NBK_OK;
+}
+
+int nbk_set_ti(nbk_ctx* c, double t) {
+    if (!c) return NBK_EINVAL;
+    if (!(t == t)) return NBK_EINVAL;
+    if (t != c->t) c->pred_valid = false;
+    c->t = t;
+    return NBK_OK;
+}
+
+int nbk_predict(nbk_ctx* c, int64_t n_j) {
+    if (!c || n_j < 0) return NBK_EINVAL;
+    if (n_j > c->n_max) return NBK_ERANGE;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    return do_predict(c, n_j);
+}
+
+int nbk_get_predicted(nbk_ctx* c, int64_t n_j, float* m, float* x, float* v) {
+    if (!c || n_j < 0) return NBK_EINVAL;
+    if (n_j > c->n_max) return NBK_ERANGE;
+    if (!c->pred_valid || c->pred_nj < n_j) return NBK_ESTATE;
+    if (n_j == 0) return NBK_OK;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    std::vector<float> tmp;
+    try {
+        tmp.resize(static_cast<size_t>(7) * n_j);
+    } catch (...) {
+        return NBK_ENOMEM;
+    }
+    for (int k = 0; k < 7; ++k)
+        NBK_CUDA(c, cudaMemcpyAsync(tmp.data() + static_cast<size_t>(k) * n_j, pred_arr(c, k),
+                                    sizeof(float) * n_j, cudaMemcpyDeviceToHost, c->stream));
+    NBK_CUDA(c, cudaStreamSynchronize(c->stream));
+    const size_t n = static_cast<size_t>(n_j);
+    for (size_t j = 0; j < n; ++j) {
+        if (x) { x[3 * j] = tmp[j]; x[3 * j + 1] = tmp[n + j]; x[3 * j + 2] = tmp[2 * n + j]; }
+        if (m) m[j] = tmp[3 * n + j];
+        if (v) { v[3 * j] = tmp[4 * n + j]; v[3 * j + 1] = tmp[5 * n + j]; v[3 * j + 2] = tmp[6 * n + j]; }
+    }
+    return NBK_OK;
+}
+
+int nbk_calc_firsthalf(nbk_ctx* c, int64_t n_j, int64_t n_i, const int32_t* i_index,
+                       const float* xi, const float* vi, float eps2, uint32_t flags) {
+    if (!c || n_j < 0 || n_i < 0 || !(eps2 >= 0.f)) return NBK_EINVAL;
+    if (n_j > c->n_max || n_i > c->ni_max) return NBK_ERANGE;
+    if (i_index) {
+        for (int64_t k = 0; k < n_i; ++k) {
+            if (i_index[k] < -1 || i_index[k] >= n_j) return NBK_ERANGE;
+            if (i_index[k] < 0 && !xi) return NBK_EINVAL;
+        }
+    } else if (n_i > n_j) {
+        return NBK_ERANGE;
+    }
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    const int32_t* d_ii = nullptr;
+    const float* d_x = nullptr;
+    const float* d_v = nullptr;
+    if (n_i > 0 && (i_index || xi || vi)) {
+        NBK_CUDA(c, cudaEventSynchronize(c->istage_free));
+        const size_t ni = static_cast<size_t>(n_i);
+        unsigned char* h = c->h_istage;
+        if (i_index) {
+            std::memcpy(h, i_index, 4 * ni);
+            NBK_CUDA(c, cudaMemcpyAsync(c->d_iidx, h, 4 * ni, cudaMemcpyHostToDevice, c->stream));
+            d_ii = c->d_iidx;
+        }
+        h += (4 * ni + 15) & ~static_cast<size_t>(15);
+        if (xi) {
+            std::memcpy(h, xi, 12 * ni);
+            NBK_CUDA(c, cudaMemcpyAsync(c->d_xi, h, 12 * ni, cudaMemcpyHostToDevice, c->stream));
+            d_x = c->d_xi;
+        }
+        h += (12 * ni + 15) & ~static_cast<size_t>(15);
+        if (vi) {
+            std::memcpy(h, vi, 12 * ni);
+            NBK_CUDA(c, cudaMemcpyAsync(c->d_vi, h, 12 * ni, cudaMemcpyHostToDevice, c->stream));
+            d_v = c->d_vi;
+        }
+        NBK_CUDA(c, cudaEventRecord(c->istage_free, c->stream));
+    }
+    return enqueue_force(c, n_j, n_i, d_ii, d_x, d_v, eps2, flags);
+}
+
+int nbk_calc_firsthalf_dev(nbk_ctx* c, int64_t n_j, int64_t n_i, const int32_t* i_index,
+                           const float* xi, const float* vi, float eps2, uint32_t flags) {
+    if (!c || n_j < 0 || n_i < 0 || !(eps2 >= 0.f)) return NBK_EINVAL;
+    if (n_j > c->n_max || n_i > c->ni_max) return NBK_ERANGE;
+    if (!i_index && n_i > n_j) return NBK_ERANGE;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    return enqueue_force(c, n_j, n_i, i_index, xi, vi, eps2, flags);
+}
+
+int nbk_calc_lasthalf(nbk_ctx* c, int64_t n_i, float* acc, float* jerk, float* pot) {
+    if (!c || n_i < 0) return NBK_EINVAL;
+    if (!c->in_flight || n_i != c->last_ni) return NBK_ESTATE;
+    if (n_i == 0) return NBK_OK;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    const size_t ni = static_cast<size_t>(n_i);
+    NBK_CUDA(c, cudaMemcpyAsync(c->h_result, c->d_result, sizeof(float) * 7 * ni,
+                                cudaMemcpyDeviceToHost, c->stream));
+    NBK_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (acc) std::memcpy(acc, c->h_result, sizeof(float) * 3 * ni);
+    if (jerk) std::memcpy(jerk, c->h_result + 3 * ni, sizeof(float) * 3 * ni);
+    if (pot) std::memcpy(pot, c->h_result + 6 * ni, sizeof(float) * ni);
+    return NBK_OK;
+}
+
+int nbk_calc_lasthalf_dev(nbk_ctx* c, int64_t n_i, float* acc, float* jerk, float* pot) {
+    if (!c || n_i < 0) return NBK_EINVAL;
+    if (!c->in_flight || n_i != c->last_ni) return NBK_ESTATE;
+    if (n_i == 0) return NBK_OK;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    const size_t ni = static_cast<size_t>(n_i);
+    if (acc) NBK_CUDA(c, cudaMemcpyAsync(acc, c->d_result, sizeof(float) * 3 * ni, cudaMemcpyDeviceToDevice, c->stream));
+    if (jerk) NBK_CUDA(c, cudaMemcpyAsync(jerk, c->d_result + 3 * ni, sizeof(float) * 3 * ni, cudaMemcpyDeviceToDevice, c->stream));
+    if (pot) NBK_CUDA(c, cudaMemcpyAsync(pot, c->d_result + 6 * ni, sizeof(float) * ni, cudaMemcpyDeviceToDevice, c->stream));
+    return NBK_OK;
+}
+
+int nbk_sync(nbk_ctx* c) {
+    if (!c) return NBK_EINVAL;
+    DeviceGuard g(c->device);
+    NBK_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NBK_OK;
+}
+
+int nbk_set_timing(nbk_ctx* c, int enable) {
+    if (!c) return NBK_EINVAL;
+    c->timing = enable != 0;
+    for (int s = 0; s < 4; ++s) c->ev_used[s] = false;
+    return NBK_OK;
+}
+
+int nbk_get_timing(nbk_ctx* c, float ms[4]) {
+    if (!c || !ms) return NBK_EINVAL;
+    DeviceGuard g(c->device);
+    NBK_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int s = 0; s < 4; ++s) {
+        ms[s] = 0.f;
+        if (c->ev_used[s]) NBK_CUDA(c, cudaEventElapsedTime(&ms[s], c->ev[s][0], c->ev[s][1]));
+        c->ev_used[s] = false;
+    }
+    return NBK_OK;
+}
+
+int nbk_last_launch(const nbk_ctx* c, int64_t out[8]) {
+    if (!c || !out) return NBK_EINVAL;
+    for (int k = 0; k < 8; ++k) out[k] = c->last_launch[k];
+    return NBK_OK;
+}
+
+int nbk_set_variant(nbk_ctx* c, int variant) {
+    if (!c || variant < 0) return NBK_EINVAL;
+    const int I = (variant >> 4) & 15;
+    if (!(I == 0 || I == 1 || I == 2 || I == 4)) return NBK_EINVAL;
+    c->variant_scalar = variant & 1;
+    c->force_I = I;
+    return NBK_OK;
+}
+
+int nbk_last_cuda_error(const nbk_ctx* c) { return c ? c->last_cuda : 0; }
+
+const char* nbk_strerror(int status) {
+    switch (status) {
+        case NBK_OK: return "ok";
+        case NBK_EINVAL: return "invalid argument";
+        case NBK_ERANGE: return "address or count out of range for this context";
+        case NBK_ENOMEM: return "out of memory";
+        case NBK_ECUDA: return "CUDA error (see nbk_last_cuda_error)";
+        case NBK_ESTATE: return "call order violated";
+        default: return "unknown status";
+    }
+}
+
+const char* nbk_version(void) { return "nbk 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,221 @@
+// nbk_hermite.cpp -- a8: host-side 4th-order Hermite predictor-corrector with power-of-two
+// block time steps, driving the device force path through the public C ABI only.
+//
+// PAPER.md L68 ("4th order predictor-corrector Hermite ... a predictor step that predicts a
+// particle's position and velocity, then the acceleration, its time derivative (jerk) and
+// potential are computed by direct summation and a corrector step ..."), L72-L76 (corrector
+// and step selection stay on the host in fp64), L74 (block time steps).  The paper prints
+// none of the formulas; the ones below are DESIGN.md reading R15 (Makino & Aarseth 1992 form
+// of the corrector, Aarseth step criterion, McMillan & Aarseth block rule).
+//
+// Per block step (call stack (5) of SURVEY.md):  pick the due block -> nbk_set_ti ->
+// nbk_calc_firsthalf (device: predict all N, gather i, force, reduce) -> [host predicts the
+// block's own particles in fp64 while the device works] -> nbk_calc_lasthalf -> corrector +
+// new step on the host -> nbk_set_j_particles_f64 for the corrected particles only.
+// The scheduler is O(n_active) per step: particles are kept in one list per power-of-two
+// level; all particles of a level share their last-update time.
+#include <chrono>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+#include "../../include/nbk.h"
+
+namespace {
+
+constexpr int kTickLog2 = 52;  // time unit 2^-52: exact integer block times up to t = 2048
+constexpr int kMaxLevel = 48;  // finest allowed step 2^-48
+
+struct Clock {
+    std::chrono::steady_clock::time_point t0 = std::chrono::steady_clock::now();
+    double seconds() const {
+        return std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    }
+};
+
+inline double norm3(const double* a) { return std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]); }
+
+// largest level-step 2^-k <= want, clamped to [2^-kMaxLevel, 2^-kmin]
+inline int level_for(double want, int kmin) {
+    if (!(want > 0.0)) return kMaxLevel;
+    int e;
+    std::frexp(want, &e);           // want = f * 2^e, f in [0.5, 1)  =>  2^(e-1) <= want
+    int k = -(e - 1);
+    if (k < kmin) k = kmin;
+    if (k > kMaxLevel) k = kMaxLevel;
+    return k;
+}
+
+struct Levels {
+    std::vector<std::vector<int32_t>> list;
+    std::vector<int32_t> pos;
+    std::vector<int8_t> lev;
+    explicit Levels(int64_t n) : list(kMaxLevel + 1), pos(n, -1), lev(n, -1) {}
+    void insert(int32_t i, int k) {
+        lev[i] = static_cast<int8_t>(k);
+        pos[i] = static_cast<int32_t>(list[k].size());
+        list[k].push_back(i);
+    }
+    void remove(int32_t i) {
+        auto& l = list[lev[i]];
+        const int32_t p = pos[i], last = l.back();
+        l[p] = last;
+        pos[last] = p;
+        l.pop_back();
+    }
+    int finest() const {
+        for (int k = kMaxLevel; k >= 0; --k)
+            if (!list[k].empty()) return k;
+        return -1;
+    }
+};
+
+}  // namespace
+
+extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, double* x, double* v,
+                                  double eps, double t_end, double eta, double dt_max,
+                                  nbk_hermite_stats* stats) {
+    if (!ctx || n < 1 || !m || !x || !v || !(eps >= 0.0) || !(t_end >= 0.0) || !(eta > 0.0) ||
+        !(dt_max > 0.0) || n > INT32_MAX)
+        return NBK_EINVAL;
+    const int kmin = level_for(dt_max, -10);  // dt_max rounded down to a power of two
+    const double dtm = std::ldexp(1.0, -kmin);
+    if (t_end > 2047.0 || std::fmod(t_end, dtm) != 0.0) return NBK_EINVAL;
+    const int64_t T_end = static_cast<int64_t>(std::ldexp(t_end, kTickLog2));
+    const float eps2 = static_cast<float>(eps * eps);
+    const uint32_t flags = NBK_JERK | NBK_POT;
+
+    Clock wall;
+    double gpu_s = 0.0;
+    nbk_hermite_stats st;
+    std::memset(&st, 0, sizeof(st));
+
+    const size_t N = static_cast<size_t>(n);
+    std::vector<double> a(3 * N), jk(3 * N), tl(N, 0.0);
+    std::vector<float> fa(3 * N), fj(3 * N);
+    std::vector<int32_t> act;
+    act.reserve(N);
+    // packed per-block buffers for set_j
+    std::vector<double> bt(N), bm(N), bx(3 * N), bv(3 * N), ba(3 * N), bj(3 * N), xp(3 * N), vp(3 * N);
+    Levels L(n);
+    int rc;
+
+#define NBK_TIMED(call)                  \
+    do {                                 \
+        Clock c__;                       \
+        rc = (call);                     \
+        gpu_s += c__.seconds();          \
+        if (rc != NBK_OK) return rc;     \
+    } while (0)
+
+    // t = 0: load everything, forces on all particles, first steps
+    NBK_TIMED(nbk_set_j_particles_f64(ctx, n, nullptr, nullptr, m, x, v, nullptr, nullptr));
+    NBK_TIMED(nbk_set_ti(ctx, 0.0));
+    NBK_TIMED(nbk_calc_firsthalf(ctx, n, n, nullptr, nullptr, nullptr, eps2, flags));
+    NBK_TIMED(nbk_calc_lasthalf(ctx, n, fa.data(), fj.data(), nullptr));
+    st.interactions += n * n;
+    for (size_t i = 0; i < N; ++i) {
+        for (int c = 0; c < 3; ++c) { a[3 * i + c] = fa[3 * i + c]; jk[3 * i + c] = fj[3 * i + c]; }
+        const double na = norm3(&a[3 * i]), nj = norm3(&jk[3 * i]);
+        double want = dtm;
+        if (nj > 0.0 && na > 0.0) want = std::fmin(0.25 * eta * na / nj, dtm);
+        L.insert(static_cast<int32_t>(i), level_for(want, kmin));
+    }
+    NBK_TIMED(nbk_set_j_particles_f64(ctx, n, nullptr, tl.data(), m, x, v, a.data(), jk.data()));
+
+    int64_t T = 0;
+    while (T < T_end) {
+        const int kf = L.finest();
+        const int64_t step = int64_t(1) << (kTickLog2 - kf);
+        const int64_t T_new = (T / step + 1) * step;
+        if (T_new > T_end) break;
+        const double t_new = std::ldexp(static_cast<double>(T_new), -kTickLog2);
+        act.clear();
+        for (int k = kf; k >= kmin; --k) {
+            if (T_new % (int64_t(1) << (kTickLog2 - k)) != 0) break;
+            act.insert(act.end(), L.list[k].begin(), L.list[k].end());
+        }
+        const int64_t ni = static_cast<int64_t>(act.size());
+
+        NBK_TIMED(nbk_set_ti(ctx, t_new));
+        NBK_TIMED(nbk_calc_firsthalf(ctx, n, ni, act.data(), nullptr, nullptr, eps2, flags));
+        // host predictor (fp64) for the block's own particles, overlapped with the device
+        for (int64_t q = 0; q < ni; ++q) {
+            const size_t i = static_cast<size_t>(act[q]);
+            const double dt = t_new - tl[i], dt2 = dt * dt / 2.0, dt3 = dt * dt * dt / 6.0;
+            for (int c = 0; c < 3; ++c) {
+                const size_t k = 3 * i + c;
+                xp[3 * q + c] = x[k] + v[k] * dt + a[k] * dt2 + jk[k] * dt3;
+                vp[3 * q + c] = v[k] + a[k] * dt + jk[k] * dt2;
+            }
+        }
+        NBK_TIMED(nbk_calc_lasthalf(ctx, ni, fa.data(), fj.data(), nullptr));
+
+        for (int64_t q = 0; q < ni; ++q) {
+            const int32_t ii = act[q];
+            const size_t i = static_cast<size_t>(ii);
+            const double dt = t_new - tl[i];
+            double a1[3], j1[3], a2e[3], a3[3];
+            for (int c = 0; c < 3; ++c) {
+                const size_t k = 3 * i + c;
+                a1[c] = fa[3 * q + c];
+                j1[c] = fj[3 * q + c];
+                const double da = a[k] - a1[c];
+                const double a2 = (-6.0 * da - dt * (4.0 * jk[k] + 2.0 * j1[c])) / (dt * dt);
+                a3[c] = (12.0 * da + 6.0 * dt * (jk[k] + j1[c])) / (dt * dt * dt);
+                const double dt3 = dt * dt * dt, dt4 = dt3 * dt;
+                x[k] = xp[3 * q + c] + a2 * (dt4 / 24.0) + a3[c] * (dt4 * dt / 120.0);
+                v[k] = vp[3 * q + c] + a2 * (dt3 / 6.0) + a3[c] * (dt4 / 24.0);
+                a2e[c] = a2 + a3[c] * dt;
+                a[k] = a1[c];
+                jk[k] = j1[c];
+            }
+            tl[i] = t_new;
+            // Aarseth criterion and block rule
+            const double na = norm3(a1), nj = norm3(j1), n2 = norm3(a2e), n3 = norm3(a3);
+            const double num = na * n2 + nj * nj, den = nj * n3 + n2 * n2;
+            double want = dtm;
+            if (den > 0.0) {
+                const double dta = std::sqrt(eta * num / den);
+                if (dta == dta && dta > 0.0) want = std::fmin(dta, dtm);
+            }
+            int k = L.lev[i];
+            const double dt_old = std::ldexp(1.0, -k);
+            if (want < dt_old) {
+                const int kn = level_for(want, kmin);
+                k = kn > k ? kn : k;
+            } else if (want >= 2.0 * dt_old && k > kmin &&
+                       T_new % (int64_t(1) << (kTickLog2 - (k - 1))) == 0) {
+                k -= 1;
+            }
+            if (k != L.lev[i]) {
+                L.remove(ii);
+                L.insert(ii, k);
+            }
+            bt[q] = t_new;
+            bm[q] = m[i];
+            for (int c = 0; c < 3; ++c) {
+                bx[3 * q + c] = x[3 * i + c];
+                bv[3 * q + c] = v[3 * i + c];
+                ba[3 * q + c] = a1[c];
+                bj[3 * q + c] = j1[c];
+            }
+        }
+        NBK_TIMED(nbk_set_j_particles_f64(ctx, ni, act.data(), bt.data(), bm.data(), bx.data(),
+                                          bv.data(), ba.data(), bj.data()));
+        T = T_new;
+        st.block_steps += 1;
+        st.particle_steps += ni;
+        st.interactions += ni * n;
+        int b = 0;
+        while ((int64_t(2) << b) <= ni && b < 31) ++b;
+        st.ni_histogram[b] += 1;
+    }
+#undef NBK_TIMED
+    st.t_reached = std::ldexp(static_cast<double>(T), -kTickLog2);
+    st.wall_seconds = wall.seconds();
+    st.gpu_call_seconds = gpu_s;
+    if (stats) *stats = st;
+    return NBK_OK;
+}

@@ -1,0 +1,615 @@
+// nbk_kernels.cu -- sm_100a kernels of the direct-summation hot path.
+//
+//   a1  scatter_kernel   set_j staging -> raw j-state
+//   a3  predict_kernel   Hermite predictor on the device (L68, L428; the paper runs it on
+//                        the host, L78 -- moving it here is what north_star asks for)
+//   a4+a5  force_kernel  i-gather + the i x j tile: acc, jerk, potential by direct summation
+//                        (L68; Eq. 1; kernel steps 1-4 L91-L96; softening L126-L132)
+//   a6  reduce_kernel    sum of the split-j partials (L112-L118, on the host in the paper),
+//                        self term removed (L96)
+//
+// What is kept from the paper's 8800GTX design (L89-L102): i-particles live in registers, one
+// thread owns whole i-particles, j-particles stream through shared memory in tiles, no use
+// of Newton's third law (L98).  What is different on sm_100a:
+//   * the inner loop is written in packed f32x2 arithmetic (FFMA2/FADD2/FMUL2): one
+//     instruction handles two j-particles, so the 26 FP32-pipe operations per interaction
+//     use 13 issue slots and the remaining slots carry MUFU, LDS and loop overhead.  The
+//     FP32 pipe (2 cycles per packed instruction, measured) is the bound, not issue.
+//   * 1/s comes from MUFU.RCP instead of a multiply (the XU pipe has the room: 2 of its 8-
+//     cycle slots per 26 FP32-pipe cycles).
+//   * j-tiles are brought in by TMA bulk copies (cp.async.bulk + mbarrier), one elected
+//     thread, 2-deep ring; all lanes read the same shared-memory address (LDS.128 broadcast).
+//   * the (i-tile, j-tile) pair list is cut into G = SMs x CTAs/SM equal contiguous ranges
+//     ("stream-K"): every SM gets the same work for any n_i, n_j; a CTA that crosses an
+//     i-tile boundary writes one partial row per i-tile it touched and reduce_kernel adds
+//     the rows in fp64.  The paper's n_i < 4096 split-j special case (L112) becomes the
+//     general path.
+//   * accumulation is hierarchical: fp32 inside one j-tile, fp64 (shared memory, one private
+//     slot per thread) across tiles, fp64 across CTAs -- needed for the 1e-5 potential bound.
+#include "nbk_kernels.cuh"
+
+#ifndef NBK_USE_RCP
+#define NBK_USE_RCP 1
+#endif
+
+namespace nbk {
+
+typedef unsigned long long u64;
+
+// ---------------------------------------------------------------- packed fp32 pair helpers
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
+    u64 d;
+    asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ u64 add2(u64 a, u64 b) {
+    u64 d;
+    asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) {
+    u64 d;
+    asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ u64 pack(float lo, float hi) {
+    u64 d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ void unpack(u64 d, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(d));
+}
+__device__ __forceinline__ float rsq(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// ---------------------------------------------------------------- mbarrier / TMA bulk helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            " selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes,
+                                         uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+
+__host__ __device__ __forceinline__ long long pair_start(long long k, long long P, int G) {
+    return (k * P) / G;
+}
+
+// Shared memory of force_kernel:  [2 mbarriers | pad to 128 B | stages x narr x kTileJ floats |
+// nacc*I x kThreads doubles]
+template <bool JERK>
+struct Shape {
+    static constexpr int narr = JERK ? 7 : 4;   // x y z m [vx vy vz]
+    static constexpr int nacc = JERK ? 10 : 4;  // ax ay az pot [j1 xyz, j2 xyz]
+    static constexpr int stage_floats = narr * kTileJ;
+};
+
+template <int I, bool JERK>
+constexpr size_t smem_bytes_of() {
+    return 128 + sizeof(float) * kStages * Shape<JERK>::stage_floats +
+           sizeof(double) * Shape<JERK>::nacc * I * kThreads;
+}
+
+// One elected thread: bring j-tile `jt` into ring slot `slot`.
+template <bool JERK>
+__device__ __forceinline__ void issue_tile(const JPred& j, int jt, float* stage, uint32_t bar) {
+    constexpr uint32_t bytes = kTileJ * sizeof(float);
+    const size_t off = static_cast<size_t>(jt) * kTileJ;
+    mbar_expect_tx(bar, bytes * Shape<JERK>::narr);
+    const uint32_t dst = smem_u32(stage);
+    bulk_g2s(dst + 0 * bytes, j.x + off, bytes, bar);
+    bulk_g2s(dst + 1 * bytes, j.y + off, bytes, bar);
+    bulk_g2s(dst + 2 * bytes, j.z + off, bytes, bar);
+    bulk_g2s(dst + 3 * bytes, j.m + off, bytes, bar);
+    if (JERK) {
+        bulk_g2s(dst + 4 * bytes, j.vx + off, bytes, bar);
+        bulk_g2s(dst + 5 * bytes, j.vy + off, bytes, bar);
+        bulk_g2s(dst + 6 * bytes, j.vz + off, bytes, bar);
+    }
+}
+
+// ------------------------------------------------------------------------------ force kernel
+// PAPER.md L91-L96 (kernel steps 1-4), restated for sm_100a as described in the file header.
+// Per ordered pair (i, j), r = x_j - x_i, w = v_j - v_i, s = r.r + eps2:
+//   pot  += m s^-1/2            (sign applied in reduce_kernel)
+//   acc  += m s^-3/2 r
+//   j1   += m s^-3/2 w ;  j2 += m s^-5/2 (r.w) r ;  jerk = j1 - 3 j2 (formed per partial row)
+template <int I, bool JERK, bool EPS0, bool PACKED>
+__global__ void __launch_bounds__(kThreads, (I == 1 ? 4 : (I == 2 ? 3 : 2)))
+force_kernel(const ForceArgs a) {
+    using S = Shape<JERK>;
+    constexpr int NACC = S::nacc;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const uint32_t bar0 = smem_u32(smem_raw);
+    float* stages = reinterpret_cast<float*>(smem_raw + 128);
+    double* sacc = reinterpret_cast<double*>(smem_raw + 128 +
+                                             sizeof(float) * kStages * S::stage_floats);
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    const int warp = tid >> 5;
+    const Decomp& d = a.d;
+    const int wjn = d.wj;
+    const int wj = warp % wjn;           // which slice of each j-tile this warp takes
+    const int wi = warp / wjn;           // which 32*I-wide group of the i-tile
+    const int jlen = kTileJ / wjn;
+    const int jbeg = wj * jlen;
+
+    const long long p0 = pair_start(blockIdx.x, d.P, d.G);
+    const long long p1 = pair_start(blockIdx.x + 1LL, d.P, d.G);
+    const int n_local = static_cast<int>(p1 - p0);
+    const int it_first = static_cast<int>(p0 / d.njt);
+
+    if (tid == 0) {
+        mbar_init(bar0, 1);
+        mbar_init(bar0 + 8, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kStages; ++s)
+            if (s < n_local)
+                issue_tile<JERK>(a.j, static_cast<int>((p0 + s) % d.njt),
+                                 stages + s * S::stage_floats, bar0 + 8 * s);
+    }
+
+    // i-state (negated, so r = x_j + (-x_i) is one add) and first-level accumulators
+    u64 nxp[I], nyp[I], nzp[I], nvxp[I], nvyp[I], nvzp[I];   // packed form: value duplicated
+    u64 accp[I][NACC];
+    float nxs[I], nys[I], nzs[I], nvxs[I], nvys[I], nvzs[I]; // scalar form
+    float accs[I][NACC];
+    const u64 e2p = pack(a.eps2, a.eps2);
+    const float e2s = a.eps2;
+
+    int it = it_first;
+    int jt = static_cast<int>(p0 - static_cast<long long>(it_first) * d.njt);
+    bool fresh = true;
+
+    for (int n = 0; n < n_local; ++n) {
+        if (fresh) {
+            // a4: i-gather (Fig. 1: "Data for particle i is taken directly from global memory")
+#pragma unroll
+            for (int q = 0; q < I; ++q) {
+                const int il = wi * 32 * I + q * 32 + lane;
+                const long long i = static_cast<long long>(it) * d.ti + il;
+                float x = 0.f, y = 0.f, z = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
+                if (il < d.ti && i < d.n_i) {
+                    const int idx = a.i_index ? a.i_index[i] : static_cast<int>(i);
+                    if (idx >= 0) {
+                        x = a.j.x[idx]; y = a.j.y[idx]; z = a.j.z[idx];
+                        if (JERK) { vx = a.j.vx[idx]; vy = a.j.vy[idx]; vz = a.j.vz[idx]; }
+                    }
+                    if (a.xi) { x = a.xi[3 * i]; y = a.xi[3 * i + 1]; z = a.xi[3 * i + 2]; }
+                    if (JERK && a.vi) { vx = a.vi[3 * i]; vy = a.vi[3 * i + 1]; vz = a.vi[3 * i + 2]; }
+                }
+                if (PACKED) {
+                    nxp[q] = pack(-x, -x); nyp[q] = pack(-y, -y); nzp[q] = pack(-z, -z);
+                    nvxp[q] = pack(-vx, -vx); nvyp[q] = pack(-vy, -vy); nvzp[q] = pack(-vz, -vz);
+                } else {
+                    nxs[q] = -x; nys[q] = -y; nzs[q] = -z; nvxs[q] = -vx; nvys[q] = -vy; nvzs[q] = -vz;
+                }
+#pragma unroll
+                for (int v = 0; v < NACC; ++v) {
+                    sacc[(q * NACC + v) * kThreads + tid] = 0.0;
+                    accp[q][v] = 0ull;
+                    accs[q][v] = 0.f;
+                }
+            }
+            fresh = false;
+        }
+
+        const int slot = n % kStages;
+        mbar_wait(bar0 + 8 * slot, (n / kStages) & 1);
+        const float* sx = stages + slot * S::stage_floats;
+
+        if (PACKED) {
+#pragma unroll 1
+            for (int jj = jbeg; jj < jbeg + jlen; jj += 4) {
+                const ulonglong2 X = *reinterpret_cast<const ulonglong2*>(sx + jj);
+                const ulonglong2 Y = *reinterpret_cast<const ulonglong2*>(sx + kTileJ + jj);
+                const ulonglong2 Z = *reinterpret_cast<const ulonglong2*>(sx + 2 * kTileJ + jj);
+                const ulonglong2 M = *reinterpret_cast<const ulonglong2*>(sx + 3 * kTileJ + jj);
+                ulonglong2 VX, VY, VZ;
+                if (JERK) {
+                    VX = *reinterpret_cast<const ulonglong2*>(sx + 4 * kTileJ + jj);
+                    VY = *reinterpret_cast<const ulonglong2*>(sx + 5 * kTileJ + jj);
+                    VZ = *reinterpret_cast<const ulonglong2*>(sx + 6 * kTileJ + jj);
+                }
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const u64 xj = h ? X.y : X.x, yj = h ? Y.y : Y.x, zj = h ? Z.y : Z.x;
+                    const u64 mj = h ? M.y : M.x;
+#pragma unroll
+                    for (int q = 0; q < I; ++q) {
+                        const u64 dx = add2(xj, nxp[q]), dy = add2(yj, nyp[q]), dz = add2(zj, nzp[q]);
+                        u64 r2 = fma2(dx, dx, e2p);
+                        r2 = fma2(dy, dy, r2);
+                        r2 = fma2(dz, dz, r2);
+                        float r2a, r2b;
+                        unpack(r2, r2a, r2b);
+                        float ra = rsq(r2a), rb = rsq(r2b);
+                        u64 rinv, rinv2;
+                        if (EPS0) {  // zero-distance pairs contribute nothing
+                            ra = r2a > 0.f ? ra : 0.f;
+                            rb = r2b > 0.f ? rb : 0.f;
+                            rinv = pack(ra, rb);
+                            rinv2 = mul2(rinv, rinv);
+                        } else if (NBK_USE_RCP) {
+                            rinv = pack(ra, rb);
+                            rinv2 = pack(rcp(r2a), rcp(r2b));
+                        } else {
+                            rinv = pack(ra, rb);
+                            rinv2 = mul2(rinv, rinv);
+                        }
+                        const u64 mrinv = mul2(mj, rinv);
+                        accp[q][3] = add2(accp[q][3], mrinv);
+                        const u64 mrinv3 = mul2(mrinv, rinv2);
+                        accp[q][0] = fma2(mrinv3, dx, accp[q][0]);
+                        accp[q][1] = fma2(mrinv3, dy, accp[q][1]);
+                        accp[q][2] = fma2(mrinv3, dz, accp[q][2]);
+                        if (JERK) {
+                            const u64 vxj = h ? VX.y : VX.x, vyj = h ? VY.y : VY.x, vzj = h ? VZ.y : VZ.x;
+                            const u64 dvx = add2(vxj, nvxp[q]), dvy = add2(vyj, nvyp[q]),
+                                      dvz = add2(vzj, nvzp[q]);
+                            u64 rv = mul2(dx, dvx);
+                            rv = fma2(dy, dvy, rv);
+                            rv = fma2(dz, dvz, rv);
+                            accp[q][4] = fma2(mrinv3, dvx, accp[q][4]);
+                            accp[q][5] = fma2(mrinv3, dvy, accp[q][5]);
+                            accp[q][6] = fma2(mrinv3, dvz, accp[q][6]);
+                            const u64 beta = mul2(mul2(rv, rinv2), mrinv3);
+                            accp[q][7] = fma2(beta, dx, accp[q][7]);
+                            accp[q][8] = fma2(beta, dy, accp[q][8]);
+                            accp[q][9] = fma2(beta, dz, accp[q][9]);
+                        }
+                    }
+                }
+            }
+        } else {
+#pragma unroll 2
+            for (int jj = jbeg; jj < jbeg + jlen; ++jj) {
+                const float xj = sx[jj], yj = sx[kTileJ + jj], zj = sx[2 * kTileJ + jj];
+                const float mj = sx[3 * kTileJ + jj];
+                float vxj = 0.f, vyj = 0.f, vzj = 0.f;
+                if (JERK) { vxj = sx[4 * kTileJ + jj]; vyj = sx[5 * kTileJ + jj]; vzj = sx[6 * kTileJ + jj]; }
+#pragma unroll
+                for (int q = 0; q < I; ++q) {
+                    const float dx = xj + nxs[q], dy = yj + nys[q], dz = zj + nzs[q];
+                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, e2s)));
+                    float rinv = rsq(r2);
+                    if (EPS0) rinv = r2 > 0.f ? rinv : 0.f;
+                    const float rinv2 = (!EPS0 && NBK_USE_RCP) ? rcp(r2) : rinv * rinv;
+                    const float mrinv = mj * rinv;
+                    accs[q][3] += mrinv;
+                    const float mrinv3 = mrinv * rinv2;
+                    accs[q][0] = fmaf(mrinv3, dx, accs[q][0]);
+                    accs[q][1] = fmaf(mrinv3, dy, accs[q][1]);
+                    accs[q][2] = fmaf(mrinv3, dz, accs[q][2]);
+                    if (JERK) {
+                        const float dvx = vxj + nvxs[q], dvy = vyj + nvys[q], dvz = vzj + nvzs[q];
+                        const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+                        accs[q][4] = fmaf(mrinv3, dvx, accs[q][4]);
+                        accs[q][5] = fmaf(mrinv3, dvy, accs[q][5]);
+                        accs[q][6] = fmaf(mrinv3, dvz, accs[q][6]);
+                        const float beta = (rv * rinv2) * mrinv3;
+                        accs[q][7] = fmaf(beta, dx, accs[q][7]);
+                        accs[q][8] = fmaf(beta, dy, accs[q][8]);
+                        accs[q][9] = fmaf(beta, dz, accs[q][9]);
+                    }
+                }
+            }
+        }
+
+        // second level: fold this tile's fp32 sums into the thread's private fp64 slots
+#pragma unroll
+        for (int q = 0; q < I; ++q) {
+#pragma unroll
+            for (int v = 0; v < NACC; ++v) {
+                float s;
+                if (PACKED) {
+                    float lo, hi;
+                    unpack(accp[q][v], lo, hi);
+                    s = lo + hi;
+                    accp[q][v] = 0ull;
+                } else {
+                    s = accs[q][v];
+                    accs[q][v] = 0.f;
+                }
+                sacc[(q * NACC + v) * kThreads + tid] += static_cast<double>(s);
+            }
+        }
+
+        __syncthreads();  // every warp is done with ring slot `slot`
+        if (tid == 0 && n + kStages < n_local)
+            issue_tile<JERK>(a.j, static_cast<int>((p0 + n + kStages) % d.njt),
+                             stages + slot * S::stage_floats, bar0 + 8 * slot);
+
+        const bool last_of_tile = (jt == d.njt - 1) || (n == n_local - 1);
+        if (last_of_tile) {
+            // one partial row per (CTA, i-tile touched, j-slice warp):  8 floats per i
+            const long long row =
+                (static_cast<long long>(blockIdx.x) * d.maxseg + (it - it_first)) * wjn + wj;
+#pragma unroll
+            for (int q = 0; q < I; ++q) {
+                const int il = wi * 32 * I + q * 32 + lane;
+                if (il < d.ti) {
+                    const double* sa = sacc + (q * NACC) * kThreads + tid;
+                    float4 o0, o1;
+                    o0.x = static_cast<float>(sa[0 * kThreads]);
+                    o0.y = static_cast<float>(sa[1 * kThreads]);
+                    o0.z = static_cast<float>(sa[2 * kThreads]);
+                    o0.w = static_cast<float>(sa[3 * kThreads]);
+                    if (JERK) {
+                        o1.x = static_cast<float>(sa[4 * kThreads] - 3.0 * sa[7 * kThreads]);
+                        o1.y = static_cast<float>(sa[5 * kThreads] - 3.0 * sa[8 * kThreads]);
+                        o1.z = static_cast<float>(sa[6 * kThreads] - 3.0 * sa[9 * kThreads]);
+                    } else {
+                        o1.x = o1.y = o1.z = 0.f;
+                    }
+                    o1.w = 0.f;
+                    float4* dst = reinterpret_cast<float4*>(a.partial + (row * d.ti + il) * 8);
+                    dst[0] = o0;
+                    dst[1] = o1;
+                }
+            }
+            fresh = true;
+        }
+        if (++jt == d.njt) { jt = 0; ++it; }
+    }
+}
+
+// ----------------------------------------------------------------------------- reduce kernel
+// PAPER.md L118 ("stored in global memory, after which they are ... summed", done on the host
+// there); L96 ("the self interaction of the potential value is removed").
+// grid = ceil(n_i / 32), block = (32, 8): 32 i-particles x 8 lanes over the partial rows.
+template <bool JERK, bool EPS0>
+__global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a) {
+    __shared__ double sh[7][8][32];
+    const Decomp& d = a.d;
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const long long i = static_cast<long long>(blockIdx.x) * 32 + tx;
+    const bool valid = i < d.n_i;
+    double s[7] = {0, 0, 0, 0, 0, 0, 0};
+    if (valid) {
+        const int it = static_cast<int>(i / d.ti);
+        const int il = static_cast<int>(i - static_cast<long long>(it) * d.ti);
+        const long long lo = static_cast<long long>(it) * d.njt, hi = lo + d.njt - 1;
+        long long k0 = (lo * d.G) / d.P;
+        while (k0 + 1 < d.G && pair_start(k0 + 1, d.P, d.G) <= lo) ++k0;
+        long long k1 = (hi * d.G) / d.P;
+        while (k1 + 1 < d.G && pair_start(k1 + 1, d.P, d.G) <= hi) ++k1;
+        const int nrows = static_cast<int>(k1 - k0 + 1) * d.wj;
+        for (int r = ty; r < nrows; r += 8) {
+            const long long k = k0 + r / d.wj;
+            const int w = r % d.wj;
+            const int seg = it - static_cast<int>(pair_start(k, d.P, d.G) / d.njt);
+            const long long row = (k * d.maxseg + seg) * d.wj + w;
+            const float4* p = reinterpret_cast<const float4*>(a.partial + (row * d.ti + il) * 8);
+            const float4 u = p[0];
+            s[0] += u.x; s[1] += u.y; s[2] += u.z; s[3] += u.w;
+            if (JERK) {
+                const float4 v = p[1];
+                s[4] += v.x; s[5] += v.y; s[6] += v.z;
+            }
+        }
+    }
+#pragma unroll
+    for (int v = 0; v < 7; ++v) sh[v][ty][tx] = s[v];
+    __syncthreads();
+    if (ty == 0 && valid) {
+#pragma unroll
+        for (int v = 0; v < 7; ++v) {
+            double t = 0.0;
+#pragma unroll
+            for (int r = 0; r < 8; ++r) t += sh[v][r][tx];
+            s[v] = t;
+        }
+        // remove the i-particle's own j entry: the same fp32 pair arithmetic as force_kernel
+        const int idx = a.i_index ? a.i_index[i] : static_cast<int>(i);
+        if (idx >= 0) {
+            const float xj = a.j.x[idx], yj = a.j.y[idx], zj = a.j.z[idx], mj = a.j.m[idx];
+            float x = xj, y = yj, z = zj, vx = 0.f, vy = 0.f, vz = 0.f, vxj = 0.f, vyj = 0.f, vzj = 0.f;
+            if (JERK) { vxj = a.j.vx[idx]; vyj = a.j.vy[idx]; vzj = a.j.vz[idx]; vx = vxj; vy = vyj; vz = vzj; }
+            if (a.xi) { x = a.xi[3 * i]; y = a.xi[3 * i + 1]; z = a.xi[3 * i + 2]; }
+            if (JERK && a.vi) { vx = a.vi[3 * i]; vy = a.vi[3 * i + 1]; vz = a.vi[3 * i + 2]; }
+            const float dx = xj + (-x), dy = yj + (-y), dz = zj + (-z);
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, a.eps2)));
+            float rinv = rsq(r2);
+            if (EPS0) rinv = r2 > 0.f ? rinv : 0.f;
+            const float rinv2 = (!EPS0 && NBK_USE_RCP) ? rcp(r2) : rinv * rinv;
+            const float mrinv = mj * rinv;
+            const float mrinv3 = mrinv * rinv2;
+            s[3] -= mrinv;
+            s[0] -= mrinv3 * dx; s[1] -= mrinv3 * dy; s[2] -= mrinv3 * dz;
+            if (JERK) {
+                const float dvx = vxj + (-vx), dvy = vyj + (-vy), dvz = vzj + (-vz);
+                const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+                const float beta = (rv * rinv2) * mrinv3;
+                s[4] -= static_cast<double>(mrinv3 * dvx) - 3.0 * static_cast<double>(beta * dx);
+                s[5] -= static_cast<double>(mrinv3 * dvy) - 3.0 * static_cast<double>(beta * dy);
+                s[6] -= static_cast<double>(mrinv3 * dvz) - 3.0 * static_cast<double>(beta * dz);
+            }
+        }
+        a.acc[3 * i + 0] = static_cast<float>(s[0]);
+        a.acc[3 * i + 1] = static_cast<float>(s[1]);
+        a.acc[3 * i + 2] = static_cast<float>(s[2]);
+        a.pot[i] = static_cast<float>(-s[3]);
+        a.jerk[3 * i + 0] = static_cast<float>(s[4]);
+        a.jerk[3 * i + 1] = static_cast<float>(s[5]);
+        a.jerk[3 * i + 2] = static_cast<float>(s[6]);
+    }
+}
+
+// ------------------------------------------------------------------ scatter (a1) / predict (a3)
+template <typename T>
+__global__ void scatter_kernel(const ScatterArgs s, const RawJ raw) {
+    const long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (k >= s.n) return;
+    const long long ad = s.addr ? static_cast<long long>(s.addr[k]) : k;
+    if (ad < 0 || ad >= s.n_max) return;
+    const T* m = static_cast<const T*>(s.m);
+    const T* x = static_cast<const T*>(s.x);
+    const T* v = static_cast<const T*>(s.v);
+    const T* ac = static_cast<const T*>(s.a);
+    const T* jk = static_cast<const T*>(s.k);
+    raw.m[ad] = static_cast<float>(m[k]);
+    raw.t[ad] = s.tj ? s.tj[k] : 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        raw.x[c * raw.cap + ad] = static_cast<double>(x[3 * k + c]);
+        raw.v[c * raw.cap + ad] = v ? static_cast<float>(v[3 * k + c]) : 0.f;
+        raw.a[c * raw.cap + ad] = ac ? static_cast<float>(ac[3 * k + c]) : 0.f;
+        raw.k[c * raw.cap + ad] = jk ? static_cast<float>(jk[3 * k + c]) : 0.f;
+    }
+}
+
+// Hermite predictor (reading R8), fp64, rounded once to fp32:
+//   x_p = x + v dt + a dt^2/2 + jerk dt^3/6 ;  v_p = v + a dt + jerk dt^2/2 ;  dt = t - t_j
+__global__ void predict_kernel(const RawJ raw, double t, long long n_j, long long n_pad, float* px,
+                               float* py, float* pz, float* pm, float* pvx, float* pvy,
+                               float* pvz) {
+    const long long j = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (j >= n_pad) return;
+    float o[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (j < n_j) {
+        const double dt = t - raw.t[j];
+        const double dt2 = dt * dt * 0.5, dt3 = dt * dt * dt * (1.0 / 6.0);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double x = raw.x[c * raw.cap + j];
+            const double v = raw.v[c * raw.cap + j];
+            const double ac = raw.a[c * raw.cap + j];
+            const double jk = raw.k[c * raw.cap + j];
+            o[c] = static_cast<float>(x + v * dt + ac * dt2 + jk * dt3);
+            o[4 + c] = static_cast<float>(v + ac * dt + jk * dt2);
+        }
+        o[3] = raw.m[j];
+    }
+    px[j] = o[0]; py[j] = o[1]; pz[j] = o[2]; pm[j] = o[3];
+    pvx[j] = o[4]; pvy[j] = o[5]; pvz[j] = o[6];
+}
+
+// --------------------------------------------------------------------------------- launchers
+template <int I, bool JERK, bool EPS0, bool PACKED>
+static int occupancy_of(cudaError_t* err) {
+    auto fn = force_kernel<I, JERK, EPS0, PACKED>;
+    const size_t smem = smem_bytes_of<I, JERK>();
+    *err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    if (*err != cudaSuccess) return -1;
+    int nb = 0;
+    *err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, kThreads, smem);
+    if (*err != cudaSuccess) return -1;
+    return nb;
+}
+
+template <int I, bool JERK, bool EPS0, bool PACKED>
+static cudaError_t launch_of(const ForceArgs& a, cudaStream_t s) {
+    force_kernel<I, JERK, EPS0, PACKED><<<a.d.G, kThreads, smem_bytes_of<I, JERK>(), s>>>(a);
+    return cudaGetLastError();
+}
+
+#define NBK_DISPATCH(CALL, ...)                                                         \
+    do {                                                                                \
+        const int key = (v.I == 1 ? 0 : v.I == 2 ? 1 : 2) * 8 + (v.jerk ? 4 : 0) +      \
+                        (v.eps0 ? 2 : 0) + (v.packed ? 1 : 0);                          \
+        switch (key) {                                                                  \
+            case 0: return CALL<1, false, false, false>(__VA_ARGS__);                   \
+            case 1: return CALL<1, false, false, true>(__VA_ARGS__);                    \
+            case 2: return CALL<1, false, true, false>(__VA_ARGS__);                    \
+            case 3: return CALL<1, false, true, true>(__VA_ARGS__);                     \
+            case 4: return CALL<1, true, false, false>(__VA_ARGS__);                    \
+            case 5: return CALL<1, true, false, true>(__VA_ARGS__);                     \
+            case 6: return CALL<1, true, true, false>(__VA_ARGS__);                     \
+            case 7: return CALL<1, true, true, true>(__VA_ARGS__);                      \
+            case 8: return CALL<2, false, false, false>(__VA_ARGS__);                   \
+            case 9: return CALL<2, false, false, true>(__VA_ARGS__);                    \
+            case 10: return CALL<2, false, true, false>(__VA_ARGS__);                   \
+            case 11: return CALL<2, false, true, true>(__VA_ARGS__);                    \
+            case 12: return CALL<2, true, false, false>(__VA_ARGS__);                   \
+            case 13: return CALL<2, true, false, true>(__VA_ARGS__);                    \
+            case 14: return CALL<2, true, true, false>(__VA_ARGS__);                    \
+            case 15: return CALL<2, true, true, true>(__VA_ARGS__);                     \
+            case 16: return CALL<4, false, false, false>(__VA_ARGS__);                  \
+            case 17: return CALL<4, false, false, true>(__VA_ARGS__);                   \
+            case 18: return CALL<4, false, true, false>(__VA_ARGS__);                   \
+            case 19: return CALL<4, false, true, true>(__VA_ARGS__);                    \
+            case 20: return CALL<4, true, false, false>(__VA_ARGS__);                   \
+            case 21: return CALL<4, true, false, true>(__VA_ARGS__);                    \
+            case 22: return CALL<4, true, true, false>(__VA_ARGS__);                    \
+            default: return CALL<4, true, true, true>(__VA_ARGS__);                     \
+        }                                                                               \
+    } while (0)
+
+size_t force_smem_bytes(const Variant& v) {
+    const int nacc = v.jerk ? 10 : 4, narr = v.jerk ? 7 : 4;
+    return 128 + sizeof(float) * kStages * narr * kTileJ + sizeof(double) * nacc * v.I * kThreads;
+}
+
+int force_occupancy(const Variant& v, cudaError_t* err) { NBK_DISPATCH(occupancy_of, err); }
+
+cudaError_t launch_force(const Variant& v, const ForceArgs& a, cudaStream_t s) {
+    NBK_DISPATCH(launch_of, a, s);
+}
+
+cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s) {
+    const dim3 block(32, 8);
+    const unsigned grid = static_cast<unsigned>((a.d.n_i + 31) / 32);
+    if (v.jerk) {
+        if (v.eps0) reduce_kernel<true, true><<<grid, block, 0, s>>>(a);
+        else reduce_kernel<true, false><<<grid, block, 0, s>>>(a);
+    } else {
+        if (v.eps0) reduce_kernel<false, true><<<grid, block, 0, s>>>(a);
+        else reduce_kernel<false, false><<<grid, block, 0, s>>>(a);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scatter(const ScatterArgs& s, const RawJ& raw, cudaStream_t st) {
+    if (s.n <= 0) return cudaSuccess;
+    const unsigned grid = static_cast<unsigned>((s.n + 255) / 256);
+    if (s.f64) scatter_kernel<double><<<grid, 256, 0, st>>>(s, raw);
+    else scatter_kernel<float><<<grid, 256, 0, st>>>(s, raw);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n_pad, float* px,
+                           float* py, float* pz, float* pm, float* pvx, float* pvy, float* pvz,
+                           cudaStream_t st) {
+    if (n_pad <= 0) return cudaSuccess;
+    const unsigned grid = static_cast<unsigned>((n_pad + 255) / 256);
+    predict_kernel<<<grid, 256, 0, st>>>(raw, t, n_j, n_pad, px, py, pz, pm, pvx, pvy, pvz);
+    return cudaGetLastError();
+}
+
+}  // namespace nbk

@@ -1,0 +1,105 @@
+// nbk_kernels.cuh -- launch-side declarations shared by nbk_kernels.cu and nbk_api.cu.
+// Internal to the CUDA path; nothing here is part of the C ABI (include/nbk.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace nbk {
+
+constexpr int kThreads = 128;   // threads per CTA of the force kernel (4 warps)
+constexpr int kWarps = kThreads / 32;
+constexpr int kTileJ = 256;     // j-particles per shared-memory tile (1 KB per array)
+constexpr int kStages = 2;      // tile ring depth (TMA bulk copies run one tile ahead)
+constexpr int kMaxI = 4;        // max i-particles per thread
+
+// Predicted j-state, structure of arrays, each padded to a multiple of kTileJ with m = 0.
+struct JPred {
+    const float* x;
+    const float* y;
+    const float* z;
+    const float* m;
+    const float* vx;
+    const float* vy;
+    const float* vz;
+};
+
+// Work decomposition ("stream-K" over the (i-tile, j-tile) pair list, i-major):
+// pair p = it * njt + jt;  CTA k owns pairs [k*P/G, (k+1)*P/G).
+struct Decomp {
+    int n_i;          // active i-particles
+    int ti;           // i-particles per CTA tile = wi * 32 * I
+    int wj;           // warps that split each j-tile (1, 2 or 4); wi = kWarps / wj
+    int nit;          // i-tiles
+    int njt;          // j-tiles
+    long long P;      // nit * njt
+    int G;            // CTAs
+    int maxseg;       // max i-tiles one CTA touches
+};
+
+struct ForceArgs {
+    JPred j;
+    const int32_t* i_index;  // [n_i] or nullptr (identity)
+    const float* xi;         // [n_i][3] or nullptr
+    const float* vi;         // [n_i][3] or nullptr
+    float* partial;          // [(k*maxseg+seg)*wj + w][ti][8]
+    float eps2;
+    Decomp d;
+};
+
+struct ReduceArgs {
+    JPred j;
+    const int32_t* i_index;
+    const float* xi;
+    const float* vi;
+    const float* partial;
+    float* acc;   // [n_i][3]
+    float* jerk;  // [n_i][3]
+    float* pot;   // [n_i]
+    float eps2;
+    Decomp d;
+};
+
+struct RawJ {        // raw j-state kept for the predictor, structure of arrays of capacity cap
+    double* x;       // [3][cap]
+    float* v;        // [3][cap]
+    float* a;        // [3][cap]
+    float* k;        // [3][cap]  (jerk)
+    float* m;        // [cap]
+    double* t;       // [cap]
+    long long cap;
+};
+
+struct Variant {
+    int I;        // 1, 2 or 4
+    bool jerk;
+    bool eps0;
+    bool packed;  // f32x2 inner loop
+};
+
+size_t force_smem_bytes(const Variant& v);
+// CTAs of this variant that fit one SM (queried once per variant; also raises the dynamic
+// shared-memory limit of the instantiation).  Returns <= 0 and sets *err on failure.
+int force_occupancy(const Variant& v, cudaError_t* err);
+cudaError_t launch_force(const Variant& v, const ForceArgs& a, cudaStream_t s);
+cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s);
+
+// set_j scatter: staged particles -> raw SoA at addr (nullptr: identity).  x, v as fp32 or fp64.
+struct ScatterArgs {
+    long long n;
+    const int32_t* addr;
+    const double* tj;
+    const void* m;      // float or double
+    const void* x;      // [n][3] float or double
+    const void* v;      // may be nullptr
+    const void* a;      // may be nullptr
+    const void* k;      // may be nullptr
+    int f64;            // 1: m, x, v, a, k are double
+    long long n_max;    // addresses outside [0, n_max) are skipped
+};
+cudaError_t launch_scatter(const ScatterArgs& s, const RawJ& raw, cudaStream_t st);
+// a3: predict raw -> predicted arrays for j < n_j, m = 0 padding for n_j <= j < n_pad.
+cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n_pad, float* px,
+                           float* py, float* pz, float* pm, float* pvx, float* pvy, float* pvz,
+                           cudaStream_t st);
+
+}  // namespace nbk
