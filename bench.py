@@ -1,0 +1,379 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the direct-summation hot path on B200, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C3|C3b|C4|C2|C1]
+
+Metric (BASELINE.json): pairwise interactions/s for acc+jerk+pot at N=131072 (config C3:
+seeded Plummer sphere, eps=1/256, all i active), interactions = n_i * n_j with the self pair
+counted as the paper does.
+
+A "step" is one pass of the whole hot path through the C ABI:
+  a1 nbk_set_j_particles[_dev]  a2 nbk_set_ti  a3 predict kernel  a4+a5 i x j force kernel
+  a6 reduce kernel  a7 nbk_calc_lasthalf[_dev]
+`value`   : inputs resident in HBM, _dev entry points, each step timed with CUDA events on the
+            stream the library launches on; L2 is flushed between steps (outside the events).
+`e2e`     : the same step through the HOST entry points (pageable numpy arrays in, numpy arrays
+            out; the library stages through its pinned buffers), host clock around K steps.
+`roofline`: the i x j force kernel alone (the library's own CUDA events around that launch),
+            bound "alu": executed fp32 flops / (SMs x 128 lanes x 2 x max SM clock).
+`cpu_baseline`: oracle/nbody_oracle.c (fp64, OpenMP) on a bounded i-slice of the same workload.
+
+N > 1 (torchrun): the path does not shard under BASELINE.json's north_star ("Everything runs on
+one GPU, with no sharding or collectives"), so every rank runs an independent replica of the
+workload ("replicas only"); value = sum of interactions over ranks / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "pairwise interactions/sec (acc+jerk+pot) and % of B200 FP32 peak at N=131072"
+UNIT = "interactions/s"
+FLOPS_EXECUTED = {True: 42.0, False: 20.0}   # per interaction, FFMA = 2
+FLOPS_PAPER = {True: 60.0, False: 38.0}      # PAPER.md Eq. 3
+FP32_OPS = {True: 27.0, False: 13.0}         # minimum FP32-pipe lane operations per interaction
+L2_FLUSH_BYTES = 256 << 20                   # > 126 MB L2
+
+WORKLOADS = {
+    # name: (config, eps, jerk, description)
+    "C1": ("C1", 1.0 / 256.0, True, "C1: N=1024 Plummer seed 1, eps=1/256, acc+jerk+pot, all i"),
+    "C2": ("C2", 1.0 / 256.0, True, "C2: N=16384 Plummer seed 2, eps=1/256, acc+jerk+pot, all i"),
+    "C3": ("C3", 1.0 / 256.0, True, "C3: N=131072 Plummer seed 3, eps=1/256, acc+jerk+pot, all i"),
+    "C3b": ("C3", 0.0, True, "C3b: N=131072 Plummer seed 3, eps=0 (self/zero-distance masked), acc+jerk+pot"),
+    "C4": ("C4", 1.0 / 256.0, False, "C4: N=1048576 Plummer seed 4, eps=1/256, acc+pot only, all i"),
+    "C5": ("C5", 1.0 / 256.0, True, "C5: N=65536 Plummer seed 5, eps=1/256, acc+jerk+pot, all i"),
+}
+
+
+# ------------------------------------------------------------------------ multi-rank plumbing
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def aggregate(local_ms: float, local_units: float, world: int, backend_device: str):
+    """max-over-ranks time and sum-over-ranks units (torch.distributed; identity at world 1)."""
+    if world == 1:
+        return local_ms, local_units
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([local_ms], dtype=torch.float64, device=backend_device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=backend_device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ------------------------------------------------------------------------ clocks during timing
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    BITS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+            0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, index: int, period: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.power = [], set(), []
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        self.error = None
+
+    def run(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
+            while not self._stop_evt.is_set():
+                self.samples.append(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                try:
+                    self.power.append(pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                    r = pynvml.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except Exception:  # older binding name
+                    r = pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, name in self.BITS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                time.sleep(self.period)
+        except Exception as e:  # NVML unavailable: report it, never fake clocks
+            self.error = repr(e)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2.0)
+        out = {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+               "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+               "samples": len(self.samples)}
+        if self.power:
+            out["power_w_max"] = max(self.power)
+        if self.error:
+            out["error"] = self.error
+        return out
+
+
+def physical_gpu_index(local: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local])
+        except Exception:
+            return local
+    return local
+
+
+# ------------------------------------------------------------------------ the oracle legs
+def oracle_sample(m, x, v, eps, jerk, target_s=15.0, seed=11):
+    """Time oracle/nbody_oracle.c on a bounded i-slice of the workload (all j).  Returns
+    (interactions/s, cores, n_i_sample, seconds)."""
+    from oracle import c_oracle
+    c_oracle.build()
+    n = m.shape[0]
+    cores = c_oracle.num_threads()
+    rng = np.random.default_rng(seed)
+    probe = min(n, 64 * cores)
+    idx = np.sort(rng.choice(n, size=probe, replace=False))
+    t0 = time.perf_counter()
+    c_oracle.force(m, x, v, eps, i_index=idx, want_jerk=jerk)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    n_i = int(min(n, max(probe, probe * target_s / dt)))
+    idx = np.sort(rng.choice(n, size=n_i, replace=False))
+    t0 = time.perf_counter()
+    c_oracle.force(m, x, v, eps, i_index=idx, want_jerk=jerk)
+    dt = time.perf_counter() - t0
+    return n_i * n / dt, cores, n_i, dt
+
+
+def run_reference(args, wl):
+    """--impl reference: the oracle as it stands, on the host cores, same metric and config."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    from paper_0707_0438_b200 import inputs
+    from oracle import c_oracle
+    cfg, eps, jerk, desc = wl
+    m, x, v = inputs.config_inputs(cfg)
+    n = m.shape[0]
+    c_oracle.build()
+    cores = c_oracle.num_threads()
+    rng = np.random.default_rng(11)
+    # size one step to ~ (120 s / (steps + warmup)), from a short probe
+    probe = min(n, 32 * cores)
+    idx = np.sort(rng.choice(n, size=probe, replace=False))
+    t0 = time.perf_counter()
+    c_oracle.force(m, x, v, eps, i_index=idx, want_jerk=jerk)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    budget = 120.0 / max(1, args.steps + args.warmup)
+    n_i = int(min(n, max(probe, probe * budget / dt)))
+    idx = np.sort(rng.choice(n, size=n_i, replace=False))
+    for _ in range(args.warmup):
+        c_oracle.force(m, x, v, eps, i_index=idx, want_jerk=jerk)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        c_oracle.force(m, x, v, eps, i_index=idx, want_jerk=jerk)
+    dt = time.perf_counter() - t0
+    value = args.steps * n_i * n / dt
+    sample = f"{n_i} of {n} i-particles (seeded choice) x all {n} j per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": desc, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------ our arm
+def run_ours(args, wl):
+    import torch
+    rank, local, world = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    from paper_0707_0438_b200 import binding as nb
+    from paper_0707_0438_b200 import inputs
+    nb.load()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg, eps, jerk, desc = wl
+    m, x, v = inputs.config_inputs(cfg)
+    n = m.shape[0]
+    eps2 = float(np.float32(eps) ** 2)
+    flags = (nb.NBK_JERK if jerk else 0) | nb.NBK_POT
+
+    stream = torch.cuda.Stream(device=dev)
+    ctx = nb.nbk_open(local, n, n, stream.cuda_stream)
+    try:
+        with torch.cuda.stream(stream):
+            d_m = torch.from_numpy(m).to(dev)
+            d_x = torch.from_numpy(x).to(dev)
+            d_v = torch.from_numpy(v).to(dev)
+            d_acc = torch.empty((n, 3), dtype=torch.float32, device=dev)
+            d_jrk = torch.empty((n, 3), dtype=torch.float32, device=dev)
+            d_pot = torch.empty((n,), dtype=torch.float32, device=dev)
+            flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+        stream.synchronize()
+
+        def step_dev():
+            nb.nbk_set_j_particles_dev(ctx, n, 0, 0, d_m.data_ptr(), d_x.data_ptr(), d_v.data_ptr())
+            nb.nbk_set_ti(ctx, 0.0)
+            nb.nbk_calc_firsthalf_dev(ctx, n, n, 0, 0, 0, eps2, flags)
+            nb.nbk_calc_lasthalf_dev(ctx, n, d_acc.data_ptr(), d_jrk.data_ptr(), d_pot.data_ptr())
+
+        def step_host():
+            nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+            nb.nbk_set_ti(ctx, 0.0)
+            nb.nbk_calc_firsthalf(ctx, n, n, None, None, None, eps2, flags)
+            return nb.nbk_calc_lasthalf(ctx, n)
+
+        def barrier():
+            if world > 1:
+                import torch.distributed as dist
+                dist.barrier()
+            torch.cuda.synchronize(dev)
+
+        # ---- device-resident arm: per-step CUDA events on the library's stream
+        nb.nbk_set_timing(ctx, True)
+        with torch.cuda.stream(stream):
+            for _ in range(max(args.warmup, 0)):
+                flush.zero_()
+                step_dev()
+        barrier()
+        sampler = ClockSampler(physical_gpu_index(local))
+        sampler.start()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+               for _ in range(args.steps)]
+        kern_ms = {"scatter": [], "predict": [], "force": [], "reduce": []}
+        with torch.cuda.stream(stream):
+            for k in range(args.steps):
+                flush.zero_()            # L2 flush between timed iterations, outside the events
+                evs[k][0].record(stream)
+                step_dev()
+                evs[k][1].record(stream)
+                t = nb.nbk_get_timing(ctx)   # waits for this step; the library's own per-kernel events
+                for key in kern_ms:
+                    kern_ms[key].append(t[key])
+        barrier()
+        clocks = sampler.stop()
+        step_ms = [a.elapsed_time(b) for a, b in evs]
+        local_ms = float(np.sum(step_ms))
+        launch = nb.nbk_last_launch(ctx)
+        nb.nbk_set_timing(ctx, False)
+        total_ms, total_units = aggregate(local_ms, float(args.steps) * n * n, world, str(dev))
+        value = total_units / (total_ms * 1e-3)
+
+        # ---- end-to-end arm: host buffers through the host entry points
+        for _ in range(min(args.warmup, 3)):
+            step_host()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            out = step_host()
+        torch.cuda.synchronize(dev)
+        e2e_local_ms = 1e3 * (time.perf_counter() - t0)
+        barrier()
+        e2e_ms, e2e_units = aggregate(e2e_local_ms, float(args.steps) * n * n, world, str(dev))
+        e2e_value = e2e_units / (e2e_ms * 1e-3)
+        assert np.all(np.isfinite(out[0])) and np.all(np.isfinite(out[2]))
+    finally:
+        nb.nbk_close(ctx)
+
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    if rank != 0:
+        return 0
+
+    # ---- roofline of the dominant kernel (i x j force tile), rank 0
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    sm_max_mhz = clocks.get("sm_max_mhz") or 1965.0
+    peak_src = "nvml max SM clock"
+    if os.path.exists(peaks_path):
+        try:
+            with open(peaks_path) as f:
+                sm_max_mhz = float(json.load(f)["sm_max_mhz"])
+            peak_src = "MEASURED_PEAKS.json sm_max_mhz"
+        except Exception:
+            pass
+    peak_tflops = sm_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12
+    force_ms = float(np.mean(kern_ms["force"]))
+    kint = n * n / (force_ms * 1e-3)
+    achieved = FLOPS_EXECUTED[jerk] * kint / 1e12
+    roofline = {
+        "bound": "alu", "kernel": "nbk::force_kernel", "achieved": achieved, "peak": peak_tflops,
+        "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
+        "peak_source": f"{sm_count} SMs x 128 fp32 lanes x 2 x {sm_max_mhz:.0f} MHz ({peak_src}); "
+                       "DESIGN.md 'Roofline'",
+        "flops_per_interaction": FLOPS_EXECUTED[jerk],
+        "kernel_ms": force_ms, "kernel_interactions_per_s": kint,
+        "tflops_paper_convention": FLOPS_PAPER[jerk] * kint / 1e12,
+        "frac_paper_convention": FLOPS_PAPER[jerk] * kint / 1e12 / peak_tflops,
+        "fp32_pipe_frac_at_max_clock": FP32_OPS[jerk] * kint / (sm_count * 128 * sm_max_mhz * 1e6),
+        "fp32_pipe_frac_at_observed_clock": (FP32_OPS[jerk] * kint / (sm_count * 128 * clocks["sm_mhz"] * 1e6)
+                                             if clocks.get("sm_mhz") else None),
+        "mufu_limit_interactions_per_s": sm_count * 16 * sm_max_mhz * 1e6,
+        "kernel_share_of_step": force_ms / float(np.mean(step_ms)),
+        "other_kernels_ms": {k: float(np.mean(kern_ms[k])) for k in ("scatter", "predict", "reduce")},
+    }
+
+    # ---- the oracle on the host cores, bounded sample
+    cpu_baseline = None
+    if not args.skip_cpu_baseline:
+        ov, cores, ni_s, secs = oracle_sample(m, x, v, eps, jerk)
+        cpu_baseline = {"value": ov, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": f"{ni_s} of {n} i-particles (seeded choice) x all {n} j, {secs:.1f} s"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": desc, "n_i": n, "n_j": n, "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB write)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "launch": launch},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(n * (4 + 12 + 12)),
+                "d2h_bytes_per_step": int(n * 28), "ms_per_step": e2e_ms / args.steps},
+        "gpu_launches": int(args.steps * 4),
+        "roofline": roofline,
+        "cpu_baseline": cpu_baseline,
+        "tflops_paper_convention": FLOPS_PAPER[jerk] * value / 1e12,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", choices=sorted(WORKLOADS), default="C3")
+    ap.add_argument("--skip-cpu-baseline", action="store_true",
+                    help="do not time the oracle (for runs under ncu); cpu_baseline is then null")
+    args = ap.parse_args(argv)
+    wl = WORKLOADS[args.workload]
+    if args.impl == "reference":
+        return run_reference(args, wl)
+    return run_ours(args, wl)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

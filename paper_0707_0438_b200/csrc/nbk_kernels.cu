@@ -101,6 +101,10 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
         : "memory");
 }
 
+#ifdef NBK_TRACE
+__device__ long long nbk_trace_buf[3 * 4096];
+#endif
+
 __host__ __device__ __forceinline__ long long pair_start(long long k, long long P, int G) {
     return (k * P) / G;
 }
@@ -158,6 +162,10 @@ force_kernel(const ForceArgs a) {
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const int warp = tid >> 5;
+#ifdef NBK_TRACE
+    long long trace_t0 = 0;
+    if (tid == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(trace_t0));
+#endif
     const Decomp& d = a.d;
     const int wjn = d.wj;
     const int wj = warp % wjn;           // which slice of each j-tile this warp takes
@@ -387,6 +395,17 @@ force_kernel(const ForceArgs a) {
         }
         if (++jt == d.njt) { jt = 0; ++it; }
     }
+#ifdef NBK_TRACE
+    if (tid == 0 && blockIdx.x < 4096) {
+        long long t1;
+        unsigned smid;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        nbk_trace_buf[3 * blockIdx.x] = trace_t0;
+        nbk_trace_buf[3 * blockIdx.x + 1] = t1;
+        nbk_trace_buf[3 * blockIdx.x + 2] = smid;
+    }
+#endif
 }
 
 // ----------------------------------------------------------------------------- reduce kernel
@@ -613,3 +632,9 @@ cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n
 }
 
 }  // namespace nbk
+
+#ifdef NBK_TRACE
+extern "C" int nbk_debug_trace(long long* out, int n) {
+    return static_cast<int>(cudaMemcpyFromSymbol(out, nbk::nbk_trace_buf, sizeof(long long) * 3 * n));
+}
+#endif
