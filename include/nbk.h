@@ -171,11 +171,20 @@ int nbk_sync(nbk_ctx* ctx);
 int nbk_set_timing(nbk_ctx* ctx, int enable);
 int nbk_get_timing(nbk_ctx* ctx, float ms[4]);
 
-/* Launch shape of the last firsthalf: out[0] grid (CTAs), out[1] threads per CTA,
- * out[2] i-particles per thread, out[3] warps splitting each j-tile, out[4] CTAs per SM the
- * grid was sized for, out[5] SM count, out[6] dynamic shared memory bytes,
- * out[7] number of kernels launched by the last firsthalf. */
+/* Launch shape of the last firsthalf: out[0] grid (CTAs, one per SM at most), out[1] threads
+ * per CTA, out[2] i-particles per thread, out[3] warps splitting each j-tile, out[4] j-tile
+ * size, out[5] SM count, out[6] dynamic shared memory bytes, out[7] number of kernels launched
+ * by the last firsthalf. */
 int nbk_last_launch(const nbk_ctx* ctx, int64_t out[8]);
+
+/* Host-only (no GPU needed): the launch plan firsthalf would use for (n_i, n_j) on a device with
+ * num_sms SMs -- the split-j / stream-K decomposition of PAPER.md L112-L118 generalised.
+ * force_i: 0 or a pinned i-per-thread count (1, 2, 4).  out[0] i per thread, out[1] threads per
+ * CTA, out[2] i-tile, out[3] j-tile, out[4] warps splitting a j-tile, out[5] i-tiles,
+ * out[6] j-tiles, out[7] pairs P, out[8] CTAs G, out[9] max i-tiles one CTA touches,
+ * out[10] floats of partial rows needed, out[11] floats a context with ni_max = n_i holds.
+ * CTA k works on pairs [k*P/G, (k+1)*P/G) of the i-major (i-tile, j-tile) list. */
+int nbk_plan(int64_t n_i, int64_t n_j, int num_sms, int force_i, int64_t out[12]);
 
 /* Choose the inner-loop form: 0 = packed f32x2 (FFMA2, two j per instruction; default),
  * 1 = scalar fp32.  Both compute the same sums; kept for measurement. */

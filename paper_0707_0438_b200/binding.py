@@ -22,7 +22,7 @@ EXPORTS = [
     "nbk_set_j_particles_dev", "nbk_set_ti", "nbk_predict", "nbk_get_predicted",
     "nbk_calc_firsthalf", "nbk_calc_firsthalf_dev", "nbk_calc_lasthalf", "nbk_calc_lasthalf_dev",
     "nbk_hermite_evolve", "nbk_sync", "nbk_set_timing", "nbk_get_timing", "nbk_last_launch",
-    "nbk_set_variant", "nbk_last_cuda_error", "nbk_strerror", "nbk_version",
+    "nbk_plan", "nbk_set_variant", "nbk_last_cuda_error", "nbk_strerror", "nbk_version",
 ]
 
 _vp, _i64, _i32, _u32, _f32, _f64 = (ctypes.c_void_p, ctypes.c_int64, ctypes.c_int,
@@ -55,6 +55,7 @@ _SIGS = {
     "nbk_set_timing": (_i32, [_vp, _i32]),
     "nbk_get_timing": (_i32, [_vp, ctypes.POINTER(_f32 * 4)]),
     "nbk_last_launch": (_i32, [_vp, ctypes.POINTER(_i64 * 8)]),
+    "nbk_plan": (_i32, [_i64, _i64, _i32, _i32, ctypes.POINTER(_i64 * 12)]),
     "nbk_set_variant": (_i32, [_vp, _i32]),
     "nbk_last_cuda_error": (_i32, [_vp]),
     "nbk_strerror": (ctypes.c_char_p, [_i32]),
@@ -235,7 +236,15 @@ def nbk_get_timing(ctx):
 def nbk_last_launch(ctx):
     out = (_i64 * 8)()
     _check("nbk_last_launch", load().nbk_last_launch(ctx, ctypes.byref(out)), ctx)
-    keys = ["grid", "threads", "i_per_thread", "j_split_warps", "ctas_per_sm", "sms", "smem_bytes", "launches"]
+    keys = ["grid", "threads", "i_per_thread", "j_split_warps", "j_tile", "sms", "smem_bytes", "launches"]
+    return dict(zip(keys, list(out)))
+
+
+def nbk_plan(n_i: int, n_j: int, num_sms: int = 148, force_i: int = 0):
+    out = (_i64 * 12)()
+    _check("nbk_plan", load().nbk_plan(n_i, n_j, num_sms, force_i, ctypes.byref(out)))
+    keys = ["i_per_thread", "threads", "i_tile", "j_tile", "j_split_warps", "i_tiles", "j_tiles", "pairs",
+            "grid", "max_segments", "partial_floats", "partial_floats_bound"]
     return dict(zip(keys, list(out)))
 
 

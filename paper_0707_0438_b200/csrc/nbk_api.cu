@@ -17,13 +17,6 @@ using namespace nbk;
 
 namespace {
 
-constexpr int kNumVariants = 24;
-
-inline int variant_key(const Variant& v) {
-    return (v.I == 1 ? 0 : v.I == 2 ? 1 : 2) * 8 + (v.jerk ? 4 : 0) + (v.eps0 ? 2 : 0) +
-           (v.packed ? 1 : 0);
-}
-
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
 
 struct DeviceGuard {  // make the context's device current for the call, restore on exit
@@ -47,7 +40,6 @@ struct nbk_ctx {
     bool own_stream = false;
     long long n_max = 0, ni_max = 0, n_cap = 0;
     int num_sms = 0;
-    int occ[kNumVariants];
 
     RawJ raw{};
     float* pred = nullptr;  // 7 arrays of n_cap floats: x y z m vx vy vz
@@ -134,7 +126,7 @@ void free_all(nbk_ctx* c) {
 }
 
 int do_predict(nbk_ctx* c, long long n_j) {
-    const long long n_pad = round_up(n_j, kTileJ);
+    const long long n_pad = round_up(n_j, kTileJMax);
     TimeScope ts(c, 1);
     NBK_CUDA(c, launch_predict(c->raw, c->t, n_j, n_pad, pred_arr(c, 0), pred_arr(c, 1),
                                pred_arr(c, 2), pred_arr(c, 3), pred_arr(c, 4), pred_arr(c, 5),
@@ -144,29 +136,75 @@ int do_predict(nbk_ctx* c, long long n_j) {
     return NBK_OK;
 }
 
-// Launch shape for (n_i, n_j): which kernel instantiation, how i-tiles and j-tiles are cut.
-void choose_shape(const nbk_ctx* c, long long n_i, long long n_j, uint32_t flags, float eps2,
-                  Variant* v, Decomp* d) {
-    v->jerk = (flags & NBK_JERK) != 0;
-    v->eps0 = (flags & NBK_EPS0) != 0 || eps2 == 0.f;
-    v->packed = c->variant_scalar == 0;
-    int wj = 1, I = 1;
-    if (n_i <= 32) wj = 4;
-    else if (n_i <= 64) wj = 2;
-    else if (n_i >= 4096) I = 2;
-    if (c->force_I > 0 && wj == 1) I = c->force_I;
-    v->I = I;
-    d->n_i = static_cast<int>(n_i);
-    d->wj = wj;
-    d->ti = (kWarps / wj) * 32 * I;
-    d->nit = static_cast<int>((n_i + d->ti - 1) / d->ti);
-    d->njt = static_cast<int>(round_up(n_j, kTileJ) / kTileJ);
-    d->P = static_cast<long long>(d->nit) * d->njt;
-    const long long slots = static_cast<long long>(c->num_sms) * c->occ[variant_key(*v)];
-    d->G = static_cast<int>(d->P < slots ? d->P : slots);
-    const long long W = (d->P + d->G - 1) / d->G;
-    d->maxseg = static_cast<int>((W - 1 + d->njt - 1) / d->njt + 1);
+}  // namespace
+
+// ---------------------------------------------------------------------------- host planner
+// Launch shape for (n_i, n_j): i-particles per thread I (=> warps per CTA), how many warps split
+// each j-tile (wj; the other W / wj warps split the i-tile), the j-tile size tj, and the
+// stream-K cut of the (i-tile, j-tile) pair list over G <= SMs persistent CTAs.
+// Cost model (relative time of the slowest CTA): pairs per CTA x warps x (j-steps per warp per
+// pair x I + fixed per-pair work) / speed(I), speed measured on B200.
+namespace nbk {
+
+void plan_shape(long long n_i, long long n_j, int num_sms, int force_I, size_t max_partial_floats,
+                Variant* v, Decomp* d) {
+    static const int kI[3] = {4, 2, 1};
+    static const double kSpeed[3] = {1.0, 0.96, 0.86};
+    static const int kTj[3] = {256, 128, 64};
+    double best = -1.0;
+    for (int a = 0; a < 3; ++a) {
+        const int I = kI[a];
+        if (force_I > 0 && I != force_I) continue;
+        const int W = warps_of(I);
+        for (int wj = 1; wj <= W; wj *= 2) {
+            if (W % wj) continue;
+            for (int b = 0; b < 3; ++b) {
+                const int tj = kTj[b];
+                if (tj / wj < 4) continue;
+                const long long ti = static_cast<long long>(W / wj) * 32 * I;
+                const long long nit = (n_i + ti - 1) / ti;
+                const long long njt = (n_j + tj - 1) / tj;
+                const long long P = nit * njt;
+                const long long G = P < num_sms ? P : num_sms;
+                const long long per = (P + G - 1) / G;
+                const long long maxseg = (per - 1 + njt - 1) / njt + 1;
+                // wj = 1 always fits the bound of plan_partial_floats_bound(); wider splits may not
+                if (static_cast<size_t>(G) * maxseg * wj * ti * 8 > max_partial_floats) continue;
+                // per-pair time of one CTA: its W warps share the FP32 pipe, each does tj/wj j-steps
+                // for I i-particles plus the per-tile work (barriers, fp64 fold)
+                const double pair = W * ((static_cast<double>(tj) / wj) * I + 6.0 * I + 24.0);
+                const double cost = per * pair / kSpeed[a];
+                if (best < 0.0 || cost < best * (1.0 - 1e-9)) {
+                    best = cost;
+                    v->I = I;
+                    d->n_i = static_cast<int>(n_i);
+                    d->ti = static_cast<int>(ti);
+                    d->tj = tj;
+                    d->wj = wj;
+                    d->nit = static_cast<int>(nit);
+                    d->njt = static_cast<int>(njt);
+                    d->P = P;
+                    d->G = static_cast<int>(G);
+                    d->maxseg = static_cast<int>(maxseg);
+                }
+            }
+        }
+    }
 }
+
+size_t plan_partial_floats(const Decomp& d) {
+    return static_cast<size_t>(d.G) * d.maxseg * d.wj * d.ti * 8;
+}
+
+// G * maxseg * wj * ti <= n_i rounded up to i-tiles + 2 rows of kMaxRowI per CTA (a CTA touches
+// at most (its share of i-tiles) + 2 i-tiles; wj * ti <= kMaxRowI).
+size_t plan_partial_floats_bound(long long ni_max, int num_sms) {
+    return 8 * (static_cast<size_t>(ni_max) + static_cast<size_t>(kMaxRowI) * (3 * static_cast<size_t>(num_sms) + 1));
+}
+
+}  // namespace nbk
+
+namespace {
 
 int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iidx,
                   const float* d_xi, const float* d_vi, float eps2, uint32_t flags) {
@@ -187,9 +225,12 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     }
     Variant v;
     Decomp d;
-    choose_shape(c, n_i, n_j, flags, eps2, &v, &d);
-    const size_t need = static_cast<size_t>(d.G) * d.maxseg * d.wj * d.ti * 8 * sizeof(float);
-    if (need > c->partial_bytes) return NBK_ENOMEM;
+    v.jerk = (flags & NBK_JERK) != 0;
+    v.eps0 = (flags & NBK_EPS0) != 0 || eps2 == 0.f;
+    v.packed = c->variant_scalar == 0;
+    d.G = 0;
+    plan_shape(n_i, n_j, c->num_sms, c->force_I, c->partial_bytes / sizeof(float), &v, &d);
+    if (d.G < 1 || plan_partial_floats(d) * sizeof(float) > c->partial_bytes) return NBK_ENOMEM;
 
     ForceArgs fa;
     fa.j = jpred_of(c);
@@ -202,21 +243,18 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
         NBK_CUDA(c, launch_force(v, fa, c->stream));
     }
     ReduceArgs ra;
-    ra.j = fa.j;
-    ra.i_index = d_iidx; ra.xi = d_xi; ra.vi = d_vi;
     ra.partial = c->d_partial;
     ra.acc = acc; ra.jerk = jerk; ra.pot = pot;
-    ra.eps2 = eps2;
     ra.d = d;
     {
         TimeScope ts(c, 3);
         NBK_CUDA(c, launch_reduce(v, ra, c->stream));
     }
     c->last_launch[0] = d.G;
-    c->last_launch[1] = kThreads;
+    c->last_launch[1] = warps_of(v.I) * 32;
     c->last_launch[2] = v.I;
     c->last_launch[3] = d.wj;
-    c->last_launch[4] = c->occ[variant_key(v)];
+    c->last_launch[4] = d.tj;
     c->last_launch[5] = c->num_sms;
     c->last_launch[6] = static_cast<long long>(force_smem_bytes(v));
     c->last_launch[7] = 2;
@@ -305,18 +343,14 @@ int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cud
         }
         c->n_max = n_max;
         c->ni_max = ni_max;
-        c->n_cap = round_up(n_max, kTileJ);
+        c->n_cap = round_up(n_max, kTileJMax);
         c->raw.cap = c->n_cap;
-        int max_occ = 1;
         for (int I : {1, 2, 4})
             for (int jk = 0; jk < 2 && e == cudaSuccess; ++jk)
                 for (int e0 = 0; e0 < 2 && e == cudaSuccess; ++e0)
                     for (int pk = 0; pk < 2 && e == cudaSuccess; ++pk) {
                         Variant v{I, jk != 0, e0 != 0, pk != 0};
-                        const int o = force_occupancy(v, &e);
-                        if (e == cudaSuccess && o < 1) e = cudaErrorLaunchOutOfResources;
-                        c->occ[variant_key(v)] = o;
-                        if (o > max_occ) max_occ = o;
+                        e = force_prepare(v);
                     }
         if (e != cudaSuccess) break;
         const size_t cap = static_cast<size_t>(c->n_cap);
@@ -340,9 +374,7 @@ int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cud
         if ((e = cudaMalloc(&c->d_vi, sizeof(float) * 3 * ni)) != cudaSuccess) break;
         if ((e = cudaMalloc(&c->d_result, sizeof(float) * 7 * ni)) != cudaSuccess) break;
         if ((e = cudaMallocHost(&c->h_result, sizeof(float) * 7 * ni)) != cudaSuccess) break;
-        // partial rows: at most (n_i rounded to a tile) + 3 tiles per CTA of slack
-        const size_t g_max = static_cast<size_t>(c->num_sms) * max_occ;
-        c->partial_bytes = 8 * sizeof(float) * (ni + 32 * kMaxI * kWarps * (1 + 3 * g_max));
+        c->partial_bytes = sizeof(float) * plan_partial_floats_bound(ni_max, c->num_sms);
         if ((e = cudaMalloc(&c->d_partial, c->partial_bytes)) != cudaSuccess) break;
         c->stage_bytes = static_cast<size_t>(n_max) * (8 + 8 + 4 * 24 + 4) + 16 * 8;
         if ((e = cudaMallocHost(&c->h_stage, c->stage_bytes)) != cudaSuccess) break;
@@ -567,6 +599,22 @@ int nbk_get_timing(nbk_ctx* c, float ms[4]) {
 int nbk_last_launch(const nbk_ctx* c, int64_t out[8]) {
     if (!c || !out) return NBK_EINVAL;
     for (int k = 0; k < 8; ++k) out[k] = c->last_launch[k];
+    return NBK_OK;
+}
+
+int nbk_plan(int64_t n_i, int64_t n_j, int num_sms, int force_i, int64_t out[12]) {
+    if (n_i < 1 || n_j < 1 || num_sms < 1 || !out || n_i > (1LL << 30) || n_j > (1LL << 30) ||
+        !(force_i == 0 || force_i == 1 || force_i == 2 || force_i == 4))
+        return NBK_EINVAL;
+    Variant v{0, true, false, true};
+    Decomp d;
+    d.G = 0;
+    plan_shape(n_i, n_j, num_sms, force_i, plan_partial_floats_bound(n_i, num_sms), &v, &d);
+    if (d.G < 1) return NBK_ENOMEM;
+    out[0] = v.I; out[1] = warps_of(v.I) * 32; out[2] = d.ti; out[3] = d.tj; out[4] = d.wj;
+    out[5] = d.nit; out[6] = d.njt; out[7] = d.P; out[8] = d.G; out[9] = d.maxseg;
+    out[10] = static_cast<int64_t>(plan_partial_floats(d));
+    out[11] = static_cast<int64_t>(plan_partial_floats_bound(n_i, num_sms));
     return NBK_OK;
 }
 

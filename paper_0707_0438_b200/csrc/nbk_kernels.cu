@@ -5,31 +5,37 @@
 //                        the host, L78 -- moving it here is what north_star asks for)
 //   a4+a5  force_kernel  i-gather + the i x j tile: acc, jerk, potential by direct summation
 //                        (L68; Eq. 1; kernel steps 1-4 L91-L96; softening L126-L132)
-//   a6  reduce_kernel    sum of the split-j partials (L112-L118, on the host in the paper),
-//                        self term removed (L96)
+//   a6  reduce_kernel    sum of the split-j partials (L112-L118, on the host in the paper)
 //
 // What is kept from the paper's 8800GTX design (L89-L102): i-particles live in registers, one
 // thread owns whole i-particles, j-particles stream through shared memory in tiles, no use
-// of Newton's third law (L98).  What is different on sm_100a:
+// of Newton's third law (L98).  What is different on sm_100a (DESIGN.md "Kernels"):
 //   * the inner loop is written in packed f32x2 arithmetic (FFMA2/FADD2/FMUL2): one
-//     instruction handles two j-particles, so the 26 FP32-pipe operations per interaction
-//     use 13 issue slots and the remaining slots carry MUFU, LDS and loop overhead.  The
-//     FP32 pipe (2 cycles per packed instruction, measured) is the bound, not issue.
-//   * 1/s comes from MUFU.RCP instead of a multiply (the XU pipe has the room: 2 of its 8-
-//     cycle slots per 26 FP32-pipe cycles).
-//   * j-tiles are brought in by TMA bulk copies (cp.async.bulk + mbarrier), one elected
-//     thread, 2-deep ring; all lanes read the same shared-memory address (LDS.128 broadcast).
-//   * the (i-tile, j-tile) pair list is cut into G = SMs x CTAs/SM equal contiguous ranges
-//     ("stream-K"): every SM gets the same work for any n_i, n_j; a CTA that crosses an
-//     i-tile boundary writes one partial row per i-tile it touched and reduce_kernel adds
-//     the rows in fp64.  The paper's n_i < 4096 split-j special case (L112) becomes the
-//     general path.
+//     instruction handles two j-particles.  Measured on B200: a packed instruction occupies
+//     the FP32 pipe for 2 cycles (same flop rate as scalar FFMA, half the issue slots), and 3
+//     cycles when its three operands are three distinct register pairs not served by the
+//     operand-reuse cache (register-file read bandwidth is two registers per cycle).
+//   * one persistent CTA per SM (8, 12 or 16 warps for 4, 2 or 1 i-particles per thread).
+//     The warp scheduler favours one CTA over its neighbours on the same SM, so several
+//     independent CTAs per SM end one after the other and the last runs alone; one CTA whose
+//     warps walk the same tile ring finishes together.
+//   * j-tiles are brought in by TMA bulk copies (cp.async.bulk) into a 6-slot ring with one
+//     "full" (transaction-count) and one "empty" (one arrival per warp) mbarrier per slot;
+//     no __syncthreads in the steady state.  All lanes read the same shared-memory address
+//     (LDS.128 broadcast, no bank conflicts).
+//   * the (i-tile, j-tile) pair list is cut into G equal contiguous ranges ("stream-K"):
+//     every SM gets the same work for any n_i, n_j; a CTA that crosses an i-tile boundary
+//     writes one partial row per i-tile it touched and reduce_kernel adds the rows in fp64.
+//     The paper's n_i < 4096 split-j special case (L112) becomes the general path.
 //   * accumulation is hierarchical: fp32 inside one j-tile, fp64 (shared memory, one private
 //     slot per thread) across tiles, fp64 across CTAs -- needed for the 1e-5 potential bound.
+//   * the i-particle's own j entry is left out by INDEX (L96; oracle reading R6): only in the
+//     j-tiles that hold the own entry of one of the warp's i-particles a second copy of the
+//     loop runs that zeroes that entry's mass.  All other tiles run the unmasked loop.
 #include "nbk_kernels.cuh"
 
 #ifndef NBK_USE_RCP
-#define NBK_USE_RCP 1
+#define NBK_USE_RCP 0
 #endif
 
 namespace nbk {
@@ -82,6 +88,9 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
                  : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     uint32_t ok;
     do {
@@ -109,52 +118,198 @@ __host__ __device__ __forceinline__ long long pair_start(long long k, long long 
     return (k * P) / G;
 }
 
-// Shared memory of force_kernel:  [2 mbarriers | pad to 128 B | stages x narr x kTileJ floats |
-// nacc*I x kThreads doubles]
+// Shared memory of force_kernel:
+//   [kStages full mbarriers | kStages empty mbarriers | pad to 128 B]
+//   [kStages x narr x kTileJMax floats]  [nacc*I x threads doubles]
 template <bool JERK>
 struct Shape {
     static constexpr int narr = JERK ? 7 : 4;   // x y z m [vx vy vz]
     static constexpr int nacc = JERK ? 10 : 4;  // ax ay az pot [j1 xyz, j2 xyz]
-    static constexpr int stage_floats = narr * kTileJ;
+    static constexpr int stage_floats = narr * kTileJMax;
 };
 
 template <int I, bool JERK>
 constexpr size_t smem_bytes_of() {
     return 128 + sizeof(float) * kStages * Shape<JERK>::stage_floats +
-           sizeof(double) * Shape<JERK>::nacc * I * kThreads;
+           sizeof(double) * Shape<JERK>::nacc * I * warps_of(I) * 32;
 }
 
-// One elected thread: bring j-tile `jt` into ring slot `slot`.
+// One elected thread: bring j-tile `jt` (tj particles) into a ring slot.
 template <bool JERK>
-__device__ __forceinline__ void issue_tile(const JPred& j, int jt, float* stage, uint32_t bar) {
-    constexpr uint32_t bytes = kTileJ * sizeof(float);
-    const size_t off = static_cast<size_t>(jt) * kTileJ;
+__device__ __forceinline__ void issue_tile(const JPred& j, int jt, int tj, float* stage,
+                                           uint32_t bar) {
+    const uint32_t bytes = tj * sizeof(float);
+    constexpr uint32_t stride = kTileJMax * sizeof(float);
+    const size_t off = static_cast<size_t>(jt) * tj;
     mbar_expect_tx(bar, bytes * Shape<JERK>::narr);
     const uint32_t dst = smem_u32(stage);
-    bulk_g2s(dst + 0 * bytes, j.x + off, bytes, bar);
-    bulk_g2s(dst + 1 * bytes, j.y + off, bytes, bar);
-    bulk_g2s(dst + 2 * bytes, j.z + off, bytes, bar);
-    bulk_g2s(dst + 3 * bytes, j.m + off, bytes, bar);
+    bulk_g2s(dst + 0 * stride, j.x + off, bytes, bar);
+    bulk_g2s(dst + 1 * stride, j.y + off, bytes, bar);
+    bulk_g2s(dst + 2 * stride, j.z + off, bytes, bar);
+    bulk_g2s(dst + 3 * stride, j.m + off, bytes, bar);
     if (JERK) {
-        bulk_g2s(dst + 4 * bytes, j.vx + off, bytes, bar);
-        bulk_g2s(dst + 5 * bytes, j.vy + off, bytes, bar);
-        bulk_g2s(dst + 6 * bytes, j.vz + off, bytes, bar);
+        bulk_g2s(dst + 4 * stride, j.vx + off, bytes, bar);
+        bulk_g2s(dst + 5 * stride, j.vy + off, bytes, bar);
+        bulk_g2s(dst + 6 * stride, j.vz + off, bytes, bar);
     }
 }
 
-// ------------------------------------------------------------------------------ force kernel
-// PAPER.md L91-L96 (kernel steps 1-4), restated for sm_100a as described in the file header.
-// Per ordered pair (i, j), r = x_j - x_i, w = v_j - v_i, s = r.r + eps2:
+// ------------------------------------------------------------------- the i x j tile loops
+// PAPER.md L91-L96 (kernel steps 1-4).  Per ordered pair (i, j), r = x_j - x_i, w = v_j - v_i,
+// s = r.r + eps2:
 //   pot  += m s^-1/2            (sign applied in reduce_kernel)
 //   acc  += m s^-3/2 r
 //   j1   += m s^-3/2 w ;  j2 += m s^-5/2 (r.w) r ;  jerk = j1 - 3 j2 (formed per partial row)
+// The i-state is held negated (r = x_j + (-x_i) is one add).  sl[q] is the position of the
+// i-particle's own j entry inside this tile (anything outside [0, tj) if it is elsewhere);
+// MASK instantiations zero the mass of that entry.
+template <int I, bool JERK, bool EPS0, bool MASK>
+__device__ __forceinline__ void tile_packed(const float* __restrict__ sx, int jbeg, int jend,
+                                            const float (&ni)[I][6], const int (&sl)[I],
+                                            u64 (&acc)[I][Shape<JERK>::nacc], float eps2) {
+    const u64 e2p = pack(eps2, eps2);
+#pragma unroll 1
+    for (int jj = jbeg; jj < jend; jj += 4) {
+        const ulonglong2 X = *reinterpret_cast<const ulonglong2*>(sx + jj);
+        const ulonglong2 Y = *reinterpret_cast<const ulonglong2*>(sx + kTileJMax + jj);
+        const ulonglong2 Z = *reinterpret_cast<const ulonglong2*>(sx + 2 * kTileJMax + jj);
+        const ulonglong2 M = *reinterpret_cast<const ulonglong2*>(sx + 3 * kTileJMax + jj);
+        ulonglong2 VX, VY, VZ;
+        if (JERK) {
+            VX = *reinterpret_cast<const ulonglong2*>(sx + 4 * kTileJMax + jj);
+            VY = *reinterpret_cast<const ulonglong2*>(sx + 5 * kTileJMax + jj);
+            VZ = *reinterpret_cast<const ulonglong2*>(sx + 6 * kTileJMax + jj);
+        }
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const u64 xj = h ? X.y : X.x, yj = h ? Y.y : Y.x, zj = h ? Z.y : Z.x;
+            const u64 mj0 = h ? M.y : M.x;
+#pragma unroll
+            for (int q = 0; q < I; ++q) {
+                u64 mj = mj0;
+                if (MASK) {  // the i-particle's own entry contributes nothing
+                    float mlo, mhi;
+                    unpack(mj0, mlo, mhi);
+                    mlo = (jj + 2 * h == sl[q]) ? 0.f : mlo;
+                    mhi = (jj + 2 * h + 1 == sl[q]) ? 0.f : mhi;
+                    mj = pack(mlo, mhi);
+                }
+                const u64 dx = add2(xj, pack(ni[q][0], ni[q][0]));
+                const u64 dy = add2(yj, pack(ni[q][1], ni[q][1]));
+                const u64 dz = add2(zj, pack(ni[q][2], ni[q][2]));
+                u64 r2 = fma2(dx, dx, e2p);
+                r2 = fma2(dy, dy, r2);
+                r2 = fma2(dz, dz, r2);
+                float r2a, r2b;
+                unpack(r2, r2a, r2b);
+                float ra = rsq(r2a), rb = rsq(r2b);
+                u64 rinv, rinv2;
+                if (EPS0) {  // zero-distance pairs contribute nothing
+                    ra = r2a > 0.f ? ra : 0.f;
+                    rb = r2b > 0.f ? rb : 0.f;
+                    rinv = pack(ra, rb);
+                    rinv2 = mul2(rinv, rinv);
+                } else if (NBK_USE_RCP) {
+                    rinv = pack(ra, rb);
+                    rinv2 = pack(rcp(r2a), rcp(r2b));
+                } else {
+                    rinv = pack(ra, rb);
+                    rinv2 = mul2(rinv, rinv);
+                }
+                const u64 mrinv = mul2(mj, rinv);
+                acc[q][3] = add2(acc[q][3], mrinv);
+                const u64 mrinv3 = mul2(mrinv, rinv2);
+                acc[q][0] = fma2(mrinv3, dx, acc[q][0]);
+                acc[q][1] = fma2(mrinv3, dy, acc[q][1]);
+                acc[q][2] = fma2(mrinv3, dz, acc[q][2]);
+                if (JERK) {
+                    const u64 vxj = h ? VX.y : VX.x, vyj = h ? VY.y : VY.x, vzj = h ? VZ.y : VZ.x;
+                    const u64 dvx = add2(vxj, pack(ni[q][3], ni[q][3]));
+                    const u64 dvy = add2(vyj, pack(ni[q][4], ni[q][4]));
+                    const u64 dvz = add2(vzj, pack(ni[q][5], ni[q][5]));
+                    u64 rv = mul2(dx, dvx);
+                    rv = fma2(dy, dvy, rv);
+                    rv = fma2(dz, dvz, rv);
+                    acc[q][4] = fma2(mrinv3, dvx, acc[q][4]);
+                    acc[q][5] = fma2(mrinv3, dvy, acc[q][5]);
+                    acc[q][6] = fma2(mrinv3, dvz, acc[q][6]);
+                    const u64 beta = mul2(mul2(rv, rinv2), mrinv3);
+                    acc[q][7] = fma2(beta, dx, acc[q][7]);
+                    acc[q][8] = fma2(beta, dy, acc[q][8]);
+                    acc[q][9] = fma2(beta, dz, acc[q][9]);
+                }
+            }
+        }
+    }
+}
+
+template <int I, bool JERK, bool EPS0, bool MASK>
+__device__ __forceinline__ void tile_scalar(const float* __restrict__ sx, int jbeg, int jend,
+                                            const float (&ni)[I][6], const int (&sl)[I],
+                                            float (&acc)[I][Shape<JERK>::nacc], float eps2) {
+#pragma unroll 2
+    for (int jj = jbeg; jj < jend; ++jj) {
+        const float xj = sx[jj], yj = sx[kTileJMax + jj], zj = sx[2 * kTileJMax + jj];
+        const float mj0 = sx[3 * kTileJMax + jj];
+        float vxj = 0.f, vyj = 0.f, vzj = 0.f;
+        if (JERK) {
+            vxj = sx[4 * kTileJMax + jj]; vyj = sx[5 * kTileJMax + jj]; vzj = sx[6 * kTileJMax + jj];
+        }
+#pragma unroll
+        for (int q = 0; q < I; ++q) {
+            const float mj = (MASK && jj == sl[q]) ? 0.f : mj0;
+            const float dx = xj + ni[q][0], dy = yj + ni[q][1], dz = zj + ni[q][2];
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
+            float rinv = rsq(r2);
+            if (EPS0) rinv = r2 > 0.f ? rinv : 0.f;
+            const float rinv2 = (!EPS0 && NBK_USE_RCP) ? rcp(r2) : rinv * rinv;
+            const float mrinv = mj * rinv;
+            acc[q][3] += mrinv;
+            const float mrinv3 = mrinv * rinv2;
+            acc[q][0] = fmaf(mrinv3, dx, acc[q][0]);
+            acc[q][1] = fmaf(mrinv3, dy, acc[q][1]);
+            acc[q][2] = fmaf(mrinv3, dz, acc[q][2]);
+            if (JERK) {
+                const float dvx = vxj + ni[q][3], dvy = vyj + ni[q][4], dvz = vzj + ni[q][5];
+                const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+                acc[q][4] = fmaf(mrinv3, dvx, acc[q][4]);
+                acc[q][5] = fmaf(mrinv3, dvy, acc[q][5]);
+                acc[q][6] = fmaf(mrinv3, dvz, acc[q][6]);
+                const float beta = (rv * rinv2) * mrinv3;
+                acc[q][7] = fmaf(beta, dx, acc[q][7]);
+                acc[q][8] = fmaf(beta, dy, acc[q][8]);
+                acc[q][9] = fmaf(beta, dz, acc[q][9]);
+            }
+        }
+    }
+}
+
+template <bool PACKED> struct AccT { typedef float type; };
+template <> struct AccT<true> { typedef u64 type; };
+
+__device__ __forceinline__ float acc_take(u64& a) {
+    float lo, hi;
+    unpack(a, lo, hi);
+    a = 0ull;
+    return lo + hi;
+}
+__device__ __forceinline__ float acc_take(float& a) {
+    const float s = a;
+    a = 0.f;
+    return s;
+}
+
+// ------------------------------------------------------------------------------ force kernel
 template <int I, bool JERK, bool EPS0, bool PACKED>
-__global__ void __launch_bounds__(kThreads, (I == 1 ? 4 : (I == 2 ? 3 : 2)))
-force_kernel(const ForceArgs a) {
+__global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceArgs a) {
     using S = Shape<JERK>;
     constexpr int NACC = S::nacc;
+    constexpr int W = warps_of(I);
+    constexpr int T = W * 32;
+    typedef typename AccT<PACKED>::type acc_t;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const uint32_t bar0 = smem_u32(smem_raw);
+    const uint32_t full0 = smem_u32(smem_raw);
+    const uint32_t empty0 = full0 + 8 * kStages;
     float* stages = reinterpret_cast<float*>(smem_raw + 128);
     double* sacc = reinterpret_cast<double*>(smem_raw + 128 +
                                              sizeof(float) * kStages * S::stage_floats);
@@ -170,41 +325,52 @@ force_kernel(const ForceArgs a) {
     const int wjn = d.wj;
     const int wj = warp % wjn;           // which slice of each j-tile this warp takes
     const int wi = warp / wjn;           // which 32*I-wide group of the i-tile
-    const int jlen = kTileJ / wjn;
+    const int jlen = d.tj / wjn;
     const int jbeg = wj * jlen;
 
     const long long p0 = pair_start(blockIdx.x, d.P, d.G);
     const long long p1 = pair_start(blockIdx.x + 1LL, d.P, d.G);
     const int n_local = static_cast<int>(p1 - p0);
     const int it_first = static_cast<int>(p0 / d.njt);
+    const int jt_first = static_cast<int>(p0 - static_cast<long long>(it_first) * d.njt);
 
     if (tid == 0) {
-        mbar_init(bar0, 1);
-        mbar_init(bar0 + 8, 1);
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, W);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < kStages; ++s)
+        for (int s = 0; s < kPrefetch; ++s)
             if (s < n_local)
-                issue_tile<JERK>(a.j, static_cast<int>((p0 + s) % d.njt),
-                                 stages + s * S::stage_floats, bar0 + 8 * s);
+                issue_tile<JERK>(a.j, (jt_first + s) % d.njt, d.tj, stages + s * S::stage_floats,
+                                 full0 + 8 * s);
     }
 
-    // i-state (negated, so r = x_j + (-x_i) is one add) and first-level accumulators
-    u64 nxp[I], nyp[I], nzp[I], nvxp[I], nvyp[I], nvzp[I];   // packed form: value duplicated
-    u64 accp[I][NACC];
-    float nxs[I], nys[I], nzs[I], nvxs[I], nvys[I], nvzs[I]; // scalar form
-    float accs[I][NACC];
-    const u64 e2p = pack(a.eps2, a.eps2);
-    const float e2s = a.eps2;
+    float ni[I][6];     // negated i-state: -x -y -z -vx -vy -vz
+    int self[I];        // the i-particle's own j index, or -1
+    acc_t acc[I][NACC];
 
     int it = it_first;
-    int jt = static_cast<int>(p0 - static_cast<long long>(it_first) * d.njt);
+    int jt = jt_first;
     bool fresh = true;
 
     for (int n = 0; n < n_local; ++n) {
+        // producer: keep the ring kPrefetch tiles ahead; a slot is refilled once every warp has
+        // arrived on its "empty" barrier (tile m - kStages was the slot's previous tenant)
+        if (tid == 0) {
+            const int m = n + kPrefetch;
+            if (m < n_local) {
+                const int slot = m % kStages;
+                if (m >= kStages) mbar_wait(empty0 + 8 * slot, ((m / kStages) - 1) & 1);
+                issue_tile<JERK>(a.j, (jt_first + m) % d.njt, d.tj,
+                                 stages + slot * S::stage_floats, full0 + 8 * slot);
+            }
+        }
         if (fresh) {
             // a4: i-gather (Fig. 1: "Data for particle i is taken directly from global memory")
 #pragma unroll
@@ -212,8 +378,9 @@ force_kernel(const ForceArgs a) {
                 const int il = wi * 32 * I + q * 32 + lane;
                 const long long i = static_cast<long long>(it) * d.ti + il;
                 float x = 0.f, y = 0.f, z = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
-                if (il < d.ti && i < d.n_i) {
-                    const int idx = a.i_index ? a.i_index[i] : static_cast<int>(i);
+                int idx = -1;
+                if (i < d.n_i) {
+                    idx = a.i_index ? a.i_index[i] : static_cast<int>(i);
                     if (idx >= 0) {
                         x = a.j.x[idx]; y = a.j.y[idx]; z = a.j.z[idx];
                         if (JERK) { vx = a.j.vx[idx]; vy = a.j.vy[idx]; vz = a.j.vz[idx]; }
@@ -221,147 +388,50 @@ force_kernel(const ForceArgs a) {
                     if (a.xi) { x = a.xi[3 * i]; y = a.xi[3 * i + 1]; z = a.xi[3 * i + 2]; }
                     if (JERK && a.vi) { vx = a.vi[3 * i]; vy = a.vi[3 * i + 1]; vz = a.vi[3 * i + 2]; }
                 }
-                if (PACKED) {
-                    nxp[q] = pack(-x, -x); nyp[q] = pack(-y, -y); nzp[q] = pack(-z, -z);
-                    nvxp[q] = pack(-vx, -vx); nvyp[q] = pack(-vy, -vy); nvzp[q] = pack(-vz, -vz);
-                } else {
-                    nxs[q] = -x; nys[q] = -y; nzs[q] = -z; nvxs[q] = -vx; nvys[q] = -vy; nvzs[q] = -vz;
-                }
+                ni[q][0] = -x; ni[q][1] = -y; ni[q][2] = -z;
+                ni[q][3] = -vx; ni[q][4] = -vy; ni[q][5] = -vz;
+                self[q] = idx;
 #pragma unroll
                 for (int v = 0; v < NACC; ++v) {
-                    sacc[(q * NACC + v) * kThreads + tid] = 0.0;
-                    accp[q][v] = 0ull;
-                    accs[q][v] = 0.f;
+                    sacc[(q * NACC + v) * T + tid] = 0.0;
+                    acc[q][v] = acc_t(0);
                 }
             }
             fresh = false;
         }
 
         const int slot = n % kStages;
-        mbar_wait(bar0 + 8 * slot, (n / kStages) & 1);
+        mbar_wait(full0 + 8 * slot, (n / kStages) & 1);
         const float* sx = stages + slot * S::stage_floats;
 
-        if (PACKED) {
-#pragma unroll 1
-            for (int jj = jbeg; jj < jbeg + jlen; jj += 4) {
-                const ulonglong2 X = *reinterpret_cast<const ulonglong2*>(sx + jj);
-                const ulonglong2 Y = *reinterpret_cast<const ulonglong2*>(sx + kTileJ + jj);
-                const ulonglong2 Z = *reinterpret_cast<const ulonglong2*>(sx + 2 * kTileJ + jj);
-                const ulonglong2 M = *reinterpret_cast<const ulonglong2*>(sx + 3 * kTileJ + jj);
-                ulonglong2 VX, VY, VZ;
-                if (JERK) {
-                    VX = *reinterpret_cast<const ulonglong2*>(sx + 4 * kTileJ + jj);
-                    VY = *reinterpret_cast<const ulonglong2*>(sx + 5 * kTileJ + jj);
-                    VZ = *reinterpret_cast<const ulonglong2*>(sx + 6 * kTileJ + jj);
-                }
+        // does this tile hold the own entry of one of this warp's i-particles?
+        int sl[I];
+        bool mine = false;
+        const int jbase = jt * d.tj;
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const u64 xj = h ? X.y : X.x, yj = h ? Y.y : Y.x, zj = h ? Z.y : Z.x;
-                    const u64 mj = h ? M.y : M.x;
-#pragma unroll
-                    for (int q = 0; q < I; ++q) {
-                        const u64 dx = add2(xj, nxp[q]), dy = add2(yj, nyp[q]), dz = add2(zj, nzp[q]);
-                        u64 r2 = fma2(dx, dx, e2p);
-                        r2 = fma2(dy, dy, r2);
-                        r2 = fma2(dz, dz, r2);
-                        float r2a, r2b;
-                        unpack(r2, r2a, r2b);
-                        float ra = rsq(r2a), rb = rsq(r2b);
-                        u64 rinv, rinv2;
-                        if (EPS0) {  // zero-distance pairs contribute nothing
-                            ra = r2a > 0.f ? ra : 0.f;
-                            rb = r2b > 0.f ? rb : 0.f;
-                            rinv = pack(ra, rb);
-                            rinv2 = mul2(rinv, rinv);
-                        } else if (NBK_USE_RCP) {
-                            rinv = pack(ra, rb);
-                            rinv2 = pack(rcp(r2a), rcp(r2b));
-                        } else {
-                            rinv = pack(ra, rb);
-                            rinv2 = mul2(rinv, rinv);
-                        }
-                        const u64 mrinv = mul2(mj, rinv);
-                        accp[q][3] = add2(accp[q][3], mrinv);
-                        const u64 mrinv3 = mul2(mrinv, rinv2);
-                        accp[q][0] = fma2(mrinv3, dx, accp[q][0]);
-                        accp[q][1] = fma2(mrinv3, dy, accp[q][1]);
-                        accp[q][2] = fma2(mrinv3, dz, accp[q][2]);
-                        if (JERK) {
-                            const u64 vxj = h ? VX.y : VX.x, vyj = h ? VY.y : VY.x, vzj = h ? VZ.y : VZ.x;
-                            const u64 dvx = add2(vxj, nvxp[q]), dvy = add2(vyj, nvyp[q]),
-                                      dvz = add2(vzj, nvzp[q]);
-                            u64 rv = mul2(dx, dvx);
-                            rv = fma2(dy, dvy, rv);
-                            rv = fma2(dz, dvz, rv);
-                            accp[q][4] = fma2(mrinv3, dvx, accp[q][4]);
-                            accp[q][5] = fma2(mrinv3, dvy, accp[q][5]);
-                            accp[q][6] = fma2(mrinv3, dvz, accp[q][6]);
-                            const u64 beta = mul2(mul2(rv, rinv2), mrinv3);
-                            accp[q][7] = fma2(beta, dx, accp[q][7]);
-                            accp[q][8] = fma2(beta, dy, accp[q][8]);
-                            accp[q][9] = fma2(beta, dz, accp[q][9]);
-                        }
-                    }
-                }
-            }
-        } else {
-#pragma unroll 2
-            for (int jj = jbeg; jj < jbeg + jlen; ++jj) {
-                const float xj = sx[jj], yj = sx[kTileJ + jj], zj = sx[2 * kTileJ + jj];
-                const float mj = sx[3 * kTileJ + jj];
-                float vxj = 0.f, vyj = 0.f, vzj = 0.f;
-                if (JERK) { vxj = sx[4 * kTileJ + jj]; vyj = sx[5 * kTileJ + jj]; vzj = sx[6 * kTileJ + jj]; }
-#pragma unroll
-                for (int q = 0; q < I; ++q) {
-                    const float dx = xj + nxs[q], dy = yj + nys[q], dz = zj + nzs[q];
-                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, e2s)));
-                    float rinv = rsq(r2);
-                    if (EPS0) rinv = r2 > 0.f ? rinv : 0.f;
-                    const float rinv2 = (!EPS0 && NBK_USE_RCP) ? rcp(r2) : rinv * rinv;
-                    const float mrinv = mj * rinv;
-                    accs[q][3] += mrinv;
-                    const float mrinv3 = mrinv * rinv2;
-                    accs[q][0] = fmaf(mrinv3, dx, accs[q][0]);
-                    accs[q][1] = fmaf(mrinv3, dy, accs[q][1]);
-                    accs[q][2] = fmaf(mrinv3, dz, accs[q][2]);
-                    if (JERK) {
-                        const float dvx = vxj + nvxs[q], dvy = vyj + nvys[q], dvz = vzj + nvzs[q];
-                        const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
-                        accs[q][4] = fmaf(mrinv3, dvx, accs[q][4]);
-                        accs[q][5] = fmaf(mrinv3, dvy, accs[q][5]);
-                        accs[q][6] = fmaf(mrinv3, dvz, accs[q][6]);
-                        const float beta = (rv * rinv2) * mrinv3;
-                        accs[q][7] = fmaf(beta, dx, accs[q][7]);
-                        accs[q][8] = fmaf(beta, dy, accs[q][8]);
-                        accs[q][9] = fmaf(beta, dz, accs[q][9]);
-                    }
-                }
-            }
+        for (int q = 0; q < I; ++q) {
+            sl[q] = self[q] - jbase;
+            mine |= static_cast<unsigned>(sl[q]) < static_cast<unsigned>(d.tj);
         }
+        if (__any_sync(0xffffffffu, mine)) {
+            if constexpr (PACKED) tile_packed<I, JERK, EPS0, true>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2);
+            else tile_scalar<I, JERK, EPS0, true>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2);
+        } else {
+            if constexpr (PACKED) tile_packed<I, JERK, EPS0, false>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2);
+            else tile_scalar<I, JERK, EPS0, false>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2);
+        }
+
+        // this warp is done with the ring slot
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty0 + 8 * slot);
 
         // second level: fold this tile's fp32 sums into the thread's private fp64 slots
 #pragma unroll
         for (int q = 0; q < I; ++q) {
 #pragma unroll
-            for (int v = 0; v < NACC; ++v) {
-                float s;
-                if (PACKED) {
-                    float lo, hi;
-                    unpack(accp[q][v], lo, hi);
-                    s = lo + hi;
-                    accp[q][v] = 0ull;
-                } else {
-                    s = accs[q][v];
-                    accs[q][v] = 0.f;
-                }
-                sacc[(q * NACC + v) * kThreads + tid] += static_cast<double>(s);
-            }
+            for (int v = 0; v < NACC; ++v)
+                sacc[(q * NACC + v) * T + tid] += static_cast<double>(acc_take(acc[q][v]));
         }
-
-        __syncthreads();  // every warp is done with ring slot `slot`
-        if (tid == 0 && n + kStages < n_local)
-            issue_tile<JERK>(a.j, static_cast<int>((p0 + n + kStages) % d.njt),
-                             stages + slot * S::stage_floats, bar0 + 8 * slot);
 
         const bool last_of_tile = (jt == d.njt - 1) || (n == n_local - 1);
         if (last_of_tile) {
@@ -371,25 +441,23 @@ force_kernel(const ForceArgs a) {
 #pragma unroll
             for (int q = 0; q < I; ++q) {
                 const int il = wi * 32 * I + q * 32 + lane;
-                if (il < d.ti) {
-                    const double* sa = sacc + (q * NACC) * kThreads + tid;
-                    float4 o0, o1;
-                    o0.x = static_cast<float>(sa[0 * kThreads]);
-                    o0.y = static_cast<float>(sa[1 * kThreads]);
-                    o0.z = static_cast<float>(sa[2 * kThreads]);
-                    o0.w = static_cast<float>(sa[3 * kThreads]);
-                    if (JERK) {
-                        o1.x = static_cast<float>(sa[4 * kThreads] - 3.0 * sa[7 * kThreads]);
-                        o1.y = static_cast<float>(sa[5 * kThreads] - 3.0 * sa[8 * kThreads]);
-                        o1.z = static_cast<float>(sa[6 * kThreads] - 3.0 * sa[9 * kThreads]);
-                    } else {
-                        o1.x = o1.y = o1.z = 0.f;
-                    }
-                    o1.w = 0.f;
-                    float4* dst = reinterpret_cast<float4*>(a.partial + (row * d.ti + il) * 8);
-                    dst[0] = o0;
-                    dst[1] = o1;
+                const double* sa = sacc + (q * NACC) * T + tid;
+                float4 o0, o1;
+                o0.x = static_cast<float>(sa[0 * T]);
+                o0.y = static_cast<float>(sa[1 * T]);
+                o0.z = static_cast<float>(sa[2 * T]);
+                o0.w = static_cast<float>(sa[3 * T]);
+                if (JERK) {
+                    o1.x = static_cast<float>(sa[4 * T] - 3.0 * sa[7 * T]);
+                    o1.y = static_cast<float>(sa[5 * T] - 3.0 * sa[8 * T]);
+                    o1.z = static_cast<float>(sa[6 * T] - 3.0 * sa[9 * T]);
+                } else {
+                    o1.x = o1.y = o1.z = 0.f;
                 }
+                o1.w = 0.f;
+                float4* dst = reinterpret_cast<float4*>(a.partial + (row * d.ti + il) * 8);
+                dst[0] = o0;
+                dst[1] = o1;
             }
             fresh = true;
         }
@@ -410,26 +478,31 @@ force_kernel(const ForceArgs a) {
 
 // ----------------------------------------------------------------------------- reduce kernel
 // PAPER.md L118 ("stored in global memory, after which they are ... summed", done on the host
-// there); L96 ("the self interaction of the potential value is removed").
-// grid = ceil(n_i / 32), block = (32, 8): 32 i-particles x 8 lanes over the partial rows.
-template <bool JERK, bool EPS0>
-__global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a) {
-    __shared__ double sh[7][8][32];
+// there).  256 threads = ix i-particles x (256 / ix) lanes over the partial rows; ix = 32 for
+// n_i >= 32, else the next power of two >= n_i so that small blocks still use every thread.
+template <bool JERK>
+__global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_log2) {
+    __shared__ double sh[7][256];
     const Decomp& d = a.d;
-    const int tx = threadIdx.x, ty = threadIdx.y;
-    const long long i = static_cast<long long>(blockIdx.x) * 32 + tx;
+    const int ix = 1 << ix_log2, ry = 256 >> ix_log2;
+    const int tid = threadIdx.x;
+    const int tx = tid & (ix - 1), ty = tid >> ix_log2;
+    const long long i = static_cast<long long>(blockIdx.x) * ix + tx;
     const bool valid = i < d.n_i;
     double s[7] = {0, 0, 0, 0, 0, 0, 0};
     if (valid) {
         const int it = static_cast<int>(i / d.ti);
         const int il = static_cast<int>(i - static_cast<long long>(it) * d.ti);
         const long long lo = static_cast<long long>(it) * d.njt, hi = lo + d.njt - 1;
+        // CTAs k0..k1 own the pairs [lo, hi] of this i-tile
         long long k0 = (lo * d.G) / d.P;
         while (k0 + 1 < d.G && pair_start(k0 + 1, d.P, d.G) <= lo) ++k0;
+        while (k0 > 0 && pair_start(k0, d.P, d.G) > lo) --k0;
         long long k1 = (hi * d.G) / d.P;
         while (k1 + 1 < d.G && pair_start(k1 + 1, d.P, d.G) <= hi) ++k1;
+        while (k1 > 0 && pair_start(k1, d.P, d.G) > hi) --k1;
         const int nrows = static_cast<int>(k1 - k0 + 1) * d.wj;
-        for (int r = ty; r < nrows; r += 8) {
+        for (int r = ty; r < nrows; r += ry) {
             const long long k = k0 + r / d.wj;
             const int w = r % d.wj;
             const int seg = it - static_cast<int>(pair_start(k, d.P, d.G) / d.njt);
@@ -444,49 +517,23 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a) {
         }
     }
 #pragma unroll
-    for (int v = 0; v < 7; ++v) sh[v][ty][tx] = s[v];
+    for (int v = 0; v < 7; ++v) sh[v][tid] = s[v];
     __syncthreads();
+    for (int st = ry >> 1; st > 0; st >>= 1) {   // fixed-order tree: deterministic result
+        if (ty < st) {
+#pragma unroll
+            for (int v = 0; v < 7; ++v) sh[v][tid] += sh[v][tid + st * ix];
+        }
+        __syncthreads();
+    }
     if (ty == 0 && valid) {
-#pragma unroll
-        for (int v = 0; v < 7; ++v) {
-            double t = 0.0;
-#pragma unroll
-            for (int r = 0; r < 8; ++r) t += sh[v][r][tx];
-            s[v] = t;
-        }
-        // remove the i-particle's own j entry: the same fp32 pair arithmetic as force_kernel
-        const int idx = a.i_index ? a.i_index[i] : static_cast<int>(i);
-        if (idx >= 0) {
-            const float xj = a.j.x[idx], yj = a.j.y[idx], zj = a.j.z[idx], mj = a.j.m[idx];
-            float x = xj, y = yj, z = zj, vx = 0.f, vy = 0.f, vz = 0.f, vxj = 0.f, vyj = 0.f, vzj = 0.f;
-            if (JERK) { vxj = a.j.vx[idx]; vyj = a.j.vy[idx]; vzj = a.j.vz[idx]; vx = vxj; vy = vyj; vz = vzj; }
-            if (a.xi) { x = a.xi[3 * i]; y = a.xi[3 * i + 1]; z = a.xi[3 * i + 2]; }
-            if (JERK && a.vi) { vx = a.vi[3 * i]; vy = a.vi[3 * i + 1]; vz = a.vi[3 * i + 2]; }
-            const float dx = xj + (-x), dy = yj + (-y), dz = zj + (-z);
-            const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, a.eps2)));
-            float rinv = rsq(r2);
-            if (EPS0) rinv = r2 > 0.f ? rinv : 0.f;
-            const float rinv2 = (!EPS0 && NBK_USE_RCP) ? rcp(r2) : rinv * rinv;
-            const float mrinv = mj * rinv;
-            const float mrinv3 = mrinv * rinv2;
-            s[3] -= mrinv;
-            s[0] -= mrinv3 * dx; s[1] -= mrinv3 * dy; s[2] -= mrinv3 * dz;
-            if (JERK) {
-                const float dvx = vxj + (-vx), dvy = vyj + (-vy), dvz = vzj + (-vz);
-                const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
-                const float beta = (rv * rinv2) * mrinv3;
-                s[4] -= static_cast<double>(mrinv3 * dvx) - 3.0 * static_cast<double>(beta * dx);
-                s[5] -= static_cast<double>(mrinv3 * dvy) - 3.0 * static_cast<double>(beta * dy);
-                s[6] -= static_cast<double>(mrinv3 * dvz) - 3.0 * static_cast<double>(beta * dz);
-            }
-        }
-        a.acc[3 * i + 0] = static_cast<float>(s[0]);
-        a.acc[3 * i + 1] = static_cast<float>(s[1]);
-        a.acc[3 * i + 2] = static_cast<float>(s[2]);
-        a.pot[i] = static_cast<float>(-s[3]);
-        a.jerk[3 * i + 0] = static_cast<float>(s[4]);
-        a.jerk[3 * i + 1] = static_cast<float>(s[5]);
-        a.jerk[3 * i + 2] = static_cast<float>(s[6]);
+        a.acc[3 * i + 0] = static_cast<float>(sh[0][tid]);
+        a.acc[3 * i + 1] = static_cast<float>(sh[1][tid]);
+        a.acc[3 * i + 2] = static_cast<float>(sh[2][tid]);
+        a.pot[i] = static_cast<float>(-sh[3][tid]);
+        a.jerk[3 * i + 0] = static_cast<float>(sh[4][tid]);
+        a.jerk[3 * i + 1] = static_cast<float>(sh[5][tid]);
+        a.jerk[3 * i + 2] = static_cast<float>(sh[6][tid]);
     }
 }
 
@@ -541,20 +588,21 @@ __global__ void predict_kernel(const RawJ raw, double t, long long n_j, long lon
 
 // --------------------------------------------------------------------------------- launchers
 template <int I, bool JERK, bool EPS0, bool PACKED>
-static int occupancy_of(cudaError_t* err) {
+static cudaError_t prepare_of() {
     auto fn = force_kernel<I, JERK, EPS0, PACKED>;
     const size_t smem = smem_bytes_of<I, JERK>();
-    *err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
-    if (*err != cudaSuccess) return -1;
+    cudaError_t err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           static_cast<int>(smem));
+    if (err != cudaSuccess) return err;
     int nb = 0;
-    *err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, kThreads, smem);
-    if (*err != cudaSuccess) return -1;
-    return nb;
+    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, warps_of(I) * 32, smem);
+    if (err != cudaSuccess) return err;
+    return nb >= 1 ? cudaSuccess : cudaErrorLaunchOutOfResources;
 }
 
 template <int I, bool JERK, bool EPS0, bool PACKED>
 static cudaError_t launch_of(const ForceArgs& a, cudaStream_t s) {
-    force_kernel<I, JERK, EPS0, PACKED><<<a.d.G, kThreads, smem_bytes_of<I, JERK>(), s>>>(a);
+    force_kernel<I, JERK, EPS0, PACKED><<<a.d.G, warps_of(I) * 32, smem_bytes_of<I, JERK>(), s>>>(a);
     return cudaGetLastError();
 }
 
@@ -592,25 +640,23 @@ static cudaError_t launch_of(const ForceArgs& a, cudaStream_t s) {
 
 size_t force_smem_bytes(const Variant& v) {
     const int nacc = v.jerk ? 10 : 4, narr = v.jerk ? 7 : 4;
-    return 128 + sizeof(float) * kStages * narr * kTileJ + sizeof(double) * nacc * v.I * kThreads;
+    return 128 + sizeof(float) * kStages * narr * kTileJMax +
+           sizeof(double) * nacc * v.I * warps_of(v.I) * 32;
 }
 
-int force_occupancy(const Variant& v, cudaError_t* err) { NBK_DISPATCH(occupancy_of, err); }
+cudaError_t force_prepare(const Variant& v) { NBK_DISPATCH(prepare_of); }
 
 cudaError_t launch_force(const Variant& v, const ForceArgs& a, cudaStream_t s) {
     NBK_DISPATCH(launch_of, a, s);
 }
 
 cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s) {
-    const dim3 block(32, 8);
-    const unsigned grid = static_cast<unsigned>((a.d.n_i + 31) / 32);
-    if (v.jerk) {
-        if (v.eps0) reduce_kernel<true, true><<<grid, block, 0, s>>>(a);
-        else reduce_kernel<true, false><<<grid, block, 0, s>>>(a);
-    } else {
-        if (v.eps0) reduce_kernel<false, true><<<grid, block, 0, s>>>(a);
-        else reduce_kernel<false, false><<<grid, block, 0, s>>>(a);
-    }
+    int ix_log2 = 5;
+    while (ix_log2 > 0 && (1 << (ix_log2 - 1)) >= a.d.n_i) --ix_log2;
+    const int ix = 1 << ix_log2;
+    const unsigned grid = static_cast<unsigned>((a.d.n_i + ix - 1) / ix);
+    if (v.jerk) reduce_kernel<true><<<grid, 256, 0, s>>>(a, ix_log2);
+    else reduce_kernel<false><<<grid, 256, 0, s>>>(a, ix_log2);
     return cudaGetLastError();
 }
 

@@ -6,13 +6,16 @@
 
 namespace nbk {
 
-constexpr int kThreads = 128;   // threads per CTA of the force kernel (4 warps)
-constexpr int kWarps = kThreads / 32;
-constexpr int kTileJ = 256;     // j-particles per shared-memory tile (1 KB per array)
-constexpr int kStages = 2;      // tile ring depth (TMA bulk copies run one tile ahead)
+constexpr int kTileJMax = 256;  // largest j-tile (particles); ring slots are sized for it
+constexpr int kStages = 6;      // tile ring depth
+constexpr int kPrefetch = 4;    // tiles the producer runs ahead (kStages - kPrefetch = drift slack)
 constexpr int kMaxI = 4;        // max i-particles per thread
+constexpr int kMaxRowI = 1024;  // max (warps * 32 * I): i-rows one CTA writes per (segment)
 
-// Predicted j-state, structure of arrays, each padded to a multiple of kTileJ with m = 0.
+// warps per CTA for each i-per-thread count: one CTA per SM, registers decide the warp count
+__host__ __device__ constexpr int warps_of(int I) { return I == 4 ? 8 : (I == 2 ? 12 : 16); }
+
+// Predicted j-state, structure of arrays, each padded to a multiple of kTileJMax with m = 0.
 struct JPred {
     const float* x;
     const float* y;
@@ -27,14 +30,31 @@ struct JPred {
 // pair p = it * njt + jt;  CTA k owns pairs [k*P/G, (k+1)*P/G).
 struct Decomp {
     int n_i;          // active i-particles
-    int ti;           // i-particles per CTA tile = wi * 32 * I
-    int wj;           // warps that split each j-tile (1, 2 or 4); wi = kWarps / wj
+    int ti;           // i-particles per CTA tile = (W / wj) * 32 * I
+    int tj;           // j-particles per tile (64, 128 or 256)
+    int wj;           // warps that split each j-tile; W / wj warps split the i-tile
     int nit;          // i-tiles
     int njt;          // j-tiles
     long long P;      // nit * njt
     int G;            // CTAs
     int maxseg;       // max i-tiles one CTA touches
 };
+
+struct Variant {
+    int I;        // 1, 2 or 4
+    bool jerk;
+    bool eps0;
+    bool packed;  // f32x2 inner loop
+};
+
+// Host-only planner (nbk_api.cu): choose I, wj, tj and the pair split for (n_i, n_j).
+// force_I > 0 pins I.  Fills *v (I only; flags are the caller's) and *d; candidates whose partial
+// rows exceed max_partial_floats are skipped (d->G stays untouched if none fits).
+void plan_shape(long long n_i, long long n_j, int num_sms, int force_I, size_t max_partial_floats,
+                Variant* v, Decomp* d);
+// Floats of partial storage a plan needs, and the bound nbk_open allocates for (ni_max, num_sms).
+size_t plan_partial_floats(const Decomp& d);
+size_t plan_partial_floats_bound(long long ni_max, int num_sms);
 
 struct ForceArgs {
     JPred j;
@@ -47,15 +67,10 @@ struct ForceArgs {
 };
 
 struct ReduceArgs {
-    JPred j;
-    const int32_t* i_index;
-    const float* xi;
-    const float* vi;
     const float* partial;
     float* acc;   // [n_i][3]
     float* jerk;  // [n_i][3]
     float* pot;   // [n_i]
-    float eps2;
     Decomp d;
 };
 
@@ -69,17 +84,9 @@ struct RawJ {        // raw j-state kept for the predictor, structure of arrays 
     long long cap;
 };
 
-struct Variant {
-    int I;        // 1, 2 or 4
-    bool jerk;
-    bool eps0;
-    bool packed;  // f32x2 inner loop
-};
-
 size_t force_smem_bytes(const Variant& v);
-// CTAs of this variant that fit one SM (queried once per variant; also raises the dynamic
-// shared-memory limit of the instantiation).  Returns <= 0 and sets *err on failure.
-int force_occupancy(const Variant& v, cudaError_t* err);
+// Raises the dynamic shared-memory limit of the instantiation and checks that one CTA fits an SM.
+cudaError_t force_prepare(const Variant& v);
 cudaError_t launch_force(const Variant& v, const ForceArgs& a, cudaStream_t s);
 cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s);
 
