@@ -1,0 +1,322 @@
+"""GPU parity at BASELINE.json's configs C2-C5, in the launch shapes bench.py times, plus the
+degenerate cases of the method.  Everything goes through the C ABI (via the thin binding); the
+expected values come from oracle/ on the same seeded inputs.  Tolerances: tests/parity.py.
+
+Run on the B200 box:  python -m pytest tests -m gpu -x -q
+"""
+import numpy as np
+import pytest
+
+from paper_0707_0438_b200 import binding as nb
+from paper_0707_0438_b200 import inputs
+from parity import assert_parity, scalar_rel_err, vec_rel_err
+
+pytestmark = pytest.mark.gpu
+
+EPS = inputs.EPS_PAPER
+FULL = nb.NBK_JERK | nb.NBK_POT
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests have no fallback")
+    nb.load()
+    return torch
+
+
+class Ctx:
+    def __init__(self, n_max, ni_max=None, stream=0):
+        self.h = nb.nbk_open(0, n_max, ni_max or n_max, stream)
+
+    def __enter__(self):
+        return self.h
+
+    def __exit__(self, *a):
+        nb.nbk_close(self.h)
+
+
+# ----------------------------------------------------------------------------- config 2
+@pytest.fixture(scope="module")
+def c2(c_oracle):
+    """N=16384, seed 2; per-particle a, jerk = the oracle's force at t_j = 0 rounded to fp32
+    (DESIGN.md input recipe: 'seeded a and jerk'); prediction time t = 0.01."""
+    m, x, v = inputs.config_inputs("C2")
+    a, jk, _ = c_oracle.force(m, x, v, EPS)
+    a32, j32 = a.astype(np.float32), jk.astype(np.float32)
+    tj = np.zeros(m.shape[0])
+    xp, vp = c_oracle.predict(0.01, tj, x, v, a32, j32)
+    return dict(m=m, x=x, v=v, a=a32, jerk=j32, tj=tj, t=0.01, xp=xp, vp=vp)
+
+
+def test_c2_predictor_matches_fp64_oracle(gpu, c2):
+    """a3: device prediction vs fp64 oracle: one fp32 rounding of the fp64 result."""
+    n = c2["m"].shape[0]
+    with Ctx(n) as ctx:
+        nb.nbk_set_j_particles(ctx, None, c2["tj"], c2["m"], c2["x"], c2["v"], c2["a"], c2["jerk"])
+        nb.nbk_set_ti(ctx, c2["t"])
+        nb.nbk_predict(ctx, n)
+        gm, gx, gv = nb.nbk_get_predicted(ctx, n)
+    assert np.array_equal(gm, c2["m"])
+    # the device evaluates the same fp64 polynomial (possibly with FMA contraction) and rounds
+    # once: at most 1 ulp of fp32 from the correctly rounded oracle value
+    for got, ref in ((gx, c2["xp"]), (gv, c2["vp"])):
+        ulp = np.spacing(np.abs(ref).astype(np.float32)).astype(np.float64)
+        assert np.all(np.abs(got.astype(np.float64) - ref) <= 1.0 * ulp)
+        assert np.mean(got == ref.astype(np.float32)) > 0.99
+
+
+@pytest.mark.parametrize("n_i", [1, 32, 256, 2048, 16384])
+def test_c2_block_step_sweep(gpu, c_oracle, c2, n_i):
+    """a4-a7 for i-blocks 'drawn uniformly without replacement' after device prediction:
+    (ii) kernel isolated: oracle on the GPU-predicted fp32 state; (iii) end to end: oracle
+    prediction + oracle force in fp64."""
+    n = c2["m"].shape[0]
+    idx = inputs.active_block(n, n_i, seed=2)
+    with Ctx(n) as ctx:
+        nb.nbk_set_j_particles(ctx, None, c2["tj"], c2["m"], c2["x"], c2["v"], c2["a"], c2["jerk"])
+        nb.nbk_set_ti(ctx, c2["t"])
+        nb.nbk_calc_firsthalf(ctx, n, n_i, idx, None, None, np.float32(EPS) ** 2, FULL)
+        got = nb.nbk_calc_lasthalf(ctx, n_i)
+        shape = nb.nbk_last_launch(ctx)
+        gm, gx, gv = nb.nbk_get_predicted(ctx, n)
+    assert shape["launches"] == 2 and shape["grid"] >= min(128, shape["sms"])
+    ref_kernel = c_oracle.force(gm, gx, gv, EPS, i_index=idx)
+    assert_parity(got, ref_kernel, what=f"C2 n_i={n_i} kernel-only")
+    ref_e2e = c_oracle.force(c2["m"], c2["xp"], c2["vp"], EPS, i_index=idx)
+    assert_parity(got, ref_e2e, what=f"C2 n_i={n_i} end-to-end")
+
+
+def test_c2_stress_mixed_times_gaussian_derivatives(gpu, c_oracle):
+    """Predictor stress: per-particle t_j = t - 2^-k (k in 7..12), Gaussian a, jerk of matched rms."""
+    m, x, v = inputs.config_inputs("C2")
+    n = m.shape[0]
+    t = 0.01
+    tj = inputs.particle_times(n, t, seed=2)
+    a, jk = inputs.gaussian_derivatives(n, seed=2)
+    xp, vp = c_oracle.predict(t, tj, x, v, a, jk)
+    idx = inputs.active_block(n, 2048, seed=3)
+    with Ctx(n) as ctx:
+        nb.nbk_set_j_particles(ctx, None, tj, m, x, v, a, jk)
+        nb.nbk_set_ti(ctx, t)
+        nb.nbk_calc_firsthalf(ctx, n, 2048, idx, None, None, np.float32(EPS) ** 2, FULL)
+        got = nb.nbk_calc_lasthalf(ctx, 2048)
+        gm, gx, gv = nb.nbk_get_predicted(ctx, n)
+    ulp = np.spacing(np.abs(xp).astype(np.float32)).astype(np.float64)
+    assert np.all(np.abs(gx.astype(np.float64) - xp) <= ulp)
+    assert_parity(got, c_oracle.force(m, xp, vp, EPS, i_index=idx), what="C2 stress")
+
+
+# ----------------------------------------------------------------------------- config 3
+@pytest.mark.parametrize("eps", [EPS, 0.0])
+def test_c3_headline_full_parity(gpu, c_oracle, eps):
+    """N=131072 seed 3, all i active, eps=1/256 and eps=0 (self pair excluded): every particle
+    against the C oracle (1.7e10 pairs), in the launch shape bench.py times."""
+    m, x, v = inputs.config_inputs("C3")
+    n = m.shape[0]
+    with Ctx(n) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, n, n, None, None, None, np.float32(eps) ** 2, FULL)
+        got = nb.nbk_calc_lasthalf(ctx, n)
+        shape = nb.nbk_last_launch(ctx)
+    assert shape["grid"] == shape["sms"] and shape["i_per_thread"] == 4
+    ref = c_oracle.force(m, x, v, eps)
+    e = assert_parity(got, ref, what=f"C3 eps={eps}")
+    # momentum: sum m a = 0 for the exact sums; the GPU's is bounded by its per-particle error
+    p = np.abs((m[:, None].astype(np.float64) * got[0]).sum(axis=0)).max()
+    assert p < 1e-6, p
+    print(f"C3 eps={eps}: {e}")
+
+
+# ----------------------------------------------------------------------------- config 4
+def test_c4_million_acc_pot_only_sampled(gpu, c_oracle):
+    """N=1048576 seed 4: acc+pot without jerk for all i; oracle on a seeded 1024-particle subset."""
+    m, x, v = inputs.config_inputs("C4")
+    n = m.shape[0]
+    with Ctx(n) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, None)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, n, n, None, None, None, np.float32(EPS) ** 2, nb.NBK_POT)
+        acc, jrk, pot = nb.nbk_calc_lasthalf(ctx, n)
+    assert np.all(jrk == 0.0)
+    assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot)) and np.all(pot < 0.0)
+    sub = inputs.active_block(n, 1024, seed=4)
+    racc, _, rpot = c_oracle.force(m, x, v, EPS, i_index=sub, want_jerk=False)
+    assert_parity((acc[sub], None, pot[sub]), (racc, None, rpot), jerk=False, what="C4 subset")
+    # a property that holds at any size: W = 1/2 sum m pot ~ -1/2 for the Plummer model in N-body
+    # units (softening and the 99.9 % mass cut move it by a few per cent)
+    w = 0.5 * np.sum(m.astype(np.float64) * pot)
+    assert -0.52 < w < -0.45, w
+
+
+# ----------------------------------------------------------------------------- config 5
+def _energy(c_oracle, m, x, v, eps):
+    _, _, pot = c_oracle.force(m, x, v, eps, want_jerk=False)
+    return 0.5 * np.sum(m * np.sum(v * v, axis=1)) + 0.5 * np.sum(m * pot)
+
+
+def test_c5_hermite_energy_conservation(gpu, c_oracle):
+    """N=65536 seed 5 integrated to t=1 with the host Hermite driver (eta=0.01, dt_max=1/16),
+    device predictor + force per block step: |dE/E| < 1e-6 (BASELINE.json north_star), energy
+    by the fp64 oracle at both ends (Eq. 2)."""
+    m, x, v = inputs.plummer(inputs.CONFIGS["C5"]["N"], inputs.CONFIGS["C5"]["seed"])
+    n = m.shape[0]
+    e0 = _energy(c_oracle, m, x, v, EPS)
+    with Ctx(n) as ctx:
+        st = nb.nbk_hermite_evolve(ctx, m, x, v, EPS, 1.0, eta=0.01, dt_max=1.0 / 16.0)
+    e1 = _energy(c_oracle, m, x, v, EPS)
+    de = abs((e0 - e1) / e0)
+    print(f"C5: dE/E={de:.3e} block_steps={st['block_steps']} particle_steps={st['particle_steps']} "
+          f"wall={st['wall_seconds']:.2f}s gpu_calls={st['gpu_call_seconds']:.2f}s "
+          f"interactions={st['interactions']:.3e}")
+    assert st["t_reached"] == 1.0
+    assert abs(e0 + 0.25) < 0.01
+    assert de < 1e-6, de
+
+
+def test_hermite_small_n_follows_the_fp64_oracle_integrator(gpu):
+    """N=256 to t=0.25: the GPU-driven run and oracle/hermite_oracle.py (same scheme, fp64 forces)
+    take the same block steps at first and end with nearby states and equal energy drift scale."""
+    from oracle import hermite_oracle, nbody_oracle
+    m, x, v = inputs.plummer(256, seed=11)
+    ref = hermite_oracle.evolve(m, x, v, EPS, 0.25)
+    gx, gv = x.copy(), v.copy()
+    with Ctx(256) as ctx:
+        st = nb.nbk_hermite_evolve(ctx, m, gx, gv, EPS, 0.25)
+    assert st["t_reached"] == 0.25
+    # fp32 forces perturb step choices slightly: counts agree to a few per cent
+    assert abs(st["particle_steps"] - ref["particle_steps"]) <= 0.05 * ref["particle_steps"]
+    e0 = nbody_oracle.energy(m, x, v, EPS)
+    assert abs((nbody_oracle.energy(m, gx, gv, EPS) - e0) / e0) < 1e-6
+    assert abs((nbody_oracle.energy(m, ref["x"], ref["v"], EPS) - e0) / e0) < 1e-6
+    # chaotic divergence over 0.25 time units is tiny: positions agree to ~1e-5 typical
+    assert np.median(np.linalg.norm(gx - ref["x"], axis=1)) < 1e-4
+
+
+# ----------------------------------------------------------------------------- degenerate cases
+def test_repeat_runs_are_bitwise_identical(gpu):
+    """Reading R11: fixed work split and fixed-order reductions => same bits run to run."""
+    m, x, v = inputs.plummer_f32(5000, seed=9)
+    idx = inputs.active_block(5000, 777, seed=1)
+    with Ctx(5000) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        outs = []
+        for _ in range(3):
+            nb.nbk_calc_firsthalf(ctx, 5000, 777, idx, None, None, np.float32(EPS) ** 2, FULL)
+            outs.append(nb.nbk_calc_lasthalf(ctx, 777))
+    for o in outs[1:]:
+        for a, b in zip(outs[0], o):
+            assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("eps", [EPS, 0.0])
+def test_duplicate_positions(gpu, c_oracle, eps):
+    """Reading R6: a coincident j != i adds -m_j/eps to pot and nothing to acc, jerk for eps > 0;
+    for eps = 0 the zero-distance pair contributes nothing at all."""
+    m, x, v = inputs.plummer_f32(300, seed=21)
+    x[17] = x[250]
+    x[100] = x[101]
+    v[100] = v[101]
+    ref = c_oracle.force(m, x, v, eps)
+    with Ctx(300) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, 300, 300, None, None, None, np.float32(eps) ** 2, FULL)
+        got = nb.nbk_calc_lasthalf(ctx, 300)
+    assert_parity(got, ref, what=f"duplicates eps={eps}")
+
+
+def test_external_test_particles_and_explicit_i_state(gpu, c_oracle):
+    """i_index = -1: external particle, no j left out; i_index >= 0 with xi/vi given: the explicit
+    state is used and the own j entry is still left out by index."""
+    m, x, v = inputs.plummer_f32(1000, seed=31)
+    rng = np.random.default_rng(5)
+    n_i = 70
+    idx = np.full(n_i, -1, np.int32)
+    idx[::2] = rng.choice(1000, size=idx[::2].size, replace=False)
+    xi = (0.5 * rng.standard_normal((n_i, 3))).astype(np.float32)
+    vi = (0.5 * rng.standard_normal((n_i, 3))).astype(np.float32)
+    ref = c_oracle.force(m, x, v, EPS, i_index=idx, xi=xi, vi=vi)
+    with Ctx(1000) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, 1000, n_i, idx, xi, vi, np.float32(EPS) ** 2, FULL)
+        got = nb.nbk_calc_lasthalf(ctx, n_i)
+    assert_parity(got, ref, what="external / explicit i-state")
+
+
+def test_heavy_particle_self_potential_is_excluded_exactly(gpu, c_oracle):
+    """A particle holding half the mass with tiny softening: m_i/eps = 5e5 |pot|.  Adding and
+    subtracting its self term in fp32 would lose the potential; exclusion by index does not."""
+    m, x, v = inputs.plummer_f32(513, seed=41)
+    m = m.copy()
+    m[300] = 0.5
+    eps = 1e-6
+    ref = c_oracle.force(m, x, v, eps)
+    with Ctx(513) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, 513, 513, None, None, None, np.float32(eps) ** 2, FULL)
+        got = nb.nbk_calc_lasthalf(ctx, 513)
+    assert_parity(got, ref, what="heavy particle")
+
+
+def test_scatter_by_address_f64_and_j_subset(gpu, c_oracle):
+    """a1 with addresses (set_j in two shuffled batches, fp64 entry point) and n_j < loaded n:
+    only j in [0, n_j) act."""
+    m, x, v = inputs.plummer(2000, seed=51)
+    perm = np.random.default_rng(6).permutation(2000).astype(np.int32)
+    with Ctx(2000) as ctx:
+        for part in (perm[:700], perm[700:]):
+            nb.nbk_set_j_particles_f64(ctx, part, None, m[part], x[part], v[part])
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, 1500, 1500, None, None, None, np.float32(EPS) ** 2, FULL)
+        got = nb.nbk_calc_lasthalf(ctx, 1500)
+        gm, gx, gv = nb.nbk_get_predicted(ctx, 1500)
+    assert np.array_equal(gx, x[:1500].astype(np.float32))
+    ref = c_oracle.force(gm, gx, gv, EPS)
+    assert_parity(got, ref, what="scatter + subset")
+
+
+def test_device_pointer_entry_points_on_a_torch_stream(gpu, c_oracle):
+    """_dev variants with torch tensors on a torch stream (PyTorch only owns memory and stream)."""
+    torch = gpu
+    m, x, v = inputs.plummer_f32(3000, seed=61)
+    ref = c_oracle.force(m, x, v, EPS)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        dm, dx, dv = (torch.from_numpy(t).cuda() for t in (m, x, v))
+        acc = torch.empty((3000, 3), dtype=torch.float32, device="cuda")
+        jrk = torch.empty_like(acc)
+        pot = torch.empty(3000, dtype=torch.float32, device="cuda")
+    stream.synchronize()
+    with Ctx(3000, stream=stream.cuda_stream) as ctx:
+        nb.nbk_set_j_particles_dev(ctx, 3000, 0, 0, dm.data_ptr(), dx.data_ptr(), dv.data_ptr())
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf_dev(ctx, 3000, 3000, 0, 0, 0, np.float32(EPS) ** 2, FULL)
+        nb.nbk_calc_lasthalf_dev(ctx, 3000, acc.data_ptr(), jrk.data_ptr(), pot.data_ptr())
+        nb.nbk_sync(ctx)
+        got = (acc.cpu().numpy(), jrk.cpu().numpy(), pot.cpu().numpy())
+    assert_parity(got, ref, what="device entry points")
+
+
+def test_errors_do_not_depend_on_which_kernel_shape_ran(gpu, c_oracle):
+    """Same 4099 x 4099 problem through every i-per-thread shape: each within tolerance of the
+    oracle and within fp32 round-off of one another."""
+    m, x, v = inputs.plummer_f32(4099, seed=71)
+    ref = c_oracle.force(m, x, v, EPS)
+    res = []
+    with Ctx(4099) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        for variant in (0x10, 0x20, 0x40, 0x41):
+            nb.nbk_set_variant(ctx, variant)
+            nb.nbk_calc_firsthalf(ctx, 4099, 4099, None, None, None, np.float32(EPS) ** 2, FULL)
+            res.append(nb.nbk_calc_lasthalf(ctx, 4099))
+            assert_parity(res[-1], ref, what=f"variant {variant:#x}")
+    for r in res[1:]:
+        assert np.percentile(vec_rel_err(r[0], res[0][0]), 99) < 5e-6
+        assert scalar_rel_err(r[2], res[0][2]).max() < 2e-6
