@@ -1,0 +1,60 @@
+"""bench.py host logic at world size 2 on the CPU (gloo): the N > 1 path is 'replicas only'
+ -- value = sum of units over ranks / max time over ranks."""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import torch.distributed as dist
+import bench
+rank, local, world = bench.dist_env()
+dist.init_process_group("gloo", rank=rank, world_size=world)
+ms, units = bench.aggregate(10.0 + 5.0 * rank, 100.0 * (rank + 1), world, "cpu")
+dist.barrier()
+dist.destroy_process_group()
+print(json.dumps({{"rank": rank, "ms": ms, "units": units}}))
+"""
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def test_aggregate_max_time_sum_units_world2(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER.format(root=ROOT))
+    port = _free_port()
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE="2",
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.PIPE, text=True))
+    outs = []
+    for p in procs:
+        out, err = p.communicate(timeout=120)
+        assert p.returncode == 0, err
+        outs.append(json.loads(out.strip().splitlines()[-1]))
+    for o in outs:
+        assert o["ms"] == 15.0 and o["units"] == 300.0
+
+
+def test_aggregate_is_identity_at_world1():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.aggregate(3.5, 7.0, 1, "cpu") == (3.5, 7.0)
+
+
+def test_reference_arm_other_ranks_exit_without_work():
+    env = dict(os.environ, RANK="1", LOCAL_RANK="1", WORLD_SIZE="2")
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
+                       env=env, capture_output=True, text=True, timeout=120)
+    assert p.returncode == 0 and p.stdout.strip() == ""
