@@ -37,6 +37,9 @@
 #ifndef NBK_USE_RCP
 #define NBK_USE_RCP 0
 #endif
+#ifndef NBK_UNROLL
+#define NBK_UNROLL 1   // trips of the 4-j step of the packed tile loop unrolled together
+#endif
 
 namespace nbk {
 
@@ -168,7 +171,8 @@ __device__ __forceinline__ void tile_packed(const float* __restrict__ sx, int jb
                                             const float (&ni)[I][6], const int (&sl)[I],
                                             u64 (&acc)[I][Shape<JERK>::nacc], float eps2) {
     const u64 e2p = pack(eps2, eps2);
-#pragma unroll 1
+    constexpr int kUnroll = NBK_UNROLL;
+#pragma unroll kUnroll
     for (int jj = jbeg; jj < jend; jj += 4) {
         const ulonglong2 X = *reinterpret_cast<const ulonglong2*>(sx + jj);
         const ulonglong2 Y = *reinterpret_cast<const ulonglong2*>(sx + kTileJMax + jj);
