@@ -174,7 +174,8 @@ int nbk_get_timing(nbk_ctx* ctx, float ms[4]);
 /* Launch shape of the last firsthalf: out[0] grid (CTAs, one per SM at most), out[1] threads
  * per CTA, out[2] i-particles per thread, out[3] warps splitting each j-tile, out[4] j-tile
  * size, out[5] SM count, out[6] dynamic shared memory bytes, out[7] number of kernels launched
- * by the last firsthalf. */
+ * by the last firsthalf (2: force + reduce; 1: small block, reduced by the force kernel's last
+ * CTA). */
 int nbk_last_launch(const nbk_ctx* ctx, int64_t out[8]);
 
 /* Host-only (no GPU needed): the launch plan firsthalf would use for (n_i, n_j) on a device with
@@ -186,8 +187,11 @@ int nbk_last_launch(const nbk_ctx* ctx, int64_t out[8]);
  * CTA k works on pairs [k*P/G, (k+1)*P/G) of the i-major (i-tile, j-tile) list. */
 int nbk_plan(int64_t n_i, int64_t n_j, int num_sms, int force_i, int64_t out[12]);
 
-/* Choose the inner-loop form: 0 = packed f32x2 (FFMA2, two j per instruction; default),
- * 1 = scalar fp32.  Both compute the same sums; kept for measurement. */
+/* Measurement knobs.  bit 0: inner-loop form, 0 = packed f32x2 (FFMA2, two j per instruction;
+ * default), 1 = scalar fp32.  bits 4-7: pin the i-particles per thread (1, 2, 4; 0 = planner's
+ * choice).  bit 8: switch off the one-launch path for blocks of <= 32 i-particles (reduction by
+ * the last CTA, indices in the launch parameters, results written to mapped host memory).  All
+ * forms compute the same sums. */
 int nbk_set_variant(nbk_ctx* ctx, int variant);
 
 int nbk_last_cuda_error(const nbk_ctx* ctx);

@@ -53,7 +53,11 @@ struct nbk_ctx {
     float* d_partial = nullptr;
     size_t partial_bytes = 0;
     float* d_result = nullptr;  // acc[3 n_i] | jerk[3 n_i] | pot[n_i] of the last call
-    float* h_result = nullptr;  // pinned
+    float* h_result = nullptr;  // pinned, mapped into the device address space
+    float* h_result_dev = nullptr;  // device view of h_result
+    unsigned* d_counter = nullptr;  // arrival counter of the fused small-block tail
+    bool host_has_result = false;   // the last firsthalf wrote h_result itself (no D2H needed)
+    InlineJ pending;                // a small set_j not yet on the device (pending.n == 0: none)
 
     unsigned char* h_stage = nullptr;  // pinned staging for set_j
     unsigned char* d_stage = nullptr;
@@ -66,6 +70,7 @@ struct nbk_ctx {
     bool in_flight = false;
     int variant_scalar = 0;
     int force_I = 0;
+    bool fused_ok = true;  // nbk_set_variant bit 8 switches the one-launch small-block path off
     int last_cuda = 0;
     long long last_launch[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 
@@ -112,7 +117,7 @@ void free_all(nbk_ctx* c) {
     cudaFree(c->raw.x); cudaFree(c->raw.v); cudaFree(c->raw.a); cudaFree(c->raw.k);
     cudaFree(c->raw.m); cudaFree(c->raw.t); cudaFree(c->pred);
     cudaFree(c->d_iidx); cudaFree(c->d_xi); cudaFree(c->d_vi);
-    cudaFree(c->d_partial); cudaFree(c->d_result); cudaFree(c->d_stage);
+    cudaFree(c->d_partial); cudaFree(c->d_result); cudaFree(c->d_stage); cudaFree(c->d_counter);
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_stage) cudaFreeHost(c->h_stage);
     if (c->h_istage) cudaFreeHost(c->h_istage);
@@ -125,12 +130,29 @@ void free_all(nbk_ctx* c) {
     (void)cudaGetLastError();
 }
 
+// A pending small set_j goes to the device on its own (before anything else touches the raw state).
+int flush_pending(nbk_ctx* c) {
+    if (c->pending.n > 0) {
+        TimeScope ts(c, 0);
+        NBK_CUDA(c, launch_scatter_inline(c->pending, c->raw, c->stream));
+        c->pending.n = 0;
+    }
+    return NBK_OK;
+}
+
 int do_predict(nbk_ctx* c, long long n_j) {
     const long long n_pad = round_up(n_j, kTileJMax);
+    bool fold = c->pending.n > 0;
+    for (int k = 0; k < c->pending.n; ++k) fold = fold && c->pending.addr[k] < n_j;
+    if (!fold) {
+        const int rc = flush_pending(c);
+        if (rc != NBK_OK) return rc;
+    }
     TimeScope ts(c, 1);
     NBK_CUDA(c, launch_predict(c->raw, c->t, n_j, n_pad, pred_arr(c, 0), pred_arr(c, 1),
                                pred_arr(c, 2), pred_arr(c, 3), pred_arr(c, 4), pred_arr(c, 5),
-                               pred_arr(c, 6), c->stream));
+                               pred_arr(c, 6), fold ? &c->pending : nullptr, c->stream));
+    c->pending.n = 0;
     c->pred_valid = true;
     c->pred_nj = n_j;
     return NBK_OK;
@@ -165,11 +187,11 @@ void plan_shape(long long n_i, long long n_j, int num_sms, int force_I, size_t m
                 const long long nit = (n_i + ti - 1) / ti;
                 const long long njt = (n_j + tj - 1) / tj;
                 const long long P = nit * njt;
-                const long long G = P < num_sms ? P : num_sms;
+                const long long gmax = num_sms < kMaxCtas ? num_sms : kMaxCtas;
+                const long long G = P < gmax ? P : gmax;
                 const long long per = (P + G - 1) / G;
                 const long long maxseg = (per - 1 + njt - 1) / njt + 1;
-                // wj = 1 always fits the bound of plan_partial_floats_bound(); wider splits may not
-                if (static_cast<size_t>(G) * maxseg * wj * ti * 8 > max_partial_floats) continue;
+                if (static_cast<size_t>(G) * maxseg * ti * 8 > max_partial_floats) continue;
                 // per-pair time of one CTA: its W warps share the FP32 pipe, each does tj/wj j-steps
                 // for I i-particles plus the per-tile work (barriers, fp64 fold)
                 const double pair = W * ((static_cast<double>(tj) / wj) * I + 6.0 * I + 24.0);
@@ -193,11 +215,11 @@ void plan_shape(long long n_i, long long n_j, int num_sms, int force_I, size_t m
 }
 
 size_t plan_partial_floats(const Decomp& d) {
-    return static_cast<size_t>(d.G) * d.maxseg * d.wj * d.ti * 8;
+    return static_cast<size_t>(d.G) * d.maxseg * d.ti * 8;
 }
 
-// G * maxseg * wj * ti <= n_i rounded up to i-tiles + 2 rows of kMaxRowI per CTA (a CTA touches
-// at most (its share of i-tiles) + 2 i-tiles; wj * ti <= kMaxRowI).
+// G * maxseg * ti <= n_i rounded up to i-tiles + 2 rows of kMaxRowI per CTA (a CTA touches at
+// most (its share of i-tiles) + 2 i-tiles; ti <= kMaxRowI).
 size_t plan_partial_floats_bound(long long ni_max, int num_sms) {
     return 8 * (static_cast<size_t>(ni_max) + static_cast<size_t>(kMaxRowI) * (3 * static_cast<size_t>(num_sms) + 1));
 }
@@ -206,8 +228,11 @@ size_t plan_partial_floats_bound(long long ni_max, int num_sms) {
 
 namespace {
 
+// h_inline: host i-indices to pass in the kernel parameters (small blocks from the host entry
+// point; d_iidx is then unused); to_host: also write the results into the mapped host buffer.
 int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iidx,
-                  const float* d_xi, const float* d_vi, float eps2, uint32_t flags) {
+                  const float* d_xi, const float* d_vi, float eps2, uint32_t flags,
+                  const int32_t* h_inline = nullptr, bool to_host = false) {
     if (!c->pred_valid || c->pred_nj != n_j) {
         const int rc = do_predict(c, n_j);
         if (rc != NBK_OK) return rc;
@@ -217,6 +242,7 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     float* pot = acc + 6 * n_i;
     c->last_ni = n_i;
     c->in_flight = true;
+    c->host_has_result = false;
     if (n_i == 0) return NBK_OK;
     if (n_j == 0) {
         NBK_CUDA(c, cudaMemsetAsync(acc, 0, sizeof(float) * 7 * n_i, c->stream));
@@ -238,17 +264,29 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     fa.partial = c->d_partial;
     fa.eps2 = eps2;
     fa.d = d;
+    std::memset(&fa.tail, 0, sizeof(fa.tail));
+    const bool fused = v.I == 1 && d.nit == 1 && n_i <= kFusedMaxI && c->fused_ok;
+    if (h_inline && !fused) {  // planner chose another shape: stage the indices after all
+        NBK_CUDA(c, cudaEventSynchronize(c->istage_free));
+        std::memcpy(c->h_istage, h_inline, sizeof(int32_t) * n_i);
+        NBK_CUDA(c, cudaMemcpyAsync(c->d_iidx, c->h_istage, sizeof(int32_t) * n_i,
+                                    cudaMemcpyHostToDevice, c->stream));
+        NBK_CUDA(c, cudaEventRecord(c->istage_free, c->stream));
+        fa.i_index = c->d_iidx;
+    }
+    if (fused) {
+        fa.tail.enabled = 1;
+        fa.tail.counter = c->d_counter;
+        fa.tail.acc = acc; fa.tail.jerk = jerk; fa.tail.pot = pot;
+        fa.tail.host_out = to_host ? c->h_result_dev : nullptr;
+        if (h_inline) {
+            fa.tail.inline_index = 1;
+            std::memcpy(fa.tail.i_inline, h_inline, sizeof(int32_t) * n_i);
+        }
+    }
     {
         TimeScope ts(c, 2);
         NBK_CUDA(c, launch_force(v, fa, c->stream));
-    }
-    ReduceArgs ra;
-    ra.partial = c->d_partial;
-    ra.acc = acc; ra.jerk = jerk; ra.pot = pot;
-    ra.d = d;
-    {
-        TimeScope ts(c, 3);
-        NBK_CUDA(c, launch_reduce(v, ra, c->stream));
     }
     c->last_launch[0] = d.G;
     c->last_launch[1] = warps_of(v.I) * 32;
@@ -257,7 +295,25 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     c->last_launch[4] = d.tj;
     c->last_launch[5] = c->num_sms;
     c->last_launch[6] = static_cast<long long>(force_smem_bytes(v));
-    c->last_launch[7] = 2;
+    c->last_launch[7] = fused ? 1 : 2;
+    if (fused) {
+        c->host_has_result = to_host;
+        return NBK_OK;
+    }
+    ReduceArgs ra;
+    for (int k = 0; k < d.G; ++k) {
+        const long long q0 = (static_cast<long long>(k) * d.P) / d.G;
+        const long long q1 = ((static_cast<long long>(k) + 1) * d.P) / d.G;
+        ra.it_first[k] = static_cast<int>(q0 / d.njt);
+        ra.it_last[k] = static_cast<int>((q1 - 1) / d.njt);
+    }
+    ra.partial = c->d_partial;
+    ra.acc = acc; ra.jerk = jerk; ra.pot = pot;
+    ra.d = d;
+    {
+        TimeScope ts(c, 3);
+        NBK_CUDA(c, launch_reduce(v, ra, c->stream));
+    }
     return NBK_OK;
 }
 
@@ -272,6 +328,27 @@ int set_j_host(nbk_ctx* c, long long n, const int32_t* addr, const double* tj, c
     if (n == 0) return NBK_OK;
     DeviceGuard g(c->device);
     if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    {
+        const int rc = flush_pending(c);
+        if (rc != NBK_OK) return rc;
+    }
+    if (n <= kInlineMaxJ) {  // a handful of particles: the data rides in the next predictor launch
+        InlineJ& p = c->pending;
+        p.n = static_cast<int>(n);
+        for (int k = 0; k < p.n; ++k) {
+            p.addr[k] = addr ? addr[k] : k;
+            p.t[k] = tj ? tj[k] : 0.0;
+            p.m[k] = static_cast<float>(m[k]);
+            for (int q = 0; q < 3; ++q) {
+                p.x[k][q] = static_cast<double>(x[3 * k + q]);
+                p.v[k][q] = v ? static_cast<float>(v[3 * k + q]) : 0.f;
+                p.a[k][q] = a ? static_cast<float>(a[3 * k + q]) : 0.f;
+                p.k[k][q] = jerk ? static_cast<float>(jerk[3 * k + q]) : 0.f;
+            }
+        }
+        c->pred_valid = false;
+        return NBK_OK;
+    }
     NBK_CUDA(c, cudaEventSynchronize(c->stage_free));
     // pack [tj | m | x | v | a | jerk | addr] into the pinned buffer: one H2D copy
     size_t off = 0;
@@ -321,6 +398,7 @@ int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cud
     nbk_ctx* c = new (std::nothrow) nbk_ctx();
     if (!c) return NBK_ENOMEM;
     std::memset(c->ev, 0, sizeof(c->ev));
+    c->pending.n = 0;
     c->device = device;
     int rc = NBK_OK;
     auto fail = [&](int code, cudaError_t e) {
@@ -373,7 +451,10 @@ int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cud
         if ((e = cudaMalloc(&c->d_xi, sizeof(float) * 3 * ni)) != cudaSuccess) break;
         if ((e = cudaMalloc(&c->d_vi, sizeof(float) * 3 * ni)) != cudaSuccess) break;
         if ((e = cudaMalloc(&c->d_result, sizeof(float) * 7 * ni)) != cudaSuccess) break;
-        if ((e = cudaMallocHost(&c->h_result, sizeof(float) * 7 * ni)) != cudaSuccess) break;
+        if ((e = cudaHostAlloc(&c->h_result, sizeof(float) * 7 * ni, cudaHostAllocMapped)) != cudaSuccess) break;
+        if ((e = cudaHostGetDevicePointer(&c->h_result_dev, c->h_result, 0)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_counter, sizeof(unsigned))) != cudaSuccess) break;
+        if ((e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned), c->stream)) != cudaSuccess) break;
         c->partial_bytes = sizeof(float) * plan_partial_floats_bound(ni_max, c->num_sms);
         if ((e = cudaMalloc(&c->d_partial, c->partial_bytes)) != cudaSuccess) break;
         c->stage_bytes = static_cast<size_t>(n_max) * (8 + 8 + 4 * 24 + 4) + 16 * 8;
@@ -434,6 +515,10 @@ int nbk_set_j_particles_dev(nbk_ctx* c, int64_t n, const int32_t* addr, const do
     if (n == 0) return NBK_OK;
     DeviceGuard g(c->device);
     if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    {
+        const int rc = flush_pending(c);
+        if (rc != NBK_OK) return rc;
+    }
     ScatterArgs s;
     s.n = n; s.addr = addr; s.tj = tj; s.m = m; s.x = x; s.v = v; s.a = a; s.k = jerk;
     s.f64 = 0;
@@ -505,6 +590,8 @@ int nbk_calc_firsthalf(nbk_ctx* c, int64_t n_j, int64_t n_i, const int32_t* i_in
     const int32_t* d_ii = nullptr;
     const float* d_x = nullptr;
     const float* d_v = nullptr;
+    if (n_i > 0 && n_i <= kFusedMaxI && !xi && !vi)   // small block: indices ride in the launch
+        return enqueue_force(c, n_j, n_i, nullptr, nullptr, nullptr, eps2, flags, i_index, true);
     if (n_i > 0 && (i_index || xi || vi)) {
         NBK_CUDA(c, cudaEventSynchronize(c->istage_free));
         const size_t ni = static_cast<size_t>(n_i);
@@ -548,8 +635,9 @@ int nbk_calc_lasthalf(nbk_ctx* c, int64_t n_i, float* acc, float* jerk, float* p
     DeviceGuard g(c->device);
     if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
     const size_t ni = static_cast<size_t>(n_i);
-    NBK_CUDA(c, cudaMemcpyAsync(c->h_result, c->d_result, sizeof(float) * 7 * ni,
-                                cudaMemcpyDeviceToHost, c->stream));
+    if (!c->host_has_result)
+        NBK_CUDA(c, cudaMemcpyAsync(c->h_result, c->d_result, sizeof(float) * 7 * ni,
+                                    cudaMemcpyDeviceToHost, c->stream));
     NBK_CUDA(c, cudaStreamSynchronize(c->stream));
     if (acc) std::memcpy(acc, c->h_result, sizeof(float) * 3 * ni);
     if (jerk) std::memcpy(jerk, c->h_result + 3 * ni, sizeof(float) * 3 * ni);
@@ -624,6 +712,7 @@ int nbk_set_variant(nbk_ctx* c, int variant) {
     if (!(I == 0 || I == 1 || I == 2 || I == 4)) return NBK_EINVAL;
     c->variant_scalar = variant & 1;
     c->force_I = I;
+    c->fused_ok = (variant & 0x100) == 0;
     return NBK_OK;
 }
 

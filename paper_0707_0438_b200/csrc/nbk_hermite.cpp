@@ -17,6 +17,8 @@
 #include <chrono>
 #include <cmath>
 #include <cstdint>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -101,11 +103,15 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
     Levels L(n);
     int rc;
 
+    double prof[4] = {0, 0, 0, 0};  // set_ti+firsthalf, lasthalf, set_j, (unused)
+    int slot = 0;
 #define NBK_TIMED(call)                  \
     do {                                 \
         Clock c__;                       \
         rc = (call);                     \
-        gpu_s += c__.seconds();          \
+        const double s__ = c__.seconds(); \
+        gpu_s += s__;                    \
+        prof[slot] += s__;               \
         if (rc != NBK_OK) return rc;     \
     } while (0)
 
@@ -138,6 +144,7 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
         }
         const int64_t ni = static_cast<int64_t>(act.size());
 
+        slot = 0;
         NBK_TIMED(nbk_set_ti(ctx, t_new));
         NBK_TIMED(nbk_calc_firsthalf(ctx, n, ni, act.data(), nullptr, nullptr, eps2, flags));
         // host predictor (fp64) for the block's own particles, overlapped with the device
@@ -150,6 +157,7 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
                 vp[3 * q + c] = v[k] + a[k] * dt + jk[k] * dt2;
             }
         }
+        slot = 1;
         NBK_TIMED(nbk_calc_lasthalf(ctx, ni, fa.data(), fj.data(), nullptr));
 
         for (int64_t q = 0; q < ni; ++q) {
@@ -202,6 +210,7 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
                 bj[3 * q + c] = j1[c];
             }
         }
+        slot = 2;
         NBK_TIMED(nbk_set_j_particles_f64(ctx, ni, act.data(), bt.data(), bm.data(), bx.data(),
                                           bv.data(), ba.data(), bj.data()));
         T = T_new;
@@ -216,6 +225,9 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
     st.t_reached = std::ldexp(static_cast<double>(T), -kTickLog2);
     st.wall_seconds = wall.seconds();
     st.gpu_call_seconds = gpu_s;
+    if (std::getenv("NBK_TRACE"))
+        std::fprintf(stderr, "nbk_hermite_evolve: firsthalf %.3f s  lasthalf %.3f s  set_j %.3f s  wall %.3f s\n",
+                     prof[0], prof[1], prof[2], st.wall_seconds);
     if (stats) *stats = st;
     return NBK_OK;
 }

@@ -384,7 +384,8 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
                 float x = 0.f, y = 0.f, z = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
                 int idx = -1;
                 if (i < d.n_i) {
-                    idx = a.i_index ? a.i_index[i] : static_cast<int>(i);
+                    if (I == 1 && a.tail.inline_index) idx = a.tail.i_inline[i];
+                    else idx = a.i_index ? a.i_index[i] : static_cast<int>(i);
                     if (idx >= 0) {
                         x = a.j.x[idx]; y = a.j.y[idx]; z = a.j.z[idx];
                         if (JERK) { vx = a.j.vx[idx]; vy = a.j.vy[idx]; vz = a.j.vz[idx]; }
@@ -439,33 +440,114 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
 
         const bool last_of_tile = (jt == d.njt - 1) || (n == n_local - 1);
         if (last_of_tile) {
-            // one partial row per (CTA, i-tile touched, j-slice warp):  8 floats per i
-            const long long row =
-                (static_cast<long long>(blockIdx.x) * d.maxseg + (it - it_first)) * wjn + wj;
+            // one partial row per (CTA, i-tile touched): 8 floats per i.  When wjn warps split
+            // the j-tiles, the warp with slice 0 adds the wjn private sums of each i (fixed order).
+            if (wjn > 1) __syncthreads();   // uniform: every warp ends the segment at the same n
+            const long long row = static_cast<long long>(blockIdx.x) * d.maxseg + (it - it_first);
+            if (wj == 0) {
 #pragma unroll
-            for (int q = 0; q < I; ++q) {
-                const int il = wi * 32 * I + q * 32 + lane;
-                const double* sa = sacc + (q * NACC) * T + tid;
-                float4 o0, o1;
-                o0.x = static_cast<float>(sa[0 * T]);
-                o0.y = static_cast<float>(sa[1 * T]);
-                o0.z = static_cast<float>(sa[2 * T]);
-                o0.w = static_cast<float>(sa[3 * T]);
-                if (JERK) {
-                    o1.x = static_cast<float>(sa[4 * T] - 3.0 * sa[7 * T]);
-                    o1.y = static_cast<float>(sa[5 * T] - 3.0 * sa[8 * T]);
-                    o1.z = static_cast<float>(sa[6 * T] - 3.0 * sa[9 * T]);
-                } else {
-                    o1.x = o1.y = o1.z = 0.f;
+                for (int q = 0; q < I; ++q) {
+                    const int il = wi * 32 * I + q * 32 + lane;
+                    const double* sa = sacc + (q * NACC) * T + tid;
+                    double t[NACC];
+#pragma unroll
+                    for (int v = 0; v < NACC; ++v) t[v] = sa[v * T];
+                    for (int w = 1; w < wjn; ++w) {
+#pragma unroll
+                        for (int v = 0; v < NACC; ++v) t[v] += sa[v * T + 32 * w];
+                    }
+                    float4 o0, o1;
+                    o0.x = static_cast<float>(t[0]);
+                    o0.y = static_cast<float>(t[1]);
+                    o0.z = static_cast<float>(t[2]);
+                    o0.w = static_cast<float>(t[3]);
+                    if (JERK) {
+                        o1.x = static_cast<float>(t[4] - 3.0 * t[7 % NACC]);
+                        o1.y = static_cast<float>(t[5 % NACC] - 3.0 * t[8 % NACC]);
+                        o1.z = static_cast<float>(t[6 % NACC] - 3.0 * t[9 % NACC]);
+                    } else {
+                        o1.x = o1.y = o1.z = 0.f;
+                    }
+                    o1.w = 0.f;
+                    float4* dst = reinterpret_cast<float4*>(a.partial + (row * d.ti + il) * 8);
+                    dst[0] = o0;
+                    dst[1] = o1;
                 }
-                o1.w = 0.f;
-                float4* dst = reinterpret_cast<float4*>(a.partial + (row * d.ti + il) * 8);
-                dst[0] = o0;
-                dst[1] = o1;
             }
+            if (wjn > 1) __syncthreads();   // slots are zeroed again by the next segment's gather
             fresh = true;
         }
         if (++jt == d.njt) { jt = 0; ++it; }
+    }
+    // a6 in the same launch for small blocks (PAPER.md L118 sums the partial forces on the host;
+    // here the last CTA to arrive does it, rows in CTA order => same bits whoever is last)
+    if constexpr (I == 1) {
+        if (a.tail.enabled) {
+            __shared__ int is_last;
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) {
+                const unsigned ticket = atomicAdd(a.tail.counter, 1u);
+                is_last = (ticket == static_cast<unsigned>(d.G) - 1u);
+                if (is_last) *a.tail.counter = 0u;
+            }
+            __syncthreads();
+            if (is_last) {
+                __threadfence();
+                constexpr int NV = JERK ? 7 : 4;
+                constexpr int RY = T / 32;          // row lanes per i
+                const int tx = tid & 31, ty = tid >> 5;
+                double s[NV];
+#pragma unroll
+                for (int v = 0; v < NV; ++v) s[v] = 0.0;
+#pragma unroll 4
+                for (int k = ty; k < d.G; k += RY) {
+                    const float4* p = reinterpret_cast<const float4*>(
+                        a.partial + (static_cast<long long>(k) * d.maxseg * d.ti + tx) * 8);
+                    const float4 u = __ldcg(p);
+                    s[0] += u.x; s[1] += u.y; s[2] += u.z; s[3] += u.w;
+                    if (JERK) {
+                        const float4 w = __ldcg(p + 1);
+                        s[4 % NV] += w.x; s[5 % NV] += w.y; s[6 % NV] += w.z;
+                    }
+                }
+#pragma unroll
+                for (int v = 0; v < NV; ++v) sacc[v * T + tid] = s[v];
+                __syncthreads();
+                for (int st = RY >> 1; st > 0; st >>= 1) {
+                    if (ty < st) {
+#pragma unroll
+                        for (int v = 0; v < NV; ++v) sacc[v * T + tid] += sacc[v * T + tid + st * 32];
+                    }
+                    __syncthreads();
+                }
+                if (ty == 0 && tx < d.n_i) {
+                    const int n = d.n_i;
+                    float r[7];
+                    r[0] = static_cast<float>(sacc[0 * T + tid]);
+                    r[1] = static_cast<float>(sacc[1 * T + tid]);
+                    r[2] = static_cast<float>(sacc[2 * T + tid]);
+                    r[6] = static_cast<float>(-sacc[3 * T + tid]);
+                    r[3] = JERK ? static_cast<float>(sacc[(4 % NV) * T + tid]) : 0.f;
+                    r[4] = JERK ? static_cast<float>(sacc[(5 % NV) * T + tid]) : 0.f;
+                    r[5] = JERK ? static_cast<float>(sacc[(6 % NV) * T + tid]) : 0.f;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        a.tail.acc[3 * tx + c] = r[c];
+                        a.tail.jerk[3 * tx + c] = r[3 + c];
+                    }
+                    a.tail.pot[tx] = r[6];
+                    if (a.tail.host_out) {
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            a.tail.host_out[3 * tx + c] = r[c];
+                            a.tail.host_out[3 * n + 3 * tx + c] = r[3 + c];
+                        }
+                        a.tail.host_out[6 * n + tx] = r[6];
+                    }
+                }
+            }
+        }
     }
 #ifdef NBK_TRACE
     if (tid == 0 && blockIdx.x < 4096) {
@@ -484,33 +566,34 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
 // PAPER.md L118 ("stored in global memory, after which they are ... summed", done on the host
 // there).  256 threads = ix i-particles x (256 / ix) lanes over the partial rows; ix = 32 for
 // n_i >= 32, else the next power of two >= n_i so that small blocks still use every thread.
+// All i of a block lie in one i-tile (ix divides 32 divides ti); the CTAs that worked on that
+// tile are found from the first/last i-tile tables the host filled (no division on the device).
 template <bool JERK>
 __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_log2) {
     __shared__ double sh[7][256];
+    __shared__ int krange[2];
     const Decomp& d = a.d;
     const int ix = 1 << ix_log2, ry = 256 >> ix_log2;
     const int tid = threadIdx.x;
     const int tx = tid & (ix - 1), ty = tid >> ix_log2;
-    const long long i = static_cast<long long>(blockIdx.x) * ix + tx;
+    const long long i0 = static_cast<long long>(blockIdx.x) * ix;
+    const long long i = i0 + tx;
     const bool valid = i < d.n_i;
+    const int it = static_cast<int>(i0 / d.ti);
+    if (tid < d.G) {
+        const bool in = a.it_first[tid] <= it && it <= a.it_last[tid];
+        if (in && (tid == 0 || a.it_last[tid - 1] < it)) krange[0] = tid;
+        if (in && (tid == d.G - 1 || a.it_first[tid + 1] > it)) krange[1] = tid;
+    }
+    __syncthreads();
     double s[7] = {0, 0, 0, 0, 0, 0, 0};
     if (valid) {
-        const int it = static_cast<int>(i / d.ti);
         const int il = static_cast<int>(i - static_cast<long long>(it) * d.ti);
-        const long long lo = static_cast<long long>(it) * d.njt, hi = lo + d.njt - 1;
-        // CTAs k0..k1 own the pairs [lo, hi] of this i-tile
-        long long k0 = (lo * d.G) / d.P;
-        while (k0 + 1 < d.G && pair_start(k0 + 1, d.P, d.G) <= lo) ++k0;
-        while (k0 > 0 && pair_start(k0, d.P, d.G) > lo) --k0;
-        long long k1 = (hi * d.G) / d.P;
-        while (k1 + 1 < d.G && pair_start(k1 + 1, d.P, d.G) <= hi) ++k1;
-        while (k1 > 0 && pair_start(k1, d.P, d.G) > hi) --k1;
-        const int nrows = static_cast<int>(k1 - k0 + 1) * d.wj;
-        for (int r = ty; r < nrows; r += ry) {
-            const long long k = k0 + r / d.wj;
-            const int w = r % d.wj;
-            const int seg = it - static_cast<int>(pair_start(k, d.P, d.G) / d.njt);
-            const long long row = (k * d.maxseg + seg) * d.wj + w;
+        const int k0 = krange[0], k1 = krange[1];
+#pragma unroll 4
+        for (int k = k0 + ty; k <= k1; k += ry) {
+            const int seg = it - a.it_first[k];
+            const long long row = static_cast<long long>(k) * d.maxseg + seg;
             const float4* p = reinterpret_cast<const float4*>(a.partial + (row * d.ti + il) * 8);
             const float4 u = p[0];
             s[0] += u.x; s[1] += u.y; s[2] += u.z; s[3] += u.w;
@@ -590,6 +673,51 @@ __global__ void predict_kernel(const RawJ raw, double t, long long n_j, long lon
     pvx[j] = o[4]; pvy[j] = o[5]; pvz[j] = o[6];
 }
 
+// The same predictor with a pending set_j of a few particles folded in (a1 + a3 in one launch):
+// the thread that owns an updated address stores the new raw state and predicts from it.
+__global__ void predict_upd_kernel(const RawJ raw, double t, long long n_j, long long n_pad,
+                                   float* px, float* py, float* pz, float* pm, float* pvx,
+                                   float* pvy, float* pvz, const InlineJ upd) {
+    const long long j = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (j >= n_pad) return;
+    float o[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (j < n_j) {
+        int hit = -1;
+        for (int k = 0; k < upd.n; ++k)
+            if (upd.addr[k] == j) hit = k;   // the last entry for an address wins
+        double tj, x[3];
+        float v[3], ac[3], jk[3], m;
+        if (hit >= 0) {
+            tj = upd.t[hit]; m = upd.m[hit];
+            raw.t[j] = tj; raw.m[j] = m;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                x[c] = upd.x[hit][c]; v[c] = upd.v[hit][c]; ac[c] = upd.a[hit][c]; jk[c] = upd.k[hit][c];
+                raw.x[c * raw.cap + j] = x[c]; raw.v[c * raw.cap + j] = v[c];
+                raw.a[c * raw.cap + j] = ac[c]; raw.k[c * raw.cap + j] = jk[c];
+            }
+        } else {
+            tj = raw.t[j]; m = raw.m[j];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                x[c] = raw.x[c * raw.cap + j]; v[c] = raw.v[c * raw.cap + j];
+                ac[c] = raw.a[c * raw.cap + j]; jk[c] = raw.k[c * raw.cap + j];
+            }
+        }
+        const double dt = t - tj;
+        const double dt2 = dt * dt * 0.5, dt3 = dt * dt * dt * (1.0 / 6.0);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double vd = v[c], ad = ac[c], kd = jk[c];
+            o[c] = static_cast<float>(x[c] + vd * dt + ad * dt2 + kd * dt3);
+            o[4 + c] = static_cast<float>(vd + ad * dt + kd * dt2);
+        }
+        o[3] = m;
+    }
+    px[j] = o[0]; py[j] = o[1]; pz[j] = o[2]; pm[j] = o[3];
+    pvx[j] = o[4]; pvy[j] = o[5]; pvz[j] = o[6];
+}
+
 // --------------------------------------------------------------------------------- launchers
 template <int I, bool JERK, bool EPS0, bool PACKED>
 static cudaError_t prepare_of() {
@@ -664,6 +792,27 @@ cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s)
     return cudaGetLastError();
 }
 
+__global__ void scatter_inline_kernel(const InlineJ p, const RawJ raw) {
+    const int k = threadIdx.x;
+    if (k >= p.n) return;
+    const long long ad = p.addr[k];
+    raw.m[ad] = p.m[k];
+    raw.t[ad] = p.t[k];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        raw.x[c * raw.cap + ad] = p.x[k][c];
+        raw.v[c * raw.cap + ad] = p.v[k][c];
+        raw.a[c * raw.cap + ad] = p.a[k][c];
+        raw.k[c * raw.cap + ad] = p.k[k][c];
+    }
+}
+
+cudaError_t launch_scatter_inline(const InlineJ& p, const RawJ& raw, cudaStream_t st) {
+    if (p.n <= 0) return cudaSuccess;
+    scatter_inline_kernel<<<1, kInlineMaxJ, 0, st>>>(p, raw);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_scatter(const ScatterArgs& s, const RawJ& raw, cudaStream_t st) {
     if (s.n <= 0) return cudaSuccess;
     const unsigned grid = static_cast<unsigned>((s.n + 255) / 256);
@@ -674,10 +823,13 @@ cudaError_t launch_scatter(const ScatterArgs& s, const RawJ& raw, cudaStream_t s
 
 cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n_pad, float* px,
                            float* py, float* pz, float* pm, float* pvx, float* pvy, float* pvz,
-                           cudaStream_t st) {
+                           const InlineJ* upd, cudaStream_t st) {
     if (n_pad <= 0) return cudaSuccess;
     const unsigned grid = static_cast<unsigned>((n_pad + 255) / 256);
-    predict_kernel<<<grid, 256, 0, st>>>(raw, t, n_j, n_pad, px, py, pz, pm, pvx, pvy, pvz);
+    if (upd && upd->n > 0)
+        predict_upd_kernel<<<grid, 256, 0, st>>>(raw, t, n_j, n_pad, px, py, pz, pm, pvx, pvy, pvz, *upd);
+    else
+        predict_kernel<<<grid, 256, 0, st>>>(raw, t, n_j, n_pad, px, py, pz, pm, pvx, pvy, pvz);
     return cudaGetLastError();
 }
 

@@ -11,6 +11,7 @@ constexpr int kStages = 6;      // tile ring depth
 constexpr int kPrefetch = 4;    // tiles the producer runs ahead (kStages - kPrefetch = drift slack)
 constexpr int kMaxI = 4;        // max i-particles per thread
 constexpr int kMaxRowI = 1024;  // max (warps * 32 * I): i-rows one CTA writes per (segment)
+constexpr int kMaxCtas = 256;   // max CTAs of a force launch (one per SM; B200 has 148)
 
 // warps per CTA for each i-per-thread count: one CTA per SM, registers decide the warp count
 __host__ __device__ constexpr int warps_of(int I) { return I == 4 ? 8 : (I == 2 ? 12 : 16); }
@@ -56,17 +57,36 @@ void plan_shape(long long n_i, long long n_j, int num_sms, int force_I, size_t m
 size_t plan_partial_floats(const Decomp& d);
 size_t plan_partial_floats_bound(long long ni_max, int num_sms);
 
+constexpr int kFusedMaxI = 32;  // largest i-block served by the one-launch small-block path
+
+// Small-block tail (n_i <= kFusedMaxI, one i-tile, I = 1): the last CTA to finish sums the partial
+// rows itself (fixed order) and writes the results, so a block step is one launch; the i-indices
+// travel in the kernel parameters and the results can go straight to mapped host memory.
+struct FusedTail {
+    int enabled;                   // 0: partial rows only, reduce_kernel follows
+    int inline_index;              // 1: i-indices are i_inline[], not ForceArgs::i_index
+    int32_t i_inline[kFusedMaxI];
+    unsigned* counter;             // device, zero between launches (the last CTA resets it)
+    float* acc;                    // device result [n_i][3]
+    float* jerk;                   // device result [n_i][3]
+    float* pot;                    // device result [n_i]
+    float* host_out;               // mapped pinned copy acc|jerk|pot (7 n_i floats) or nullptr
+};
+
 struct ForceArgs {
     JPred j;
     const int32_t* i_index;  // [n_i] or nullptr (identity)
     const float* xi;         // [n_i][3] or nullptr
     const float* vi;         // [n_i][3] or nullptr
-    float* partial;          // [(k*maxseg+seg)*wj + w][ti][8]
+    float* partial;          // [k*maxseg+seg][ti][8]
     float eps2;
     Decomp d;
+    FusedTail tail;
 };
 
 struct ReduceArgs {
+    int it_first[kMaxCtas];  // first / last i-tile CTA k works on (host-filled from the pair split)
+    int it_last[kMaxCtas];
     const float* partial;
     float* acc;   // [n_i][3]
     float* jerk;  // [n_i][3]
@@ -104,9 +124,26 @@ struct ScatterArgs {
     long long n_max;    // addresses outside [0, n_max) are skipped
 };
 cudaError_t launch_scatter(const ScatterArgs& s, const RawJ& raw, cudaStream_t st);
-// a3: predict raw -> predicted arrays for j < n_j, m = 0 padding for n_j <= j < n_pad.
+
+// set_j of a few particles with the data in the kernel parameters (no staging copy): what a
+// block step of a handful of corrected particles needs.
+constexpr int kInlineMaxJ = 16;
+struct InlineJ {
+    int n;
+    int32_t addr[kInlineMaxJ];
+    double t[kInlineMaxJ];
+    double x[kInlineMaxJ][3];     // kept in fp64 (see RawJ)
+    float m[kInlineMaxJ];
+    float v[kInlineMaxJ][3];
+    float a[kInlineMaxJ][3];
+    float k[kInlineMaxJ][3];
+};
+cudaError_t launch_scatter_inline(const InlineJ& p, const RawJ& raw, cudaStream_t st);
+
+// a3: predict raw -> predicted arrays for j < n_j, m = 0 padding for n_j <= j < n_pad.  upd (may be
+// nullptr): a pending small set_j whose addresses are all < n_j, stored and used in the same launch.
 cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n_pad, float* px,
                            float* py, float* pz, float* pm, float* pvx, float* pvy, float* pvz,
-                           cudaStream_t st);
+                           const InlineJ* upd, cudaStream_t st);
 
 }  // namespace nbk

@@ -81,7 +81,7 @@ def test_c2_block_step_sweep(gpu, c_oracle, c2, n_i):
         got = nb.nbk_calc_lasthalf(ctx, n_i)
         shape = nb.nbk_last_launch(ctx)
         gm, gx, gv = nb.nbk_get_predicted(ctx, n)
-    assert shape["launches"] == 2 and shape["grid"] >= min(128, shape["sms"])
+    assert shape["launches"] == (1 if n_i <= 32 else 2) and shape["grid"] >= min(128, shape["sms"])
     ref_kernel = c_oracle.force(gm, gx, gv, EPS, i_index=idx)
     assert_parity(got, ref_kernel, what=f"C2 n_i={n_i} kernel-only")
     ref_e2e = c_oracle.force(c2["m"], c2["xp"], c2["vp"], EPS, i_index=idx)
@@ -320,3 +320,57 @@ def test_errors_do_not_depend_on_which_kernel_shape_ran(gpu, c_oracle):
     for r in res[1:]:
         assert np.percentile(vec_rel_err(r[0], res[0][0]), 99) < 5e-6
         assert scalar_rel_err(r[2], res[0][2]).max() < 2e-6
+
+
+@pytest.mark.parametrize("n_i", [1, 5, 32])
+def test_small_block_one_launch_path_matches_two_kernel_path(gpu, c_oracle, n_i):
+    """Blocks of <= 32 i-particles are reduced by the force kernel's last CTA (one launch, indices in
+    the launch parameters, results in mapped host memory).  Same sums as force + reduce kernels."""
+    m, x, v = inputs.plummer_f32(6000, seed=81)
+    idx = inputs.active_block(6000, n_i, seed=4)
+    ref = c_oracle.force(m, x, v, EPS, i_index=idx)
+    with Ctx(6000) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        out = {}
+        for variant in (0x000, 0x100):
+            nb.nbk_set_variant(ctx, variant)
+            runs = []
+            for _ in range(3):
+                nb.nbk_calc_firsthalf(ctx, 6000, n_i, idx, None, None, np.float32(EPS) ** 2, FULL)
+                runs.append(nb.nbk_calc_lasthalf(ctx, n_i))
+            assert nb.nbk_last_launch(ctx)["launches"] == (1 if variant == 0 else 2)
+            for r in runs[1:]:
+                assert all(np.array_equal(a, b) for a, b in zip(runs[0], r))
+            out[variant] = runs[0]
+            assert_parity(runs[0], ref, what=f"small block n_i={n_i} variant {variant:#x}")
+        # identity index (i_index = NULL) through the same path
+        nb.nbk_set_variant(ctx, 0)
+        nb.nbk_calc_firsthalf(ctx, 6000, n_i, None, None, None, np.float32(EPS) ** 2, FULL)
+        ident = nb.nbk_calc_lasthalf(ctx, n_i)
+    assert np.abs(out[0][0] - out[0x100][0]).max() <= 2e-6 * np.abs(ref[0]).max()
+    assert scalar_rel_err(out[0][2], out[0x100][2]).max() < 1e-6
+    assert_parity(ident, c_oracle.force(m, x, v, EPS, i_index=np.arange(n_i)), what="identity small block")
+
+
+def test_set_j_of_a_few_particles_rides_in_the_launch(gpu):
+    """n <= 16 particles go through the parameter-space scatter; the stored state must equal what the
+    staged path stores (read back through the predictor at dt = 0)."""
+    m, x, v = inputs.plummer(500, seed=91)
+    with Ctx(500) as ctx:
+        nb.nbk_set_j_particles_f64(ctx, None, None, m, x, v)
+        addr = np.array([499, 3, 250, 17, 0], np.int32)
+        x2 = x[addr] + 0.125
+        v2 = v[addr] * 0.5
+        nb.nbk_set_j_particles_f64(ctx, addr, np.full(5, 0.25), m[addr] * 2, x2, v2)
+        nb.nbk_set_ti(ctx, 0.25)
+        nb.nbk_predict(ctx, 500)
+        gm, gx, gv = nb.nbk_get_predicted(ctx, 500)
+    ex, ev, em = x.copy(), v.copy(), m.copy()
+    ex[addr], ev[addr], em[addr] = x2, v2, m[addr] * 2
+    # untouched particles have t_j = 0, v != 0: they moved by v * 0.25; touched ones (t_j = t) did not
+    rest = np.setdiff1d(np.arange(500), addr)
+    assert np.array_equal(gx[addr], ex[addr].astype(np.float32))
+    assert np.array_equal(gv[addr], ev[addr].astype(np.float32))
+    assert np.array_equal(gm, em.astype(np.float32))
+    assert np.array_equal(gx[rest], (x[rest] + v[rest].astype(np.float32).astype(np.float64) * 0.25).astype(np.float32))

@@ -35,7 +35,7 @@ def test_plan_invariants(n_i, n_j, sms, force_i):
     njt = p["j_tiles"]
     touched = max((b - 1) // njt - a // njt + 1 for a, b in zip(starts, starts[1:]))
     assert touched <= p["max_segments"]
-    assert p["partial_floats"] == G * p["max_segments"] * wj * ti * 8
+    assert p["partial_floats"] == G * p["max_segments"] * ti * 8
     assert p["partial_floats"] <= p["partial_floats_bound"]
 
 
