@@ -37,6 +37,8 @@ def _load():
                                       _D, _D, ctypes.c_uint, _D, _D, _D]
         _lib.oracle_predict.restype = ctypes.c_int
         _lib.oracle_predict.argtypes = [ctypes.c_int64, ctypes.c_double, _D, _D, _D, _D, _D, _D, _D]
+        _lib.oracle_nearest.restype = ctypes.c_int
+        _lib.oracle_nearest.argtypes = [ctypes.c_int64, _D, ctypes.c_int64, _I, _D, _I, _D]
         _lib.oracle_num_threads.restype = ctypes.c_int
     return _lib
 
@@ -69,6 +71,22 @@ def force(m, x, v, eps, i_index=None, want_jerk=True, xi=None, vi=None):
     if rc != 0:
         raise ValueError("oracle_force: bad arguments")
     return acc, jrk, pot
+
+
+def nearest_neighbour(x, i_index=None, xi=None):
+    lib = _load()
+    x, xi = _c64(x), _c64(xi)
+    n = x.shape[0]
+    if i_index is None:
+        i_index = np.arange(n)
+    idx = np.ascontiguousarray(i_index, dtype=np.int64)
+    nn = np.empty(idx.shape[0], dtype=np.int64)
+    r2 = np.empty(idx.shape[0])
+    rc = lib.oracle_nearest(n, _p(x), idx.shape[0], idx.ctypes.data_as(_I), _p(xi),
+                            nn.ctypes.data_as(_I), _p(r2))
+    if rc != 0:
+        raise ValueError("oracle_nearest: bad arguments")
+    return nn, r2
 
 
 def predict(t, tj, x, v, a, jerk):

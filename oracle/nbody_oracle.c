@@ -95,6 +95,38 @@ int oracle_force(int64_t n_j, const double *m, const double *x, const double *v,
     return 0;
 }
 
+/* Nearest neighbour of each i-particle, own entry excluded by index, ties to
+ * the lowest index (reading R20).  nn[k] = -1, r2[k] = INFINITY if there is no other particle. */
+int oracle_nearest(int64_t n_j, const double *x, int64_t n_i, const int64_t *i_index,
+                   const double *xi, int64_t *nn, double *r2out)
+{
+    if (n_j < 0 || n_i < 0 || !x || !nn || !r2out) return -1;
+    for (int64_t k = 0; k < n_i; ++k) {
+        int64_t idx = i_index ? i_index[k] : k;
+        if (idx >= n_j) return -1;
+        if (idx < 0 && !xi) return -1;
+    }
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t k = 0; k < n_i; ++k) {
+        const int64_t self = i_index ? i_index[k] : k;
+        double xk[3];
+        for (int d = 0; d < 3; ++d) xk[d] = xi ? xi[3 * k + d] : x[3 * self + d];
+        int64_t best = -1;
+        double bestr2 = INFINITY;
+        for (int64_t j = 0; j < n_j; ++j) {
+            if (j == self) continue;
+            const double rx = x[3 * j + 0] - xk[0];
+            const double ry = x[3 * j + 1] - xk[1];
+            const double rz = x[3 * j + 2] - xk[2];
+            const double r2 = rx * rx + ry * ry + rz * rz;
+            if (r2 < bestr2) { bestr2 = r2; best = j; }
+        }
+        nn[k] = best;
+        r2out[k] = bestr2;
+    }
+    return 0;
+}
+
 /* Hermite predictor (reading R8): Taylor series through the jerk. */
 int oracle_predict(int64_t n, double t, const double *tj, const double *x, const double *v,
                    const double *a, const double *jerk, double *xp, double *vp)

@@ -103,6 +103,30 @@ def force(m, x, v, eps, i_index=None, want_jerk=True, xi=None, vi=None):
     return acc, jrk, pot
 
 
+def nearest_neighbour(x, i_index=None, xi=None):
+    """Index of, and squared distance to, the nearest j-particle of each i-particle (PAPER.md L128:
+    "comparing the distance between each particle and all other particles ... maintain the particle
+    with the minimum distance"), own entry excluded by index, fp64.  Reading R20: ties go to the
+    lowest index; a particle with no other j gets index -1 and distance inf."""
+    x = _as64(x, (3,))
+    n = x.shape[0]
+    if i_index is None:
+        i_index = np.arange(n)
+    idx = np.asarray(i_index, dtype=np.int64)
+    xs = x[np.maximum(idx, 0)] if xi is None else _as64(xi, (3,))
+    nn = np.full(idx.shape[0], -1, dtype=np.int64)
+    r2min = np.full(idx.shape[0], np.inf)
+    for k in range(idx.shape[0]):          # plain loop over i: one pass over j each
+        d = x - xs[k]
+        r2 = np.einsum("ij,ij->i", d, d)
+        if idx[k] >= 0:
+            r2[idx[k]] = np.inf
+        if n > 0 and np.isfinite(r2).any():
+            j = int(np.argmin(r2))         # argmin returns the first (lowest-index) minimum
+            nn[k], r2min[k] = j, r2[j]
+    return nn, r2min
+
+
 def predict(t, tj, x, v, a, jerk):
     """Hermite predictor, R8: Taylor series through the jerk, fp64."""
     dt = (float(t) - _as64(tj))[:, None]

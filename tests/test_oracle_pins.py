@@ -274,3 +274,51 @@ def test_flop_convention_reproduces_paper_tables(fname, k):
         # times are printed to 2-7 significant digits (worst case 0.000090 s: half a unit in the last
         # place is 0.6 %; the printed speed deviates by up to 0.8 % from the printed time)
         assert abs(got / gf - 1.0) < 0.01, (n, got, gf)
+
+
+# --- nearest neighbour (reading R20) -----------------------------------------
+def test_nearest_neighbour_on_a_line_and_lattice(oracle):
+    """Closed cases: points on a line at 0, 1, 3, 7, 15 (gaps double) => nn = 1, 0, 1, 2, 3;
+    a simple cubic lattice => every nearest distance is the spacing, and ties go to the lowest index."""
+    x = np.zeros((5, 3))
+    x[:, 0] = [0.0, 1.0, 3.0, 7.0, 15.0]
+    nn, r2 = oracle.nearest_neighbour(x)
+    assert list(nn) == [1, 0, 1, 2, 3]
+    assert np.allclose(r2, [1.0, 1.0, 4.0, 16.0, 64.0], rtol=0, atol=0)
+    g = np.arange(4.0)
+    lat = np.array([[a, b, c] for a in g for b in g for c in g]) * 0.5      # index = 16a + 4b + c
+    nn, r2 = oracle.nearest_neighbour(lat)
+    assert np.all(r2 == 0.25)
+    for i, (a, b, c) in enumerate([(a, b, c) for a in range(4) for b in range(4) for c in range(4)]):
+        cand = [16 * aa + 4 * bb + cc for aa, bb, cc in
+                [(a - 1, b, c), (a, b - 1, c), (a, b, c - 1), (a, b, c + 1), (a, b + 1, c), (a + 1, b, c)]
+                if 0 <= aa < 4 and 0 <= bb < 4 and 0 <= cc < 4]
+        assert nn[i] == min(cand)
+
+
+def test_nearest_neighbour_brute_force_subset_external_and_degenerate(oracle):
+    rng = np.random.default_rng(12)
+    x = rng.standard_normal((57, 3))
+    idx = np.array([5, 56, 0, 33])
+    nn, r2 = oracle.nearest_neighbour(x, i_index=idx)
+    for k, i in enumerate(idx):
+        best, bj = None, -1
+        for j in range(57):
+            if j == i:
+                continue
+            d = sum((x[j, c] - x[i, c]) ** 2 for c in range(3))
+            if best is None or d < best:
+                best, bj = d, j
+        assert nn[k] == bj and abs(r2[k] - best) <= 1e-15 * best
+    # external particle: nothing excluded; a j at the same place is the neighbour at distance 0
+    nn, r2 = oracle.nearest_neighbour(x, i_index=np.array([-1]), xi=x[7:8])
+    assert nn[0] == 7 and r2[0] == 0.0
+    # mutual pairs: the closest pair of the set are each other's neighbours
+    nn, r2 = oracle.nearest_neighbour(x)
+    i = int(np.argmin(r2))
+    assert nn[nn[i]] == i
+    # translation invariance of the index, and a lone particle has none
+    nn2, _ = oracle.nearest_neighbour(x + 3.0)
+    assert np.array_equal(nn, nn2)
+    nn1, r1 = oracle.nearest_neighbour(x[:1])
+    assert nn1[0] == -1 and np.isinf(r1[0])
