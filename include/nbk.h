@@ -58,6 +58,7 @@ typedef enum nbk_status {
 #define NBK_JERK 1u /* also compute the jerk (needs v of the j-particles)                */
 #define NBK_POT 2u  /* kept for GRAPE-style callers: the potential is always computed    */
 #define NBK_EPS0 4u /* mask pairs with s == 0; forced on if eps2==0 */
+#define NBK_NN 8u   /* also find each i-particle's nearest neighbour (L126-L128); needs NBK_JERK */
 
 /* ---- life cycle (GPU_open / GPU_close / GPU_npipes) ----------------- */
 
@@ -137,6 +138,20 @@ int nbk_calc_lasthalf(nbk_ctx* ctx, int64_t n_i, float* acc, float* jerk, float*
 /* Same to DEVICE arrays, asynchronous on the stream, no synchronisation. */
 int nbk_calc_lasthalf_dev(nbk_ctx* ctx, int64_t n_i, float* acc, float* jerk, float* pot);
 
+/* ---- nearest neighbour ("the GRAPE hardware also calculates the nearest
+ * neighbour of every particle that is being updated ... done as part of the force calculation";
+ * SURVEY.md 8(f)-2) ------------------------------------------------------------------------------ */
+
+/* After a firsthalf with NBK_NN: nn_index[n_i] = the j in [0, n_j) with the smallest softened
+ * squared distance s = r.r + eps2 to i-particle k as the kernel computes it in fp32, the own entry
+ * left out by index, ties to the lowest j (-1 if there is no other j); nn_r2[n_i] = its unsoftened
+ * squared distance in fp32 (inf if none).  The search rides in the force kernel (one min per pair);
+ * the index is recovered by re-scanning the one j-tile that held the minimum.  Host arrays (either
+ * may be NULL); waits for the stream.  NBK_ESTATE if the last firsthalf had no NBK_NN. */
+int nbk_get_neighbours(nbk_ctx* ctx, int64_t n_i, int32_t* nn_index, float* nn_r2);
+/* Same to DEVICE arrays, asynchronous on the stream. */
+int nbk_get_neighbours_dev(nbk_ctx* ctx, int64_t n_i, int32_t* nn_index, float* nn_r2);
+
 /* ---- a8: host Hermite driver (reading R15) ------------------- */
 
 typedef struct nbk_hermite_stats {
@@ -175,7 +190,7 @@ int nbk_get_timing(nbk_ctx* ctx, float ms[4]);
  * per CTA, out[2] i-particles per thread, out[3] warps splitting each j-tile, out[4] j-tile
  * size, out[5] SM count, out[6] dynamic shared memory bytes, out[7] number of kernels launched
  * by the last firsthalf (2: force + reduce; 1: small block, reduced by the force kernel's last
- * CTA). */
+ * CTA; 3: force + reduce + neighbour re-scan). */
 int nbk_last_launch(const nbk_ctx* ctx, int64_t out[8]);
 
 /* Host-only (no GPU needed): the launch plan firsthalf would use for (n_i, n_j) on a device with

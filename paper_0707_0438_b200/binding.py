@@ -15,12 +15,13 @@ import numpy as np
 from . import build as _build
 
 NBK_OK, NBK_EINVAL, NBK_ERANGE, NBK_ENOMEM, NBK_ECUDA, NBK_ESTATE = 0, -1, -2, -3, -4, -5
-NBK_JERK, NBK_POT, NBK_EPS0 = 1, 2, 4
+NBK_JERK, NBK_POT, NBK_EPS0, NBK_NN = 1, 2, 4, 8
 
 EXPORTS = [
     "nbk_open", "nbk_close", "nbk_npipes", "nbk_set_j_particles", "nbk_set_j_particles_f64",
     "nbk_set_j_particles_dev", "nbk_set_ti", "nbk_predict", "nbk_get_predicted",
     "nbk_calc_firsthalf", "nbk_calc_firsthalf_dev", "nbk_calc_lasthalf", "nbk_calc_lasthalf_dev",
+    "nbk_get_neighbours", "nbk_get_neighbours_dev",
     "nbk_hermite_evolve", "nbk_sync", "nbk_set_timing", "nbk_get_timing", "nbk_last_launch",
     "nbk_plan", "nbk_set_variant", "nbk_last_cuda_error", "nbk_strerror", "nbk_version",
 ]
@@ -49,6 +50,8 @@ _SIGS = {
     "nbk_calc_firsthalf_dev": (_i32, [_vp, _i64, _i64, _vp, _vp, _vp, _f32, _u32]),
     "nbk_calc_lasthalf": (_i32, [_vp, _i64, _vp, _vp, _vp]),
     "nbk_calc_lasthalf_dev": (_i32, [_vp, _i64, _vp, _vp, _vp]),
+    "nbk_get_neighbours": (_i32, [_vp, _i64, _vp, _vp]),
+    "nbk_get_neighbours_dev": (_i32, [_vp, _i64, _vp, _vp]),
     "nbk_hermite_evolve": (_i32, [_vp, _i64, _vp, _vp, _vp, _f64, _f64, _f64, _f64,
                                   ctypes.POINTER(HermiteStats)]),
     "nbk_sync": (_i32, [_vp]),
@@ -199,6 +202,18 @@ def nbk_calc_lasthalf(ctx, n_i):
 def nbk_calc_lasthalf_dev(ctx, n_i, acc=0, jerk=0, pot=0):
     _check("nbk_calc_lasthalf_dev",
            load().nbk_calc_lasthalf_dev(ctx, n_i, acc or None, jerk or None, pot or None), ctx)
+
+
+def nbk_get_neighbours(ctx, n_i):
+    nn = np.empty(n_i, np.int32)
+    r2 = np.empty(n_i, np.float32)
+    _check("nbk_get_neighbours", load().nbk_get_neighbours(ctx, n_i, nn.ctypes.data, r2.ctypes.data), ctx)
+    return nn, r2
+
+
+def nbk_get_neighbours_dev(ctx, n_i, nn_index=0, nn_r2=0):
+    _check("nbk_get_neighbours_dev",
+           load().nbk_get_neighbours_dev(ctx, n_i, nn_index or None, nn_r2 or None), ctx)
 
 
 def nbk_hermite_evolve(ctx, m, x, v, eps, t_end, eta=0.01, dt_max=1.0 / 16.0):

@@ -56,6 +56,12 @@ struct nbk_ctx {
     float* h_result = nullptr;  // pinned, mapped into the device address space
     float* h_result_dev = nullptr;  // device view of h_result
     unsigned* d_counter = nullptr;  // arrival counter of the fused small-block tail
+    float2* d_nn_partial = nullptr; // nearest neighbour: per partial row (smallest s, its j-tile)
+    float* d_nn_best = nullptr;     // [ni_max]
+    int32_t* d_nn_tile = nullptr;   // [ni_max]
+    int32_t* d_nn_index = nullptr;  // [ni_max] result
+    float* d_nn_r2 = nullptr;       // [ni_max] result
+    bool last_nn = false;           // the last firsthalf asked for nearest neighbours
     bool host_has_result = false;   // the last firsthalf wrote h_result itself (no D2H needed)
     InlineJ pending;                // a small set_j not yet on the device (pending.n == 0: none)
 
@@ -118,6 +124,8 @@ void free_all(nbk_ctx* c) {
     cudaFree(c->raw.m); cudaFree(c->raw.t); cudaFree(c->pred);
     cudaFree(c->d_iidx); cudaFree(c->d_xi); cudaFree(c->d_vi);
     cudaFree(c->d_partial); cudaFree(c->d_result); cudaFree(c->d_stage); cudaFree(c->d_counter);
+    cudaFree(c->d_nn_partial); cudaFree(c->d_nn_best); cudaFree(c->d_nn_tile);
+    cudaFree(c->d_nn_index); cudaFree(c->d_nn_r2);
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_stage) cudaFreeHost(c->h_stage);
     if (c->h_istage) cudaFreeHost(c->h_istage);
@@ -253,7 +261,9 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     Decomp d;
     v.jerk = (flags & NBK_JERK) != 0;
     v.eps0 = (flags & NBK_EPS0) != 0 || eps2 == 0.f;
-    v.packed = c->variant_scalar == 0;
+    v.nn = (flags & NBK_NN) != 0;
+    v.packed = c->variant_scalar == 0 || v.nn;   // the neighbour search exists in the packed form
+    c->last_nn = v.nn;
     d.G = 0;
     plan_shape(n_i, n_j, c->num_sms, c->force_I, c->partial_bytes / sizeof(float), &v, &d);
     if (d.G < 1 || plan_partial_floats(d) * sizeof(float) > c->partial_bytes) return NBK_ENOMEM;
@@ -262,7 +272,11 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     fa.j = jpred_of(c);
     fa.i_index = d_iidx; fa.xi = d_xi; fa.vi = d_vi;
     fa.partial = c->d_partial;
+    fa.nn_partial = c->d_nn_partial;
+    fa.nn_index = c->d_nn_index;
+    fa.nn_r2 = c->d_nn_r2;
     fa.eps2 = eps2;
+    d.n_j = static_cast<int>(n_j);
     fa.d = d;
     std::memset(&fa.tail, 0, sizeof(fa.tail));
     const bool fused = v.I == 1 && d.nit == 1 && n_i <= kFusedMaxI && c->fused_ok;
@@ -308,11 +322,25 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
         ra.it_last[k] = static_cast<int>((q1 - 1) / d.njt);
     }
     ra.partial = c->d_partial;
+    ra.nn_partial = c->d_nn_partial;
+    ra.nn_best = c->d_nn_best;
+    ra.nn_tile = c->d_nn_tile;
     ra.acc = acc; ra.jerk = jerk; ra.pot = pot;
     ra.d = d;
     {
         TimeScope ts(c, 3);
         NBK_CUDA(c, launch_reduce(v, ra, c->stream));
+        if (v.nn) {
+            NnScanArgs na;
+            na.j = fa.j;
+            na.i_index = fa.i_index; na.xi = d_xi;
+            na.nn_best = c->d_nn_best; na.nn_tile = c->d_nn_tile;
+            na.nn_index = c->d_nn_index; na.nn_r2 = c->d_nn_r2;
+            na.n_i = static_cast<int>(n_i); na.n_j = static_cast<int>(n_j); na.tj = d.tj;
+            na.eps2 = eps2;
+            NBK_CUDA(c, launch_nn_scan(na, c->stream));
+            c->last_launch[7] = 3;
+        }
     }
     return NBK_OK;
 }
@@ -451,12 +479,17 @@ int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cud
         if ((e = cudaMalloc(&c->d_xi, sizeof(float) * 3 * ni)) != cudaSuccess) break;
         if ((e = cudaMalloc(&c->d_vi, sizeof(float) * 3 * ni)) != cudaSuccess) break;
         if ((e = cudaMalloc(&c->d_result, sizeof(float) * 7 * ni)) != cudaSuccess) break;
-        if ((e = cudaHostAlloc(&c->h_result, sizeof(float) * 7 * ni, cudaHostAllocMapped)) != cudaSuccess) break;
+        if ((e = cudaHostAlloc(&c->h_result, sizeof(float) * 9 * ni, cudaHostAllocMapped)) != cudaSuccess) break;
         if ((e = cudaHostGetDevicePointer(&c->h_result_dev, c->h_result, 0)) != cudaSuccess) break;
         if ((e = cudaMalloc(&c->d_counter, sizeof(unsigned))) != cudaSuccess) break;
         if ((e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned), c->stream)) != cudaSuccess) break;
         c->partial_bytes = sizeof(float) * plan_partial_floats_bound(ni_max, c->num_sms);
         if ((e = cudaMalloc(&c->d_partial, c->partial_bytes)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_nn_partial, c->partial_bytes / 4)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_nn_best, sizeof(float) * ni)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_nn_tile, sizeof(int32_t) * ni)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_nn_index, sizeof(int32_t) * ni)) != cudaSuccess) break;
+        if ((e = cudaMalloc(&c->d_nn_r2, sizeof(float) * ni)) != cudaSuccess) break;
         c->stage_bytes = static_cast<size_t>(n_max) * (8 + 8 + 4 * 24 + 4) + 16 * 8;
         if ((e = cudaMallocHost(&c->h_stage, c->stage_bytes)) != cudaSuccess) break;
         if ((e = cudaMalloc(&c->d_stage, c->stage_bytes)) != cudaSuccess) break;
@@ -576,6 +609,7 @@ int nbk_get_predicted(nbk_ctx* c, int64_t n_j, float* m, float* x, float* v) {
 int nbk_calc_firsthalf(nbk_ctx* c, int64_t n_j, int64_t n_i, const int32_t* i_index,
                        const float* xi, const float* vi, float eps2, uint32_t flags) {
     if (!c || n_j < 0 || n_i < 0 || !(eps2 >= 0.f)) return NBK_EINVAL;
+    if ((flags & NBK_NN) && !(flags & NBK_JERK)) return NBK_EINVAL;
     if (n_j > c->n_max || n_i > c->ni_max) return NBK_ERANGE;
     if (i_index) {
         for (int64_t k = 0; k < n_i; ++k) {
@@ -621,6 +655,7 @@ int nbk_calc_firsthalf(nbk_ctx* c, int64_t n_j, int64_t n_i, const int32_t* i_in
 int nbk_calc_firsthalf_dev(nbk_ctx* c, int64_t n_j, int64_t n_i, const int32_t* i_index,
                            const float* xi, const float* vi, float eps2, uint32_t flags) {
     if (!c || n_j < 0 || n_i < 0 || !(eps2 >= 0.f)) return NBK_EINVAL;
+    if ((flags & NBK_NN) && !(flags & NBK_JERK)) return NBK_EINVAL;
     if (n_j > c->n_max || n_i > c->ni_max) return NBK_ERANGE;
     if (!i_index && n_i > n_j) return NBK_ERANGE;
     DeviceGuard g(c->device);
@@ -655,6 +690,36 @@ int nbk_calc_lasthalf_dev(nbk_ctx* c, int64_t n_i, float* acc, float* jerk, floa
     if (acc) NBK_CUDA(c, cudaMemcpyAsync(acc, c->d_result, sizeof(float) * 3 * ni, cudaMemcpyDeviceToDevice, c->stream));
     if (jerk) NBK_CUDA(c, cudaMemcpyAsync(jerk, c->d_result + 3 * ni, sizeof(float) * 3 * ni, cudaMemcpyDeviceToDevice, c->stream));
     if (pot) NBK_CUDA(c, cudaMemcpyAsync(pot, c->d_result + 6 * ni, sizeof(float) * ni, cudaMemcpyDeviceToDevice, c->stream));
+    return NBK_OK;
+}
+
+int nbk_get_neighbours(nbk_ctx* c, int64_t n_i, int32_t* nn_index, float* nn_r2) {
+    if (!c || n_i < 0) return NBK_EINVAL;
+    if (!c->in_flight || n_i != c->last_ni || !c->last_nn) return NBK_ESTATE;
+    if (n_i == 0) return NBK_OK;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    const size_t ni = static_cast<size_t>(n_i);
+    float* h = c->h_result + 7 * ni;   // [nn_index as int bits | nn_r2]
+    if (!c->host_has_result) {
+        NBK_CUDA(c, cudaMemcpyAsync(h, c->d_nn_index, sizeof(int32_t) * ni, cudaMemcpyDeviceToHost, c->stream));
+        NBK_CUDA(c, cudaMemcpyAsync(h + ni, c->d_nn_r2, sizeof(float) * ni, cudaMemcpyDeviceToHost, c->stream));
+    }
+    NBK_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (nn_index) std::memcpy(nn_index, h, sizeof(int32_t) * ni);
+    if (nn_r2) std::memcpy(nn_r2, h + ni, sizeof(float) * ni);
+    return NBK_OK;
+}
+
+int nbk_get_neighbours_dev(nbk_ctx* c, int64_t n_i, int32_t* nn_index, float* nn_r2) {
+    if (!c || n_i < 0) return NBK_EINVAL;
+    if (!c->in_flight || n_i != c->last_ni || !c->last_nn) return NBK_ESTATE;
+    if (n_i == 0) return NBK_OK;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    const size_t ni = static_cast<size_t>(n_i);
+    if (nn_index) NBK_CUDA(c, cudaMemcpyAsync(nn_index, c->d_nn_index, sizeof(int32_t) * ni, cudaMemcpyDeviceToDevice, c->stream));
+    if (nn_r2) NBK_CUDA(c, cudaMemcpyAsync(nn_r2, c->d_nn_r2, sizeof(float) * ni, cudaMemcpyDeviceToDevice, c->stream));
     return NBK_OK;
 }
 

@@ -134,7 +134,8 @@ struct Shape {
 template <int I, bool JERK>
 constexpr size_t smem_bytes_of() {
     return 128 + sizeof(float) * kStages * Shape<JERK>::stage_floats +
-           sizeof(double) * Shape<JERK>::nacc * I * warps_of(I) * 32;
+           sizeof(double) * Shape<JERK>::nacc * I * warps_of(I) * 32 +
+           8 * I * warps_of(I) * 32;   // nearest-neighbour (distance, tile) per thread and i
 }
 
 // One elected thread: bring j-tile `jt` (tj particles) into a ring slot.
@@ -166,10 +167,14 @@ __device__ __forceinline__ void issue_tile(const JPred& j, int jt, int tj, float
 // The i-state is held negated (r = x_j + (-x_i) is one add).  sl[q] is the position of the
 // i-particle's own j entry inside this tile (anything outside [0, tj) if it is elsewhere);
 // MASK instantiations zero the mass of that entry.
-template <int I, bool JERK, bool EPS0, bool MASK>
+// NN instantiations also keep, per i, the smallest s seen in this tile ("a
+// comparison is added with each force calculation to maintain the particle with the minimum
+// distance"); which j it was is found afterwards by re-scanning the one winning tile (nn_scan).
+template <int I, bool JERK, bool EPS0, bool MASK, bool NN>
 __device__ __forceinline__ void tile_packed(const float* __restrict__ sx, int jbeg, int jend,
                                             const float (&ni)[I][6], const int (&sl)[I],
-                                            u64 (&acc)[I][Shape<JERK>::nacc], float eps2) {
+                                            u64 (&acc)[I][Shape<JERK>::nacc], float eps2,
+                                            float (&tmin)[I]) {
     const u64 e2p = pack(eps2, eps2);
     constexpr int kUnroll = NBK_UNROLL;
 #pragma unroll kUnroll
@@ -206,6 +211,14 @@ __device__ __forceinline__ void tile_packed(const float* __restrict__ sx, int jb
                 r2 = fma2(dz, dz, r2);
                 float r2a, r2b;
                 unpack(r2, r2a, r2b);
+                if (NN) {
+                    float qa = r2a, qb = r2b;
+                    if (MASK) {  // the own entry is nobody's neighbour
+                        qa = (jj + 2 * h == sl[q]) ? __int_as_float(0x7f800000) : qa;
+                        qb = (jj + 2 * h + 1 == sl[q]) ? __int_as_float(0x7f800000) : qb;
+                    }
+                    tmin[q] = fminf(tmin[q], fminf(qa, qb));
+                }
                 float ra = rsq(r2a), rb = rsq(r2b);
                 u64 rinv, rinv2;
                 if (EPS0) {  // zero-distance pairs contribute nothing
@@ -288,6 +301,51 @@ __device__ __forceinline__ void tile_scalar(const float* __restrict__ sx, int jb
     }
 }
 
+// Nearest neighbour, second step: one warp re-scans the one j-tile whose minimum won, with the
+// arithmetic of the tile loop (same s for the same pair), and returns the lowest j that attains the
+// tile's minimum, the own entry left out by index (reading R20: ties go to the lowest index).
+// r2out is the unsoftened squared distance of that pair in fp32.
+__device__ __forceinline__ float sfma(float a, float b, float c) {
+    float d;
+    asm("fma.rn.ftz.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
+}
+__device__ __forceinline__ float sadd(float a, float b) {
+    float d;
+    asm("add.rn.ftz.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+    return d;
+}
+__device__ __forceinline__ void nn_scan(const JPred& j, int n_j, int tile, int tj, float nx,
+                                        float ny, float nz, int self, float eps2, int lane,
+                                        int* nn_out, float* r2_out) {
+    float best = __int_as_float(0x7f800000);
+    int bj = 0x7fffffff;
+    if (tile >= 0) {
+        const int j0 = tile * tj;
+        for (int jj = j0 + lane; jj < j0 + tj && jj < n_j; jj += 32) {
+            const float dx = sadd(j.x[jj], nx), dy = sadd(j.y[jj], ny), dz = sadd(j.z[jj], nz);
+            const float s = sfma(dz, dz, sfma(dy, dy, sfma(dx, dx, eps2)));
+            if (jj != self && s < best) { best = s; bj = jj; }   // ascending jj: first minimum kept
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float ob = __shfl_xor_sync(0xffffffffu, best, o);
+        const int oj = __shfl_xor_sync(0xffffffffu, bj, o);
+        if (ob < best || (ob == best && oj < bj)) { best = ob; bj = oj; }
+    }
+    if (lane == 0) {
+        if (bj == 0x7fffffff) {
+            *nn_out = -1;
+            *r2_out = __int_as_float(0x7f800000);
+        } else {
+            const float dx = sadd(j.x[bj], nx), dy = sadd(j.y[bj], ny), dz = sadd(j.z[bj], nz);
+            *nn_out = bj;
+            *r2_out = sfma(dz, dz, sfma(dy, dy, dx * dx));
+        }
+    }
+}
+
 template <bool PACKED> struct AccT { typedef float type; };
 template <> struct AccT<true> { typedef u64 type; };
 
@@ -304,7 +362,7 @@ __device__ __forceinline__ float acc_take(float& a) {
 }
 
 // ------------------------------------------------------------------------------ force kernel
-template <int I, bool JERK, bool EPS0, bool PACKED>
+template <int I, bool JERK, bool EPS0, bool PACKED, bool NN>
 __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceArgs a) {
     using S = Shape<JERK>;
     constexpr int NACC = S::nacc;
@@ -317,6 +375,8 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
     float* stages = reinterpret_cast<float*>(smem_raw + 128);
     double* sacc = reinterpret_cast<double*>(smem_raw + 128 +
                                              sizeof(float) * kStages * S::stage_floats);
+    float* snn_best = reinterpret_cast<float*>(sacc + NACC * I * T);   // [I][T]
+    int* snn_tile = reinterpret_cast<int*>(snn_best + I * T);          // [I][T]
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
@@ -358,6 +418,8 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
     float ni[I][6];     // negated i-state: -x -y -z -vx -vy -vz
     int self[I];        // the i-particle's own j index, or -1
     acc_t acc[I][NACC];
+    float nn_best[I], tmin[I];   // NN: smallest s so far / in the current tile, and its j-tile
+    int nn_tile[I];
 
     int it = it_first;
     int jt = jt_first;
@@ -396,6 +458,8 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
                 ni[q][0] = -x; ni[q][1] = -y; ni[q][2] = -z;
                 ni[q][3] = -vx; ni[q][4] = -vy; ni[q][5] = -vz;
                 self[q] = idx;
+                nn_best[q] = tmin[q] = __int_as_float(0x7f800000);
+                nn_tile[q] = -1;
 #pragma unroll
                 for (int v = 0; v < NACC; ++v) {
                     sacc[(q * NACC + v) * T + tid] = 0.0;
@@ -419,13 +483,20 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
             mine |= static_cast<unsigned>(sl[q]) < static_cast<unsigned>(d.tj);
         }
         if (__any_sync(0xffffffffu, mine)) {
-            if constexpr (PACKED) tile_packed<I, JERK, EPS0, true>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2);
+            if constexpr (PACKED) tile_packed<I, JERK, EPS0, true, NN>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2, tmin);
             else tile_scalar<I, JERK, EPS0, true>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2);
         } else {
-            if constexpr (PACKED) tile_packed<I, JERK, EPS0, false>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2);
+            if constexpr (PACKED) tile_packed<I, JERK, EPS0, false, NN>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2, tmin);
             else tile_scalar<I, JERK, EPS0, false>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2);
         }
 
+        if (NN) {
+#pragma unroll
+            for (int q = 0; q < I; ++q) {
+                if (tmin[q] < nn_best[q]) { nn_best[q] = tmin[q]; nn_tile[q] = jt; }
+                tmin[q] = __int_as_float(0x7f800000);
+            }
+        }
         // this warp is done with the ring slot
         __syncwarp();
         if (lane == 0) mbar_arrive(empty0 + 8 * slot);
@@ -442,12 +513,29 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
         if (last_of_tile) {
             // one partial row per (CTA, i-tile touched): 8 floats per i.  When wjn warps split
             // the j-tiles, the warp with slice 0 adds the wjn private sums of each i (fixed order).
+            if (NN) {
+#pragma unroll
+                for (int q = 0; q < I; ++q) {
+                    snn_best[q * T + tid] = nn_best[q];
+                    snn_tile[q * T + tid] = nn_tile[q];
+                }
+            }
             if (wjn > 1) __syncthreads();   // uniform: every warp ends the segment at the same n
             const long long row = static_cast<long long>(blockIdx.x) * d.maxseg + (it - it_first);
             if (wj == 0) {
 #pragma unroll
                 for (int q = 0; q < I; ++q) {
                     const int il = wi * 32 * I + q * 32 + lane;
+                    if (NN) {   // slices hold disjoint tiles' parts: smallest s, then lowest tile
+                        float b = snn_best[q * T + tid];
+                        int bt = snn_tile[q * T + tid];
+                        for (int w = 1; w < wjn; ++w) {
+                            const float ob = snn_best[q * T + tid + 32 * w];
+                            const int ot = snn_tile[q * T + tid + 32 * w];
+                            if (ob < b || (ob == b && ot < bt)) { b = ob; bt = ot; }
+                        }
+                        a.nn_partial[row * d.ti + il] = make_float2(b, __int_as_float(bt));
+                    }
                     const double* sa = sacc + (q * NACC) * T + tid;
                     double t[NACC];
 #pragma unroll
@@ -521,6 +609,48 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
                     }
                     __syncthreads();
                 }
+                if (NN) {
+                    // smallest s over the CTAs' rows (ties: lowest tile), then re-scan that tile
+                    float b = __int_as_float(0x7f800000);
+                    int bt = -1;
+                    for (int k = ty; k < d.G; k += RY) {
+                        const float2 c = __ldcg(a.nn_partial + static_cast<long long>(k) * d.maxseg * d.ti + tx);
+                        const int ct = __float_as_int(c.y);
+                        if (c.x < b || (c.x == b && ct < bt)) { b = c.x; bt = ct; }
+                    }
+                    snn_best[tid] = b;
+                    snn_tile[tid] = bt;
+                    __syncthreads();
+                    for (int st = RY >> 1; st > 0; st >>= 1) {
+                        if (ty < st) {
+                            const float ob = snn_best[tid + st * 32];
+                            const int ot = snn_tile[tid + st * 32];
+                            if (ob < snn_best[tid] || (ob == snn_best[tid] && ot < snn_tile[tid])) {
+                                snn_best[tid] = ob;
+                                snn_tile[tid] = ot;
+                            }
+                        }
+                        __syncthreads();
+                    }
+                    for (int i = warp; i < d.n_i; i += W) {   // one warp per i-particle
+                        int idx = a.tail.inline_index ? a.tail.i_inline[i]
+                                                      : (a.i_index ? a.i_index[i] : i);
+                        float x = 0.f, y = 0.f, z = 0.f;
+                        if (idx >= 0) { x = a.j.x[idx]; y = a.j.y[idx]; z = a.j.z[idx]; }
+                        if (a.xi) { x = a.xi[3 * i]; y = a.xi[3 * i + 1]; z = a.xi[3 * i + 2]; }
+                        int nn;
+                        float r2;
+                        nn_scan(a.j, d.n_j, snn_tile[i], d.tj, -x, -y, -z, idx, a.eps2, lane, &nn, &r2);
+                        if (lane == 0) {
+                            a.nn_index[i] = nn;
+                            a.nn_r2[i] = r2;
+                            if (a.tail.host_out) {
+                                a.tail.host_out[7 * d.n_i + i] = __int_as_float(nn);
+                                a.tail.host_out[8 * d.n_i + i] = r2;
+                            }
+                        }
+                    }
+                }
                 if (ty == 0 && tx < d.n_i) {
                     const int n = d.n_i;
                     float r[7];
@@ -568,9 +698,11 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
 // n_i >= 32, else the next power of two >= n_i so that small blocks still use every thread.
 // All i of a block lie in one i-tile (ix divides 32 divides ti); the CTAs that worked on that
 // tile are found from the first/last i-tile tables the host filled (no division on the device).
-template <bool JERK>
+template <bool JERK, bool NN>
 __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_log2) {
     __shared__ double sh[7][256];
+    __shared__ float shb[NN ? 256 : 1];
+    __shared__ int sht[NN ? 256 : 1];
     __shared__ int krange[2];
     const Decomp& d = a.d;
     const int ix = 1 << ix_log2, ry = 256 >> ix_log2;
@@ -587,6 +719,8 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
     }
     __syncthreads();
     double s[7] = {0, 0, 0, 0, 0, 0, 0};
+    float nb = __int_as_float(0x7f800000);
+    int nt = -1;
     if (valid) {
         const int il = static_cast<int>(i - static_cast<long long>(it) * d.ti);
         const int k0 = krange[0], k1 = krange[1];
@@ -594,6 +728,11 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
         for (int k = k0 + ty; k <= k1; k += ry) {
             const int seg = it - a.it_first[k];
             const long long row = static_cast<long long>(k) * d.maxseg + seg;
+            if (NN) {
+                const float2 c = a.nn_partial[row * d.ti + il];
+                const int ct = __float_as_int(c.y);
+                if (c.x < nb || (c.x == nb && ct < nt)) { nb = c.x; nt = ct; }
+            }
             const float4* p = reinterpret_cast<const float4*>(a.partial + (row * d.ti + il) * 8);
             const float4 u = p[0];
             s[0] += u.x; s[1] += u.y; s[2] += u.z; s[3] += u.w;
@@ -605,13 +744,23 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
     }
 #pragma unroll
     for (int v = 0; v < 7; ++v) sh[v][tid] = s[v];
+    if (NN) { shb[tid] = nb; sht[tid] = nt; }
     __syncthreads();
     for (int st = ry >> 1; st > 0; st >>= 1) {   // fixed-order tree: deterministic result
         if (ty < st) {
 #pragma unroll
             for (int v = 0; v < 7; ++v) sh[v][tid] += sh[v][tid + st * ix];
+            if (NN) {
+                const float ob = shb[tid + st * ix];
+                const int ot = sht[tid + st * ix];
+                if (ob < shb[tid] || (ob == shb[tid] && ot < sht[tid])) { shb[tid] = ob; sht[tid] = ot; }
+            }
         }
         __syncthreads();
+    }
+    if (NN && ty == 0 && valid) {
+        a.nn_best[i] = shb[tid];
+        a.nn_tile[i] = sht[tid];
     }
     if (ty == 0 && valid) {
         a.acc[3 * i + 0] = static_cast<float>(sh[0][tid]);
@@ -621,6 +770,24 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
         a.jerk[3 * i + 0] = static_cast<float>(sh[4][tid]);
         a.jerk[3 * i + 1] = static_cast<float>(sh[5][tid]);
         a.jerk[3 * i + 2] = static_cast<float>(sh[6][tid]);
+    }
+}
+
+// One warp per i-particle: find the index inside the winning tile (two-kernel path).
+__global__ void __launch_bounds__(256) nn_scan_kernel(const NnScanArgs a) {
+    const int lane = threadIdx.x & 31;
+    const int i = blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (i >= a.n_i) return;
+    const int idx = a.i_index ? a.i_index[i] : i;
+    float x = 0.f, y = 0.f, z = 0.f;
+    if (idx >= 0) { x = a.j.x[idx]; y = a.j.y[idx]; z = a.j.z[idx]; }
+    if (a.xi) { x = a.xi[3 * i]; y = a.xi[3 * i + 1]; z = a.xi[3 * i + 2]; }
+    int nn;
+    float r2;
+    nn_scan(a.j, a.n_j, a.nn_tile[i], a.tj, -x, -y, -z, idx, a.eps2, lane, &nn, &r2);
+    if (lane == 0) {
+        a.nn_index[i] = nn;
+        a.nn_r2[i] = r2;
     }
 }
 
@@ -654,7 +821,8 @@ __global__ void predict_kernel(const RawJ raw, double t, long long n_j, long lon
                                float* pvz) {
     const long long j = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (j >= n_pad) return;
-    float o[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    // padding (n_j <= j < n_pad): massless and far away, so that it is nobody's neighbour
+    float o[7] = {1e18f, 1e18f, 1e18f, 0.f, 0.f, 0.f, 0.f};
     if (j < n_j) {
         const double dt = t - raw.t[j];
         const double dt2 = dt * dt * 0.5, dt3 = dt * dt * dt * (1.0 / 6.0);
@@ -680,7 +848,8 @@ __global__ void predict_upd_kernel(const RawJ raw, double t, long long n_j, long
                                    float* pvy, float* pvz, const InlineJ upd) {
     const long long j = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (j >= n_pad) return;
-    float o[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    // padding (n_j <= j < n_pad): massless and far away, so that it is nobody's neighbour
+    float o[7] = {1e18f, 1e18f, 1e18f, 0.f, 0.f, 0.f, 0.f};
     if (j < n_j) {
         int hit = -1;
         for (int k = 0; k < upd.n; ++k)
@@ -719,9 +888,9 @@ __global__ void predict_upd_kernel(const RawJ raw, double t, long long n_j, long
 }
 
 // --------------------------------------------------------------------------------- launchers
-template <int I, bool JERK, bool EPS0, bool PACKED>
-static cudaError_t prepare_of() {
-    auto fn = force_kernel<I, JERK, EPS0, PACKED>;
+template <int I, bool JERK, bool EPS0, bool PACKED, bool NN>
+static cudaError_t prepare_nn() {
+    auto fn = force_kernel<I, JERK, EPS0, PACKED, NN>;
     const size_t smem = smem_bytes_of<I, JERK>();
     cudaError_t err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            static_cast<int>(smem));
@@ -732,9 +901,26 @@ static cudaError_t prepare_of() {
     return nb >= 1 ? cudaSuccess : cudaErrorLaunchOutOfResources;
 }
 
+// the nearest-neighbour form exists for the packed acc + jerk + pot kernels only
 template <int I, bool JERK, bool EPS0, bool PACKED>
-static cudaError_t launch_of(const ForceArgs& a, cudaStream_t s) {
-    force_kernel<I, JERK, EPS0, PACKED><<<a.d.G, warps_of(I) * 32, smem_bytes_of<I, JERK>(), s>>>(a);
+static cudaError_t prepare_of() {
+    cudaError_t err = prepare_nn<I, JERK, EPS0, PACKED, false>();
+    if (err != cudaSuccess) return err;
+    if constexpr (JERK && PACKED) err = prepare_nn<I, JERK, EPS0, PACKED, true>();
+    return err;
+}
+
+template <int I, bool JERK, bool EPS0, bool PACKED>
+static cudaError_t launch_of(const ForceArgs& a, bool nn, cudaStream_t s) {
+    const size_t smem = smem_bytes_of<I, JERK>();
+    if constexpr (JERK && PACKED) {
+        if (nn) {
+            force_kernel<I, JERK, EPS0, PACKED, true><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
+            return cudaGetLastError();
+        }
+    }
+    if (nn) return cudaErrorInvalidValue;
+    force_kernel<I, JERK, EPS0, PACKED, false><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -773,13 +959,13 @@ static cudaError_t launch_of(const ForceArgs& a, cudaStream_t s) {
 size_t force_smem_bytes(const Variant& v) {
     const int nacc = v.jerk ? 10 : 4, narr = v.jerk ? 7 : 4;
     return 128 + sizeof(float) * kStages * narr * kTileJMax +
-           sizeof(double) * nacc * v.I * warps_of(v.I) * 32;
+           sizeof(double) * nacc * v.I * warps_of(v.I) * 32 + 8 * v.I * warps_of(v.I) * 32;
 }
 
 cudaError_t force_prepare(const Variant& v) { NBK_DISPATCH(prepare_of); }
 
 cudaError_t launch_force(const Variant& v, const ForceArgs& a, cudaStream_t s) {
-    NBK_DISPATCH(launch_of, a, s);
+    NBK_DISPATCH(launch_of, a, v.nn, s);
 }
 
 cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s) {
@@ -787,8 +973,15 @@ cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s)
     while (ix_log2 > 0 && (1 << (ix_log2 - 1)) >= a.d.n_i) --ix_log2;
     const int ix = 1 << ix_log2;
     const unsigned grid = static_cast<unsigned>((a.d.n_i + ix - 1) / ix);
-    if (v.jerk) reduce_kernel<true><<<grid, 256, 0, s>>>(a, ix_log2);
-    else reduce_kernel<false><<<grid, 256, 0, s>>>(a, ix_log2);
+    if (v.jerk && v.nn) reduce_kernel<true, true><<<grid, 256, 0, s>>>(a, ix_log2);
+    else if (v.jerk) reduce_kernel<true, false><<<grid, 256, 0, s>>>(a, ix_log2);
+    else reduce_kernel<false, false><<<grid, 256, 0, s>>>(a, ix_log2);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_nn_scan(const NnScanArgs& a, cudaStream_t s) {
+    if (a.n_i <= 0) return cudaSuccess;
+    nn_scan_kernel<<<(a.n_i + 7) / 8, 256, 0, s>>>(a);
     return cudaGetLastError();
 }
 

@@ -31,6 +31,7 @@ struct JPred {
 // pair p = it * njt + jt;  CTA k owns pairs [k*P/G, (k+1)*P/G).
 struct Decomp {
     int n_i;          // active i-particles
+    int n_j;          // j-particles (unpadded)
     int ti;           // i-particles per CTA tile = (W / wj) * 32 * I
     int tj;           // j-particles per tile (64, 128 or 256)
     int wj;           // warps that split each j-tile; W / wj warps split the i-tile
@@ -46,6 +47,7 @@ struct Variant {
     bool jerk;
     bool eps0;
     bool packed;  // f32x2 inner loop
+    bool nn;      // nearest neighbour too (instantiated for jerk && packed only)
 };
 
 // Host-only planner (nbk_api.cu): choose I, wj, tj and the pair split for (n_i, n_j).
@@ -79,6 +81,9 @@ struct ForceArgs {
     const float* xi;         // [n_i][3] or nullptr
     const float* vi;         // [n_i][3] or nullptr
     float* partial;          // [k*maxseg+seg][ti][8]
+    float2* nn_partial;      // [k*maxseg+seg][ti] (smallest s, its j-tile as int bits); NN only
+    int32_t* nn_index;       // [n_i] results of the nearest-neighbour search (NN only)
+    float* nn_r2;            // [n_i]
     float eps2;
     Decomp d;
     FusedTail tail;
@@ -88,6 +93,9 @@ struct ReduceArgs {
     int it_first[kMaxCtas];  // first / last i-tile CTA k works on (host-filled from the pair split)
     int it_last[kMaxCtas];
     const float* partial;
+    const float2* nn_partial;  // NN only
+    float* nn_best;            // [n_i] smallest s over all rows (NN only)
+    int32_t* nn_tile;          // [n_i] its j-tile
     float* acc;   // [n_i][3]
     float* jerk;  // [n_i][3]
     float* pot;   // [n_i]
@@ -109,6 +117,19 @@ size_t force_smem_bytes(const Variant& v);
 cudaError_t force_prepare(const Variant& v);
 cudaError_t launch_force(const Variant& v, const ForceArgs& a, cudaStream_t s);
 cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s);
+// Nearest neighbour, second step for the two-kernel path: one warp per i re-scans the winning tile.
+struct NnScanArgs {
+    JPred j;
+    const int32_t* i_index;
+    const float* xi;
+    const float* nn_best;
+    const int32_t* nn_tile;
+    int32_t* nn_index;
+    float* nn_r2;
+    int n_i, n_j, tj;
+    float eps2;
+};
+cudaError_t launch_nn_scan(const NnScanArgs& a, cudaStream_t s);
 
 // set_j scatter: staged particles -> raw SoA at addr (nullptr: identity).  x, v as fp32 or fp64.
 struct ScatterArgs {

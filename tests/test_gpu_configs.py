@@ -374,3 +374,85 @@ def test_set_j_of_a_few_particles_rides_in_the_launch(gpu):
     assert np.array_equal(gv[addr], ev[addr].astype(np.float32))
     assert np.array_equal(gm, em.astype(np.float32))
     assert np.array_equal(gx[rest], (x[rest] + v[rest].astype(np.float32).astype(np.float64) * 0.25).astype(np.float32))
+
+
+# ----------------------------------------------------------------------------- nearest neighbour
+def _check_nn(got_nn, got_r2, ref_nn, ref_r2, x, idx, xi=None, what=""):
+    """Index bit-exact where the answer is unique in fp32; where the GPU picked another j, that j
+    must be as near as the true neighbour to within fp32 rounding of the squared distance."""
+    got_nn = np.asarray(got_nn, np.int64)
+    same = got_nn == ref_nn
+    xs = x[np.maximum(idx, 0)].astype(np.float64) if xi is None else xi.astype(np.float64)
+    bad = np.nonzero(~same)[0]
+    for k in bad:
+        assert got_nn[k] >= 0 and got_nn[k] != idx[k], f"{what}: invalid neighbour for i={k}"
+        d = x[got_nn[k]].astype(np.float64) - xs[k]
+        r2 = float(d @ d)
+        assert r2 <= ref_r2[k] * (1 + 1e-6) + 1e-12, f"{what}: i={k} got j={got_nn[k]} r2={r2} ref {ref_r2[k]}"
+    assert bad.size <= max(2, 1e-4 * same.size), f"{what}: {bad.size} near-ties of {same.size}"
+    fin = np.isfinite(ref_r2)
+    assert np.allclose(got_r2[fin], ref_r2[fin], rtol=2e-6, atol=1e-12), what
+    return bad.size
+
+
+@pytest.mark.parametrize("n,n_i,eps", [(1024, 1024, EPS), (4099, 777, EPS), (4099, 4099, 0.0),
+                                       (6000, 1, EPS), (6000, 5, EPS), (6000, 32, 0.0), (300, 300, EPS)])
+def test_nearest_neighbour_matches_oracle(gpu, c_oracle, n, n_i, eps):
+    """SURVEY 8(f)-2 / PAPER.md L126-L128: neighbour index and distance from the force kernel, every
+    launch shape (one-launch small blocks, split-j, full), plus: the forces do not change."""
+    m, x, v = inputs.plummer_f32(n, seed=200 + n)
+    if n == 300:                       # duplicates: the twin is the neighbour at distance 0
+        x[17] = x[250]
+        x[100] = x[101]
+    idx = inputs.active_block(n, n_i, seed=9)
+    ref_nn, ref_r2 = c_oracle.nearest_neighbour(x, i_index=idx)
+    with Ctx(n) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, n, n_i, idx, None, None, np.float32(eps) ** 2, FULL)
+        plain = nb.nbk_calc_lasthalf(ctx, n_i)
+        nb.nbk_calc_firsthalf(ctx, n, n_i, idx, None, None, np.float32(eps) ** 2, FULL | nb.NBK_NN)
+        withnn = nb.nbk_calc_lasthalf(ctx, n_i)
+        nn, r2 = nb.nbk_get_neighbours(ctx, n_i)
+        with pytest.raises(nb.NbkError):
+            nb.nbk_calc_firsthalf(ctx, n, n_i, idx, None, None, np.float32(eps) ** 2, nb.NBK_POT | nb.NBK_NN)
+    for a, b in zip(plain, withnn):
+        assert np.array_equal(a, b)
+    _check_nn(nn, r2, ref_nn, ref_r2, x, idx, what=f"nn n={n} n_i={n_i} eps={eps}")
+    if n == 300:
+        pos = {int(i): k for k, i in enumerate(idx)}
+        assert nn[pos[17]] == 250 and nn[pos[250]] == 17 and nn[pos[100]] == 101 and r2[pos[100]] == 0.0
+
+
+def test_nearest_neighbour_external_particles_and_j_subset(gpu, c_oracle):
+    m, x, v = inputs.plummer_f32(3000, seed=231)
+    rng = np.random.default_rng(3)
+    n_i, n_j = 90, 2500
+    idx = np.full(n_i, -1, np.int32)
+    idx[::3] = rng.choice(n_j, size=idx[::3].size, replace=False)
+    xi = (0.4 * rng.standard_normal((n_i, 3))).astype(np.float32)
+    ref_nn, ref_r2 = c_oracle.nearest_neighbour(x[:n_j], i_index=idx, xi=xi)
+    with Ctx(3000) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, n_j, n_i, idx, xi, None, np.float32(EPS) ** 2, FULL | nb.NBK_NN)
+        nb.nbk_calc_lasthalf(ctx, n_i)
+        nn, r2 = nb.nbk_get_neighbours(ctx, n_i)
+    assert nn.max() < n_j
+    _check_nn(nn, r2, ref_nn, ref_r2, x, idx, xi=xi, what="nn external")
+
+
+def test_nearest_neighbour_c3_full(gpu, c_oracle):
+    """N = 131072, all i, in the launch shape of the headline run."""
+    m, x, v = inputs.config_inputs("C3")
+    n = m.shape[0]
+    ref_nn, ref_r2 = c_oracle.nearest_neighbour(x)
+    with Ctx(n) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, n, n, None, None, None, np.float32(EPS) ** 2, FULL | nb.NBK_NN)
+        nb.nbk_calc_lasthalf(ctx, n)
+        nn, r2 = nb.nbk_get_neighbours(ctx, n)
+        assert nb.nbk_last_launch(ctx)["launches"] == 3
+    nbad = _check_nn(nn, r2, ref_nn, ref_r2, x, np.arange(n), what="nn C3")
+    print(f"C3 nearest neighbour: {nbad} fp32 near-ties of {n}")
