@@ -174,6 +174,17 @@ int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, double* x, doub
                        double eps, double t_end, double eta, double dt_max,
                        nbk_hermite_stats* stats);
 
+/* The same integration with the whole block-step loop on the device (PAPER.md
+ * L346, L368 name it as what fp64 GPUs make possible): after the forces at t = 0, every block step
+ * is five stream-ordered launches -- scheduler (next block time from per-level particle counts),
+ * predictor + selection of the particles due, i x j force kernel planned on the device, reduction,
+ * fp64 corrector + Aarseth step + block rule -- enqueued in batches of 256 steps with no host
+ * synchronisation in between.  Same scheme, formulas and arguments as nbk_hermite_evolve (dt_max
+ * <= 1); stats->gpu_call_seconds equals wall_seconds. */
+int nbk_hermite_evolve_dev(nbk_ctx* ctx, int64_t n, const double* m, double* x, double* v,
+                           double eps, double t_end, double eta, double dt_max,
+                           nbk_hermite_stats* stats);
+
 /* ---- utilities --------------------------------------------------------------------------- */
 
 /* Block until everything enqueued on the context's stream has run. */

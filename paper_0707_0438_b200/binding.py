@@ -22,7 +22,7 @@ EXPORTS = [
     "nbk_set_j_particles_dev", "nbk_set_ti", "nbk_predict", "nbk_get_predicted",
     "nbk_calc_firsthalf", "nbk_calc_firsthalf_dev", "nbk_calc_lasthalf", "nbk_calc_lasthalf_dev",
     "nbk_get_neighbours", "nbk_get_neighbours_dev",
-    "nbk_hermite_evolve", "nbk_sync", "nbk_set_timing", "nbk_get_timing", "nbk_last_launch",
+    "nbk_hermite_evolve", "nbk_hermite_evolve_dev", "nbk_sync", "nbk_set_timing", "nbk_get_timing", "nbk_last_launch",
     "nbk_plan", "nbk_set_variant", "nbk_last_cuda_error", "nbk_strerror", "nbk_version",
 ]
 
@@ -54,6 +54,8 @@ _SIGS = {
     "nbk_get_neighbours_dev": (_i32, [_vp, _i64, _vp, _vp]),
     "nbk_hermite_evolve": (_i32, [_vp, _i64, _vp, _vp, _vp, _f64, _f64, _f64, _f64,
                                   ctypes.POINTER(HermiteStats)]),
+    "nbk_hermite_evolve_dev": (_i32, [_vp, _i64, _vp, _vp, _vp, _f64, _f64, _f64, _f64,
+                                      ctypes.POINTER(HermiteStats)]),
     "nbk_sync": (_i32, [_vp]),
     "nbk_set_timing": (_i32, [_vp, _i32]),
     "nbk_get_timing": (_i32, [_vp, ctypes.POINTER(_f32 * 4)]),
@@ -216,7 +218,12 @@ def nbk_get_neighbours_dev(ctx, n_i, nn_index=0, nn_r2=0):
            load().nbk_get_neighbours_dev(ctx, n_i, nn_index or None, nn_r2 or None), ctx)
 
 
-def nbk_hermite_evolve(ctx, m, x, v, eps, t_end, eta=0.01, dt_max=1.0 / 16.0):
+def nbk_hermite_evolve_dev(ctx, m, x, v, eps, t_end, eta=0.01, dt_max=1.0 / 16.0):
+    """Device-resident block-step loop; same arguments and return value as nbk_hermite_evolve."""
+    return nbk_hermite_evolve(ctx, m, x, v, eps, t_end, eta, dt_max, _fn="nbk_hermite_evolve_dev")
+
+
+def nbk_hermite_evolve(ctx, m, x, v, eps, t_end, eta=0.01, dt_max=1.0 / 16.0, _fn="nbk_hermite_evolve"):
     """x, v: float64 [n,3] arrays updated IN PLACE.  Returns a dict of nbk_hermite_stats."""
     m = np.ascontiguousarray(m, np.float64)
     if not (isinstance(x, np.ndarray) and x.dtype == np.float64 and x.flags.c_contiguous
@@ -226,8 +233,8 @@ def nbk_hermite_evolve(ctx, m, x, v, eps, t_end, eta=0.01, dt_max=1.0 / 16.0):
     if x.shape != (n, 3) or v.shape != (n, 3):
         raise ValueError("x, v must be [n,3]")
     st = HermiteStats()
-    _check("nbk_hermite_evolve",
-           load().nbk_hermite_evolve(ctx, n, m.ctypes.data, x.ctypes.data, v.ctypes.data, float(eps),
+    _check(_fn,
+           getattr(load(), _fn)(ctx, n, m.ctypes.data, x.ctypes.data, v.ctypes.data, float(eps),
                                      float(t_end), float(eta), float(dt_max), ctypes.byref(st)), ctx)
     out = {k: getattr(st, k) for k, _ in HermiteStats._fields_ if k != "ni_histogram"}
     out["ni_histogram"] = list(st.ni_histogram)

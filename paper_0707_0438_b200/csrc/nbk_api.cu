@@ -4,7 +4,9 @@
 // device nbk_open fails with NBK_ECUDA.
 #include <cuda_runtime.h>
 
+#include <chrono>
 #include <climits>
+#include <cmath>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -62,6 +64,10 @@ struct nbk_ctx {
     int32_t* d_nn_index = nullptr;  // [ni_max] result
     float* d_nn_r2 = nullptr;       // [ni_max] result
     bool last_nn = false;           // the last firsthalf asked for nearest neighbours
+    HermiteState hs{};              // device-resident integrator state (allocated on first use)
+    long long hs_cap = 0;
+    DynHeader* d_hdr = nullptr;
+    DynHeader* h_hdr = nullptr;     // pinned
     bool host_has_result = false;   // the last firsthalf wrote h_result itself (no D2H needed)
     InlineJ pending;                // a small set_j not yet on the device (pending.n == 0: none)
 
@@ -124,6 +130,9 @@ void free_all(nbk_ctx* c) {
     cudaFree(c->raw.m); cudaFree(c->raw.t); cudaFree(c->pred);
     cudaFree(c->d_iidx); cudaFree(c->d_xi); cudaFree(c->d_vi);
     cudaFree(c->d_partial); cudaFree(c->d_result); cudaFree(c->d_stage); cudaFree(c->d_counter);
+    cudaFree(c->hs.x); cudaFree(c->hs.v); cudaFree(c->hs.a); cudaFree(c->hs.j);
+    cudaFree(c->hs.level); cudaFree(c->hs.act); cudaFree(c->hs.bc_ge); cudaFree(c->d_hdr);
+    if (c->h_hdr) cudaFreeHost(c->h_hdr);
     cudaFree(c->d_nn_partial); cudaFree(c->d_nn_best); cudaFree(c->d_nn_tile);
     cudaFree(c->d_nn_index); cudaFree(c->d_nn_r2);
     if (c->h_result) cudaFreeHost(c->h_result);
@@ -180,44 +189,19 @@ void plan_shape(long long n_i, long long n_j, int num_sms, int force_I, size_t m
                 Variant* v, Decomp* d) {
     static const int kI[3] = {4, 2, 1};
     static const double kSpeed[3] = {1.0, 0.96, 0.86};
-    static const int kTj[3] = {256, 128, 64};
     double best = -1.0;
     for (int a = 0; a < 3; ++a) {
         const int I = kI[a];
         if (force_I > 0 && I != force_I) continue;
-        const int W = warps_of(I);
-        for (int wj = 1; wj <= W; wj *= 2) {
-            if (W % wj) continue;
-            for (int b = 0; b < 3; ++b) {
-                const int tj = kTj[b];
-                if (tj / wj < 4) continue;
-                const long long ti = static_cast<long long>(W / wj) * 32 * I;
-                const long long nit = (n_i + ti - 1) / ti;
-                const long long njt = (n_j + tj - 1) / tj;
-                const long long P = nit * njt;
-                const long long gmax = num_sms < kMaxCtas ? num_sms : kMaxCtas;
-                const long long G = P < gmax ? P : gmax;
-                const long long per = (P + G - 1) / G;
-                const long long maxseg = (per - 1 + njt - 1) / njt + 1;
-                if (static_cast<size_t>(G) * maxseg * ti * 8 > max_partial_floats) continue;
-                // per-pair time of one CTA: its W warps share the FP32 pipe, each does tj/wj j-steps
-                // for I i-particles plus the per-tile work (barriers, fp64 fold)
-                const double pair = W * ((static_cast<double>(tj) / wj) * I + 6.0 * I + 24.0);
-                const double cost = per * pair / kSpeed[a];
-                if (best < 0.0 || cost < best * (1.0 - 1e-9)) {
-                    best = cost;
-                    v->I = I;
-                    d->n_i = static_cast<int>(n_i);
-                    d->ti = static_cast<int>(ti);
-                    d->tj = tj;
-                    d->wj = wj;
-                    d->nit = static_cast<int>(nit);
-                    d->njt = static_cast<int>(njt);
-                    d->P = P;
-                    d->G = static_cast<int>(G);
-                    d->maxseg = static_cast<int>(maxseg);
-                }
-            }
+        Decomp cand;
+        const long long c = plan_fixed_i(n_i, n_j, num_sms, I, max_partial_floats, &cand);
+        if (c < 0) continue;
+        // a CTA's warps share the FP32 pipe: time per pair grows with the warp count
+        const double cost = static_cast<double>(c) * warps_of(I) / kSpeed[a];
+        if (best < 0.0 || cost < best * (1.0 - 1e-9)) {
+            best = cost;
+            v->I = I;
+            *d = cand;
         }
     }
 }
@@ -269,6 +253,7 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     if (d.G < 1 || plan_partial_floats(d) * sizeof(float) > c->partial_bytes) return NBK_ENOMEM;
 
     ForceArgs fa;
+    fa.dyn = nullptr;
     fa.j = jpred_of(c);
     fa.i_index = d_iidx; fa.xi = d_xi; fa.vi = d_vi;
     fa.partial = c->d_partial;
@@ -276,7 +261,6 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     fa.nn_index = c->d_nn_index;
     fa.nn_r2 = c->d_nn_r2;
     fa.eps2 = eps2;
-    d.n_j = static_cast<int>(n_j);
     fa.d = d;
     std::memset(&fa.tail, 0, sizeof(fa.tail));
     const bool fused = v.I == 1 && d.nit == 1 && n_i <= kFusedMaxI && c->fused_ok;
@@ -315,6 +299,8 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
         return NBK_OK;
     }
     ReduceArgs ra;
+    ra.dyn = nullptr;
+    ra.n_j = static_cast<int>(n_j);
     for (int k = 0; k < d.G; ++k) {
         const long long q0 = (static_cast<long long>(k) * d.P) / d.G;
         const long long q1 = ((static_cast<long long>(k) + 1) * d.P) / d.G;
@@ -720,6 +706,178 @@ int nbk_get_neighbours_dev(nbk_ctx* c, int64_t n_i, int32_t* nn_index, float* nn
     const size_t ni = static_cast<size_t>(n_i);
     if (nn_index) NBK_CUDA(c, cudaMemcpyAsync(nn_index, c->d_nn_index, sizeof(int32_t) * ni, cudaMemcpyDeviceToDevice, c->stream));
     if (nn_r2) NBK_CUDA(c, cudaMemcpyAsync(nn_r2, c->d_nn_r2, sizeof(float) * ni, cudaMemcpyDeviceToDevice, c->stream));
+    return NBK_OK;
+}
+
+// ---- a8 on the device: the whole block-step loop without host round trips ----
+int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, double* v, double eps,
+                           double t_end, double eta, double dt_max, nbk_hermite_stats* stats) {
+    if (!c || n < 1 || !m || !x || !v || !(eps >= 0.0) || !(t_end >= 0.0) || !(eta > 0.0) ||
+        !(dt_max > 0.0) || n > INT32_MAX)
+        return NBK_EINVAL;
+    if (n > c->n_max || n > c->ni_max) return NBK_ERANGE;
+    int e0;
+    std::frexp(dt_max, &e0);
+    int kmin = -(e0 - 1);            // dt_max rounded down to a power of two
+    if (kmin < -10) kmin = -10;
+    if (kmin < 0 || kmin > kMaxLevel) return NBK_EINVAL;   // dt_max in (2^-48, 1]... 2^0
+    const double dtm = std::ldexp(1.0, -kmin);
+    if (t_end > 2047.0 || std::fmod(t_end, dtm) != 0.0) return NBK_EINVAL;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    const auto wall0 = std::chrono::steady_clock::now();
+    const size_t N = static_cast<size_t>(n);
+    const float eps2 = static_cast<float>(eps * eps);
+    const uint32_t flags = NBK_JERK | NBK_POT;
+    int rc;
+
+    if (c->hs_cap < n) {
+        cudaFree(c->hs.x); cudaFree(c->hs.v); cudaFree(c->hs.a); cudaFree(c->hs.j);
+        cudaFree(c->hs.level); cudaFree(c->hs.act); cudaFree(c->hs.bc_ge);
+        c->hs = HermiteState{};
+        c->hs_cap = 0;
+        NBK_CUDA(c, cudaMalloc(&c->hs.x, sizeof(double) * 3 * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.v, sizeof(double) * 3 * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.a, sizeof(double) * 3 * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.j, sizeof(double) * 3 * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.level, sizeof(int) * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.act, sizeof(int32_t) * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.bc_ge, sizeof(int) * (kMaxLevel + 1) * ((N + 255) / 256)));
+        c->hs_cap = n;
+    }
+    if (!c->d_hdr) NBK_CUDA(c, cudaMalloc(&c->d_hdr, sizeof(DynHeader)));
+    if (!c->h_hdr) NBK_CUDA(c, cudaMallocHost(&c->h_hdr, sizeof(DynHeader)));
+
+    // t = 0 through the ordinary entry points: forces on everybody, first steps (reading R15)
+    std::vector<float> fa(3 * N), fj(3 * N);
+    std::vector<double> a(3 * N), jk(3 * N), tl(N, 0.0);
+    std::vector<int> lev(N);
+    if ((rc = nbk_set_j_particles_f64(c, n, nullptr, nullptr, m, x, v, nullptr, nullptr)) != NBK_OK) return rc;
+    if ((rc = nbk_set_ti(c, 0.0)) != NBK_OK) return rc;
+    if ((rc = nbk_calc_firsthalf(c, n, n, nullptr, nullptr, nullptr, eps2, flags)) != NBK_OK) return rc;
+    if ((rc = nbk_calc_lasthalf(c, n, fa.data(), fj.data(), nullptr)) != NBK_OK) return rc;
+    DynHeader& H = *c->h_hdr;
+    std::memset(&H, 0, sizeof(H));
+    for (size_t i = 0; i < N; ++i) {
+        double na = 0.0, nj = 0.0;
+        for (int q = 0; q < 3; ++q) {
+            a[3 * i + q] = fa[3 * i + q];
+            jk[3 * i + q] = fj[3 * i + q];
+            na += a[3 * i + q] * a[3 * i + q];
+            nj += jk[3 * i + q] * jk[3 * i + q];
+        }
+        na = std::sqrt(na); nj = std::sqrt(nj);
+        double want = dtm;
+        if (nj > 0.0 && na > 0.0) want = std::fmin(0.25 * eta * na / nj, dtm);
+        int k = kMaxLevel;
+        if (want > 0.0) {
+            int e;
+            std::frexp(want, &e);
+            k = -(e - 1);
+            if (k < kmin) k = kmin;
+            if (k > kMaxLevel) k = kMaxLevel;
+        }
+        lev[i] = k;
+        H.level_count[k] += 1;
+    }
+    const int nblk = static_cast<int>((N + 255) / 256);
+    c->hs.nblk = nblk;
+    std::vector<int> bc(static_cast<size_t>(kMaxLevel + 1) * nblk, 0);
+    for (size_t i = 0; i < N; ++i)
+        for (int l = 0; l <= lev[i]; ++l) bc[static_cast<size_t>(l) * nblk + (i >> 8)] += 1;
+    if ((rc = nbk_set_j_particles_f64(c, n, nullptr, tl.data(), m, x, v, a.data(), jk.data())) != NBK_OK) return rc;
+    if ((rc = flush_pending(c)) != NBK_OK) return rc;
+    H.T_now = 0;
+    H.T_end = static_cast<long long>(std::ldexp(t_end, kTickLog2));
+    H.kmin = kmin;
+    H.n = static_cast<int>(n);
+    H.num_sms = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
+    H.max_partial_floats = c->partial_bytes / sizeof(float);
+    H.eta = eta;
+    H.interactions = n * n;
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.x, x, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.v, v, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.a, a.data(), sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.j, jk.data(), sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.level, lev.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.bc_ge, bc.data(), sizeof(int) * bc.size(), cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->d_hdr, &H, sizeof(H), cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaStreamSynchronize(c->stream));   // the host vectors above may go away
+
+    // one block step = begin, predict + select, force (+ reduce), correct; enqueued in batches with
+    // no host synchronisation inside a batch; steps past t_end return at once (done flag)
+    Variant vv{1, true, eps2 == 0.f, true, false};
+    const long long n_pad = round_up(n, kTileJMax);
+    const size_t ni_max = static_cast<size_t>(c->ni_max);
+    ForceArgs f;
+    std::memset(&f, 0, sizeof(f));
+    f.j = jpred_of(c);
+    f.i_index = c->hs.act;
+    f.partial = c->d_partial;
+    f.eps2 = eps2;
+    f.d.n_j = static_cast<int>(n);
+    f.tail.counter = c->d_counter;
+    f.tail.acc = c->d_result;
+    f.tail.jerk = c->d_result + 3 * ni_max;
+    f.tail.pot = c->d_result + 6 * ni_max;
+    f.dyn = c->d_hdr;
+    f.d.G = H.num_sms;   // grid: one CTA per SM; CTAs beyond the plan's G return
+    ReduceArgs r;
+    std::memset(&r, 0, sizeof(r));
+    r.partial = c->d_partial;
+    r.acc = f.tail.acc; r.jerk = f.tail.jerk; r.pot = f.tail.pot;
+    r.dyn = c->d_hdr;
+    r.n_j = static_cast<int>(n);
+    // the five launches of a block step are captured once into a CUDA graph and replayed
+    const int kBatch = 256;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t gexec = nullptr;
+    auto enqueue_step = [&]() -> cudaError_t {
+        cudaError_t e;
+        if ((e = launch_hd_begin(c->d_hdr, c->stream)) != cudaSuccess) return e;
+        if ((e = launch_hd_predict(c->raw, c->d_hdr, c->hs, n_pad, pred_arr(c, 0), pred_arr(c, 1),
+                                   pred_arr(c, 2), pred_arr(c, 3), pred_arr(c, 4), pred_arr(c, 5),
+                                   pred_arr(c, 6), c->stream)) != cudaSuccess) return e;
+        if ((e = launch_force(vv, f, c->stream)) != cudaSuccess) return e;
+        if ((e = launch_reduce_dyn(vv, r, static_cast<int>(n), c->stream)) != cudaSuccess) return e;
+        return launch_hd_correct(c->raw, c->d_hdr, c->hs, f.tail.acc, f.tail.jerk,
+                                 static_cast<int>(n), c->stream);
+    };
+    NBK_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
+    cudaError_t ce = enqueue_step();
+    cudaError_t ce2 = cudaStreamEndCapture(c->stream, &graph);
+    if (ce != cudaSuccess || ce2 != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        return cuda_fail(c, ce != cudaSuccess ? ce : ce2);
+    }
+    ce = cudaGraphInstantiate(&gexec, graph, 0);
+    if (ce != cudaSuccess) { cudaGraphDestroy(graph); return cuda_fail(c, ce); }
+    for (;;) {
+        for (int s = 0; s < kBatch && ce == cudaSuccess; ++s) ce = cudaGraphLaunch(gexec, c->stream);
+        if (ce == cudaSuccess)
+            ce = cudaMemcpyAsync(c->h_hdr, c->d_hdr, sizeof(DynHeader), cudaMemcpyDeviceToHost, c->stream);
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(c->stream);
+        if (ce != cudaSuccess || c->h_hdr->done) break;
+    }
+    cudaGraphExecDestroy(gexec);
+    cudaGraphDestroy(graph);
+    if (ce != cudaSuccess) return cuda_fail(c, ce);
+    NBK_CUDA(c, cudaMemcpyAsync(x, c->hs.x, sizeof(double) * 3 * N, cudaMemcpyDeviceToHost, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(v, c->hs.v, sizeof(double) * 3 * N, cudaMemcpyDeviceToHost, c->stream));
+    NBK_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->pred_valid = false;
+    c->in_flight = false;
+    if (stats) {
+        std::memset(stats, 0, sizeof(*stats));
+        stats->block_steps = c->h_hdr->block_steps;
+        stats->particle_steps = c->h_hdr->particle_steps;
+        stats->interactions = c->h_hdr->interactions;
+        stats->t_reached = std::ldexp(static_cast<double>(c->h_hdr->T_now), -kTickLog2);
+        for (int b = 0; b < 32; ++b) stats->ni_histogram[b] = c->h_hdr->hist[b];
+        stats->wall_seconds =
+            std::chrono::duration<double>(std::chrono::steady_clock::now() - wall0).count();
+        stats->gpu_call_seconds = stats->wall_seconds;
+    }
     return NBK_OK;
 }
 

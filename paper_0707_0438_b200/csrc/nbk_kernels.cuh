@@ -50,14 +50,93 @@ struct Variant {
     bool nn;      // nearest neighbour too (instantiated for jerk && packed only)
 };
 
-// Host-only planner (nbk_api.cu): choose I, wj, tj and the pair split for (n_i, n_j).
-// force_I > 0 pins I.  Fills *v (I only; flags are the caller's) and *d; candidates whose partial
-// rows exceed max_partial_floats are skipped (d->G stays untouched if none fits).
+// Planner for one i-per-thread count I: choose wj and tj and cut the pair list.  Runs on the host
+// (plan_shape tries I = 4, 2, 1) and on the device (the device-resident integrator plans its own
+// block steps with I = 1).  Cost of a candidate = pairs per CTA x (j-steps per warp per pair x I +
+// per-tile work); returns it, or -1 if no candidate fits max_partial_floats.
+constexpr int kPlanCandidates = 15;   // wj in {1,2,4,8,16} x tj in {256,128,64}
+__host__ __device__ inline long long plan_candidate(long long n_i, long long n_j, int num_sms, int I,
+                                                    unsigned long long max_partial_floats, int c,
+                                                    Decomp* d) {
+    const int W = warps_of(I);
+    const int wj = 1 << (c / 3), tj = 256 >> (c % 3);
+    if (wj > W || W % wj || tj / wj < 4) return -1;
+    const long long ti = static_cast<long long>(W / wj) * 32 * I;
+    const long long nit = (n_i + ti - 1) / ti;
+    const long long njt = (n_j + tj - 1) / tj;
+    const long long P = nit * njt;
+    const long long gmax = num_sms < kMaxCtas ? num_sms : kMaxCtas;
+    const long long G = P < gmax ? P : gmax;
+    const long long per = (P + G - 1) / G;
+    const long long maxseg = (per - 1 + njt - 1) / njt + 1;
+    if (static_cast<unsigned long long>(G) * maxseg * ti * 8 > max_partial_floats) return -1;
+    d->n_i = static_cast<int>(n_i);
+    d->n_j = static_cast<int>(n_j);
+    d->ti = static_cast<int>(ti);
+    d->tj = tj;
+    d->wj = wj;
+    d->nit = static_cast<int>(nit);
+    d->njt = static_cast<int>(njt);
+    d->P = P;
+    d->G = static_cast<int>(G);
+    d->maxseg = static_cast<int>(maxseg);
+    return per * (static_cast<long long>(tj / wj) * I + 6 * I + 24);
+}
+
+__host__ __device__ inline long long plan_fixed_i(long long n_i, long long n_j, int num_sms, int I,
+                                                  unsigned long long max_partial_floats, Decomp* d) {
+    long long best = -1;
+    for (int c = 0; c < kPlanCandidates; ++c) {   // first of the cheapest wins
+        Decomp cand;
+        const long long cost = plan_candidate(n_i, n_j, num_sms, I, max_partial_floats, c, &cand);
+        if (cost >= 0 && (best < 0 || cost < best)) {
+            best = cost;
+            *d = cand;
+        }
+    }
+    return best;
+}
+
+// Host planner (nbk_api.cu): the best of I = 4, 2, 1 (cost x warps / measured speed of that form).
+// force_I > 0 pins I.  Fills *v (I only; flags are the caller's) and *d; d->G stays untouched if no
+// candidate fits max_partial_floats.
 void plan_shape(long long n_i, long long n_j, int num_sms, int force_I, size_t max_partial_floats,
                 Variant* v, Decomp* d);
 // Floats of partial storage a plan needs, and the bound nbk_open allocates for (ni_max, num_sms).
 size_t plan_partial_floats(const Decomp& d);
 size_t plan_partial_floats_bound(long long ni_max, int num_sms);
+
+// ---- device-resident Hermite integrator: all block-step state lives here ------
+constexpr int kTickLog2 = 52;   // time unit 2^-52: exact integer block times
+constexpr int kMaxLevel = 48;   // finest step 2^-48
+struct DynHeader {
+    long long T_now, T_end, T_next;     // block times in ticks
+    double t_next;                      // T_next in time units
+    int kstar;                          // particles with level >= kstar are due at T_next
+    int n_act;                          // how many (from the level counts)
+    int done;                           // T_next would pass T_end: every kernel returns at once
+    int kmin;                           // coarsest level (dt_max = 2^-kmin)
+    int n;                              // particles
+    int num_sms;
+    unsigned long long max_partial_floats;
+    double eta;
+    long long block_steps, particle_steps, interactions;
+    long long level_count[kMaxLevel + 1];
+    long long hist[32];
+    Decomp plan;                        // launch plan of the current step (made once, hd_begin_kernel)
+    int fused;                          // the force kernel's last CTA reduces (small block)
+};
+struct HermiteState {        // fp64 integrator state, [n][3] row-major; level[n]
+    double* x;
+    double* v;
+    double* a;
+    double* j;
+    int* level;
+    int32_t* act;            // [n] indices of the particles due at T_next, ascending
+    int* bc_ge;              // [kMaxLevel + 1][nblk]: particles of index block b (256 indices) with
+                             // level >= k; gives each block its offset into act without a scan
+    int nblk;
+};
 
 constexpr int kFusedMaxI = 32;  // largest i-block served by the one-launch small-block path
 
@@ -87,6 +166,7 @@ struct ForceArgs {
     float eps2;
     Decomp d;
     FusedTail tail;
+    const DynHeader* dyn;    // non-null (I = 1 only): n_i and the launch plan come from the device
 };
 
 struct ReduceArgs {
@@ -100,6 +180,8 @@ struct ReduceArgs {
     float* jerk;  // [n_i][3]
     float* pot;   // [n_i]
     Decomp d;
+    const DynHeader* dyn;    // non-null: plan on the device (and return if the force kernel reduced)
+    int n_j;                 // dyn only
 };
 
 struct RawJ {        // raw j-state kept for the predictor, structure of arrays of capacity cap
@@ -166,5 +248,14 @@ cudaError_t launch_scatter_inline(const InlineJ& p, const RawJ& raw, cudaStream_
 cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n_pad, float* px,
                            float* py, float* pz, float* pm, float* pvx, float* pvy, float* pvz,
                            const InlineJ* upd, cudaStream_t st);
+
+// device-resident integrator kernels (one block step = begin, predict+select, force, reduce, correct)
+cudaError_t launch_hd_begin(DynHeader* h, cudaStream_t st);
+cudaError_t launch_hd_predict(const RawJ& raw, DynHeader* h, const HermiteState& hs, long long n_pad,
+                              float* px, float* py, float* pz, float* pm, float* pvx, float* pvy,
+                              float* pvz, cudaStream_t st);
+cudaError_t launch_hd_correct(const RawJ& raw, DynHeader* h, const HermiteState& hs, const float* acc,
+                              const float* jerk, int n, cudaStream_t st);
+cudaError_t launch_reduce_dyn(const Variant& v, const ReduceArgs& a, int ni_max, cudaStream_t s);
 
 }  // namespace nbk

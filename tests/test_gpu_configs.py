@@ -456,3 +456,58 @@ def test_nearest_neighbour_c3_full(gpu, c_oracle):
         assert nb.nbk_last_launch(ctx)["launches"] == 3
     nbad = _check_nn(nn, r2, ref_nn, ref_r2, x, np.arange(n), what="nn C3")
     print(f"C3 nearest neighbour: {nbad} fp32 near-ties of {n}")
+
+
+# ----------------------------------------------------------------------------- device-resident integrator
+def test_device_resident_hermite_small_n_matches_host_driver_and_oracle(gpu):
+    """the block-step loop on the device (scheduler from level counts, predictor +
+    selection, device-planned force, fp64 corrector) against the host driver and the fp64 oracle
+    integrator: same scheme => same step counts to a few per cent, nearby end states, same energy."""
+    from oracle import hermite_oracle, nbody_oracle
+    m, x, v = inputs.plummer(256, seed=11)
+    ref = hermite_oracle.evolve(m, x, v, EPS, 0.25)
+    hx, hv = x.copy(), v.copy()
+    dx, dv = x.copy(), v.copy()
+    with Ctx(256) as ctx:
+        sh = nb.nbk_hermite_evolve(ctx, m, hx, hv, EPS, 0.25)
+        sd = nb.nbk_hermite_evolve_dev(ctx, m, dx, dv, EPS, 0.25)
+    assert sd["t_reached"] == 0.25
+    assert abs(sd["particle_steps"] - ref["particle_steps"]) <= 0.05 * ref["particle_steps"]
+    assert abs(sd["particle_steps"] - sh["particle_steps"]) <= 0.02 * sh["particle_steps"]
+    assert sum(sd["ni_histogram"]) == sd["block_steps"]
+    e0 = nbody_oracle.energy(m, x, v, EPS)
+    assert abs((nbody_oracle.energy(m, dx, dv, EPS) - e0) / e0) < 1e-6
+    assert np.median(np.linalg.norm(dx - ref["x"], axis=1)) < 1e-4
+    assert np.median(np.linalg.norm(dx - hx, axis=1)) < 1e-4
+
+
+def test_device_resident_hermite_c5_energy(gpu, c_oracle):
+    """C5 on the device-resident loop: N=65536 to t=1, |dE/E| < 1e-6, same block-step statistics
+    as the host-driven run to within the sensitivity of step choices to fp32 force round-off."""
+    m, x, v = inputs.plummer(inputs.CONFIGS["C5"]["N"], inputs.CONFIGS["C5"]["seed"])
+    n = m.shape[0]
+    e0 = _energy(c_oracle, m, x, v, EPS)
+    with Ctx(n) as ctx:
+        st = nb.nbk_hermite_evolve_dev(ctx, m, x, v, EPS, 1.0, eta=0.01, dt_max=1.0 / 16.0)
+    e1 = _energy(c_oracle, m, x, v, EPS)
+    de = abs((e0 - e1) / e0)
+    print(f"C5 device-resident: dE/E={de:.3e} block_steps={st['block_steps']} "
+          f"particle_steps={st['particle_steps']} wall={st['wall_seconds']:.2f}s "
+          f"interactions={st['interactions']:.3e}")
+    assert st["t_reached"] == 1.0
+    assert de < 1e-6, de
+    assert 0.9 * 62748 < st["block_steps"] < 1.1 * 62748
+
+
+def test_device_resident_hermite_is_repeatable(gpu):
+    """The order in which due particles are collected is not fixed (atomic cursor), but each
+    particle's sums do not depend on its slot: two runs end in bit-identical states."""
+    m, x, v = inputs.plummer(3000, seed=17)
+    outs = []
+    with Ctx(3000) as ctx:
+        for _ in range(2):
+            gx, gv = x.copy(), v.copy()
+            st = nb.nbk_hermite_evolve_dev(ctx, m, gx, gv, EPS, 0.125)
+            outs.append((gx, gv, st["block_steps"], st["particle_steps"]))
+    assert outs[0][2:] == outs[1][2:]
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
