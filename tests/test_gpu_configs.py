@@ -511,3 +511,34 @@ def test_device_resident_hermite_is_repeatable(gpu):
             outs.append((gx, gv, st["block_steps"], st["particle_steps"]))
     assert outs[0][2:] == outs[1][2:]
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+@pytest.mark.parametrize("n_i", [1, 7, 32, 33, 200, 1531])
+def test_every_kernel_form_flag_and_block_size(gpu, c_oracle, n_i):
+    """Matrix: block sizes on both sides of the one-launch limit x {acc+jerk+pot, acc+pot, +NN, eps=0}
+    x {planner's choice, I pinned to 1/2/4, scalar loop, two-kernel path}; prediction active.
+    Every combination against the oracle on the device-predicted state."""
+    n = 1531
+    m, x, v = inputs.plummer_f32(n, seed=7)
+    a0, j0 = (0.1 * v).astype(np.float32), (0.01 * v).astype(np.float32)
+    idx = inputs.active_block(n, n_i, seed=3)
+    with Ctx(n) as ctx:
+        nb.nbk_set_j_particles(ctx, None, np.zeros(n), m, x, v, a0, j0)
+        nb.nbk_set_ti(ctx, 0.01)
+        nb.nbk_predict(ctx, n)
+        gm, gx, gv = nb.nbk_get_predicted(ctx, n)
+        refs = {eps: c_oracle.force(gm, gx, gv, eps, i_index=idx) for eps in (EPS, 0.0)}
+        ref_nn, ref_r2 = c_oracle.nearest_neighbour(gx, i_index=idx)
+        for flags in (FULL, nb.NBK_POT, FULL | nb.NBK_NN, FULL | nb.NBK_EPS0):
+            eps = 0.0 if flags & nb.NBK_EPS0 else EPS
+            jerk = bool(flags & nb.NBK_JERK)
+            for variant in (0x000, 0x010, 0x020, 0x040, 0x041, 0x100):
+                nb.nbk_set_variant(ctx, variant)
+                nb.nbk_calc_firsthalf(ctx, n, n_i, idx, None, None, np.float32(eps) ** 2, flags)
+                got = nb.nbk_calc_lasthalf(ctx, n_i)
+                assert_parity(got, refs[eps], jerk=jerk, what=f"n_i={n_i} flags={flags} variant={variant:#x}")
+                if not jerk:
+                    assert np.all(got[1] == 0)
+                if flags & nb.NBK_NN:
+                    nn, r2 = nb.nbk_get_neighbours(ctx, n_i)
+                    _check_nn(nn, r2, ref_nn, ref_r2, gx, idx, what=f"nn n_i={n_i} variant={variant:#x}")
