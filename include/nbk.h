@@ -152,6 +152,30 @@ int nbk_get_neighbours(nbk_ctx* ctx, int64_t n_i, int32_t* nn_index, float* nn_r
 /* Same to DEVICE arrays, asynchronous on the stream. */
 int nbk_get_neighbours_dev(nbk_ctx* ctx, int64_t n_i, int32_t* nn_index, float* nn_r2);
 
+/* ---- batched acceleration + potential calls --------------------------------
+ * the GRAPE treecode asks, for each group of particles, for the
+ * acceleration (no jerk, no neighbours) due to that group's interaction list; with one library
+ * call per group the paper needed groups of 8192-32768 particles.  Here all groups of a step are
+ * one call and one force launch (the tree walk itself is the caller's).
+ *   i_offset[n_groups + 1], j_offset[n_groups + 1]   HOST arrays, ascending from 0: group g owns
+ *       i-particles [i_offset[g], i_offset[g+1]) of xi / acc / pot and list entries
+ *       [j_offset[g], j_offset[g+1]) of mj / xj.
+ *   xi[n_i][3], mj[n_j], xj[n_j][3]    inputs;  acc[n_i][3], pot[n_i]  outputs
+ *       (host pointers for nbk_calc_batch, device pointers for nbk_calc_batch_dev).
+ * For every i of group g:  acc_i = sum_j m_j r s^(-3/2),  pot_i = -sum_j m_j s^(-1/2) over the
+ * group's list, r = x_j - x_i, s = r.r + eps2.  Nothing is left out by index: a list entry at the
+ * i-particle's own position adds 0 to acc and -m_j/eps to pot for eps2 > 0 (GRAPE callers subtract
+ * it), and is skipped with NBK_EPS0 or eps2 == 0.  flags: NBK_POT | NBK_EPS0 (NBK_JERK, NBK_NN:
+ * NBK_EINVAL).  i-particles of a group with an empty list get zeros.  Independent of the context's
+ * j-state; the library keeps its own growable device arena for the packed lists.  Both forms
+ * return after the work has run (the host form has then filled acc and pot). */
+int nbk_calc_batch(nbk_ctx* ctx, int64_t n_groups, const int64_t* i_offset, const float* xi,
+                   const int64_t* j_offset, const float* mj, const float* xj, float eps2,
+                   uint32_t flags, float* acc, float* pot);
+int nbk_calc_batch_dev(nbk_ctx* ctx, int64_t n_groups, const int64_t* i_offset, const float* xi,
+                       const int64_t* j_offset, const float* mj, const float* xj, float eps2,
+                       uint32_t flags, float* acc, float* pot);
+
 /* ---- a8: host Hermite driver (reading R15) ------------------- */
 
 typedef struct nbk_hermite_stats {

@@ -21,7 +21,7 @@ EXPORTS = [
     "nbk_open", "nbk_close", "nbk_npipes", "nbk_set_j_particles", "nbk_set_j_particles_f64",
     "nbk_set_j_particles_dev", "nbk_set_ti", "nbk_predict", "nbk_get_predicted",
     "nbk_calc_firsthalf", "nbk_calc_firsthalf_dev", "nbk_calc_lasthalf", "nbk_calc_lasthalf_dev",
-    "nbk_get_neighbours", "nbk_get_neighbours_dev",
+    "nbk_get_neighbours", "nbk_get_neighbours_dev", "nbk_calc_batch", "nbk_calc_batch_dev",
     "nbk_hermite_evolve", "nbk_hermite_evolve_dev", "nbk_sync", "nbk_set_timing", "nbk_get_timing", "nbk_last_launch",
     "nbk_plan", "nbk_set_variant", "nbk_last_cuda_error", "nbk_strerror", "nbk_version",
 ]
@@ -50,6 +50,8 @@ _SIGS = {
     "nbk_calc_firsthalf_dev": (_i32, [_vp, _i64, _i64, _vp, _vp, _vp, _f32, _u32]),
     "nbk_calc_lasthalf": (_i32, [_vp, _i64, _vp, _vp, _vp]),
     "nbk_calc_lasthalf_dev": (_i32, [_vp, _i64, _vp, _vp, _vp]),
+    "nbk_calc_batch": (_i32, [_vp, _i64, _vp, _vp, _vp, _vp, _vp, _f32, _u32, _vp, _vp]),
+    "nbk_calc_batch_dev": (_i32, [_vp, _i64, _vp, _vp, _vp, _vp, _vp, _f32, _u32, _vp, _vp]),
     "nbk_get_neighbours": (_i32, [_vp, _i64, _vp, _vp]),
     "nbk_get_neighbours_dev": (_i32, [_vp, _i64, _vp, _vp]),
     "nbk_hermite_evolve": (_i32, [_vp, _i64, _vp, _vp, _vp, _f64, _f64, _f64, _f64,
@@ -204,6 +206,31 @@ def nbk_calc_lasthalf(ctx, n_i):
 def nbk_calc_lasthalf_dev(ctx, n_i, acc=0, jerk=0, pot=0):
     _check("nbk_calc_lasthalf_dev",
            load().nbk_calc_lasthalf_dev(ctx, n_i, acc or None, jerk or None, pot or None), ctx)
+
+
+def nbk_calc_batch(ctx, i_offset, xi, j_offset, mj, xj, eps2=0.0, flags=NBK_POT):
+    """Host arrays in, (acc[n_i,3], pot[n_i]) out."""
+    io, pio = _host(i_offset, np.int64)
+    jo, pjo = _host(j_offset, np.int64)
+    xi_, pxi = _host(xi, np.float32, (3,))
+    mj_, pmj = _host(mj, np.float32)
+    xj_, pxj = _host(xj, np.float32, (3,))
+    n_groups = io.shape[0] - 1
+    if jo.shape[0] != n_groups + 1 or xi_.shape[0] != io[-1] or mj_.shape[0] != jo[-1] or xj_.shape[0] != jo[-1]:
+        raise ValueError("calc_batch: offsets and arrays disagree")
+    acc = np.empty((xi_.shape[0], 3), np.float32)
+    pot = np.empty(xi_.shape[0], np.float32)
+    _check("nbk_calc_batch", load().nbk_calc_batch(ctx, n_groups, pio, pxi, pjo, pmj, pxj, float(eps2), flags,
+                                                   acc.ctypes.data, pot.ctypes.data), ctx)
+    return acc, pot
+
+
+def nbk_calc_batch_dev(ctx, i_offset, xi, j_offset, mj, xj, eps2, flags, acc, pot):
+    """i_offset, j_offset: host int64 arrays; xi, mj, xj, acc, pot: device addresses."""
+    io, pio = _host(i_offset, np.int64)
+    jo, pjo = _host(j_offset, np.int64)
+    _check("nbk_calc_batch_dev", load().nbk_calc_batch_dev(ctx, io.shape[0] - 1, pio, xi or None, pjo, mj or None,
+                                                           xj or None, float(eps2), flags, acc or None, pot or None), ctx)
 
 
 def nbk_get_neighbours(ctx, n_i):

@@ -249,6 +249,45 @@ cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n
                            float* py, float* pz, float* pm, float* pvx, float* pvy, float* pvz,
                            const InlineJ* upd, cudaStream_t st);
 
+// ---- batched acc + pot calls: many (i-group, j-list) problems in one launch ----
+struct BatchArgs {
+    const float* x;            // packed j-lists, SoA, each list padded to a multiple of tj (m = 0 far away)
+    const float* y;
+    const float* z;
+    const float* m;
+    const float* xi;           // [n_i_total][3] i-positions, groups back to back (caller's order)
+    const long long* pair_prefix;  // [n_groups + 1] pairs (i-tiles x j-tiles) before group g
+    const long long* seg_prefix;   // [n_groups + 1] i-tiles before group g
+    const long long* j_off;        // [n_groups] start of the group's padded list in x, y, z, m
+    const int* i_off;              // [n_groups] start / end of the group's i-particles in xi and the
+    const int* i_end;              //            outputs (the caller's offsets)
+    const int* njt;                // [n_groups] j-tiles of the group's list
+    float* partial;                // [seg + cta][ti][4]
+    float* acc;                    // [n_i_total][3]  (reduce)
+    float* pot;                    // [n_i_total]     (reduce)
+    int n_groups;                  // non-empty groups only
+    int ti, tj, wj;
+    long long P;
+    long long n_seg;
+    int G;
+    float eps2;
+};
+struct BatchPackArgs {
+    const float* mj;               // caller's lists: [n_j_total], [n_j_total][3]
+    const float* xj;
+    const long long* src_off;      // [n_groups] start and length of the caller's list of each group
+    const long long* src_len;
+    const long long* dst_off;      // [n_groups + 1] padded offsets
+    float* x; float* y; float* z; float* m;
+    int n_groups;
+    long long n_padded;
+};
+cudaError_t launch_batch_pack(const BatchPackArgs& a, cudaStream_t s);
+cudaError_t batch_prepare();
+size_t batch_smem_bytes();
+cudaError_t launch_batch(const BatchArgs& a, bool eps0, cudaStream_t s);
+cudaError_t launch_batch_reduce(const BatchArgs& a, cudaStream_t s);
+
 // device-resident integrator kernels (one block step = begin, predict+select, force, reduce, correct)
 cudaError_t launch_hd_begin(DynHeader* h, cudaStream_t st);
 cudaError_t launch_hd_predict(const RawJ& raw, DynHeader* h, const HermiteState& hs, long long n_pad,

@@ -542,3 +542,78 @@ def test_every_kernel_form_flag_and_block_size(gpu, c_oracle, n_i):
                 if flags & nb.NBK_NN:
                     nn, r2 = nb.nbk_get_neighbours(ctx, n_i)
                     _check_nn(nn, r2, ref_nn, ref_r2, gx, idx, what=f"nn n_i={n_i} variant={variant:#x}")
+
+
+# ----------------------------------------------------------------------------- batched acc + pot calls
+def _batch_problem(seed, n_groups, ni_range, nj_range, with_empty=False):
+    """Treecode-shaped synthetic batch: per group a clump of i-particles and an interaction list of
+    'cells' (masses, positions) around it; the group's own particles are part of their list."""
+    rng = np.random.default_rng(seed)
+    ni = rng.integers(ni_range[0], ni_range[1] + 1, n_groups)
+    nj = rng.integers(nj_range[0], nj_range[1] + 1, n_groups)
+    if with_empty:
+        ni[3] = 0
+        nj[5] = 0
+        nj[6] = 1
+    io = np.concatenate([[0], np.cumsum(ni)]).astype(np.int64)
+    jo = np.concatenate([[0], np.cumsum(nj)]).astype(np.int64)
+    xi = np.empty((io[-1], 3), np.float32)
+    xj = np.empty((jo[-1], 3), np.float32)
+    mj = rng.uniform(0.5, 2.0, jo[-1]).astype(np.float32) / 1000.0
+    for g in range(n_groups):
+        centre = rng.standard_normal(3)
+        xi[io[g]:io[g + 1]] = (centre + 0.05 * rng.standard_normal((ni[g], 3))).astype(np.float32)
+        lst = centre + rng.standard_normal((nj[g], 3)) * rng.uniform(0.05, 2.0, (nj[g], 1))
+        k = min(ni[g], nj[g])
+        lst[:k] = xi[io[g]:io[g] + k]          # own particles sit in their own list
+        xj[jo[g]:jo[g + 1]] = lst.astype(np.float32)
+    return io, jo, xi, mj, xj
+
+
+def _batch_oracle(c_oracle, io, jo, xi, mj, xj, eps):
+    acc = np.zeros((io[-1], 3))
+    pot = np.zeros(io[-1])
+    for g in range(io.shape[0] - 1):
+        a, b, c, d = io[g], io[g + 1], jo[g], jo[g + 1]
+        if b > a and d > c:
+            ra, _, rp = c_oracle.force(mj[c:d], xj[c:d], None, eps, i_index=np.full(b - a, -1),
+                                       want_jerk=False, xi=xi[a:b])
+            acc[a:b], pot[a:b] = ra, rp
+    return acc, pot
+
+
+@pytest.mark.parametrize("shape", [dict(n_groups=40, ni_range=(1, 90), nj_range=(1, 700)),
+                                   dict(n_groups=300, ni_range=(8, 300), nj_range=(100, 2500)),
+                                   dict(n_groups=7, ni_range=(400, 1500), nj_range=(3000, 9000)),
+                                   dict(n_groups=1, ni_range=(5, 5), nj_range=(3, 3))])
+@pytest.mark.parametrize("eps", [EPS, 0.0])
+def test_batched_calls_match_oracle(gpu, c_oracle, shape, eps):
+    """many (i-group, interaction list) problems of irregular sizes in one launch,
+    acc + pot only, against the oracle group by group (external i-particles, nothing excluded by
+    index; eps = 0 skips the zero-distance own entries).  Includes empty groups and empty lists."""
+    io, jo, xi, mj, xj = _batch_problem(5 + shape["n_groups"], with_empty=shape["n_groups"] >= 40, **shape)
+    racc, rpot = _batch_oracle(c_oracle, io, jo, xi, mj, xj, eps)
+    with Ctx(64) as ctx:
+        flags = nb.NBK_POT | (nb.NBK_EPS0 if eps == 0.0 else 0)
+        outs = [nb.nbk_calc_batch(ctx, io, xi, jo, mj, xj, np.float32(eps) ** 2, flags) for _ in range(2)]
+        with pytest.raises(nb.NbkError):
+            nb.nbk_calc_batch(ctx, io, xi, jo, mj, xj, 0.0, nb.NBK_JERK)
+    acc, pot = outs[0]
+    assert np.array_equal(acc, outs[1][0]) and np.array_equal(pot, outs[1][1])
+    live = np.abs(rpot) > 0
+    assert np.all(acc[~live] == 0) and np.all(pot[~live] == 0)
+    assert_parity((acc[live], None, pot[live]), (racc[live], None, rpot[live]), jerk=False, what=f"batch {shape}")
+
+
+def test_batched_calls_device_pointers(gpu, c_oracle):
+    torch = gpu
+    io, jo, xi, mj, xj = _batch_problem(77, 120, (16, 200), (200, 1500))
+    racc, rpot = _batch_oracle(c_oracle, io, jo, xi, mj, xj, EPS)
+    dxi, dmj, dxj = (torch.from_numpy(t).cuda() for t in (xi, mj, xj))
+    acc = torch.empty((io[-1], 3), dtype=torch.float32, device="cuda")
+    pot = torch.empty(io[-1], dtype=torch.float32, device="cuda")
+    torch.cuda.synchronize()
+    with Ctx(64) as ctx:
+        nb.nbk_calc_batch_dev(ctx, io, dxi.data_ptr(), jo, dmj.data_ptr(), dxj.data_ptr(), np.float32(EPS) ** 2,
+                              nb.NBK_POT, acc.data_ptr(), pot.data_ptr())
+    assert_parity((acc.cpu().numpy(), None, pot.cpu().numpy()), (racc, None, rpot), jerk=False, what="batch dev")
