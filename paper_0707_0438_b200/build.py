@@ -16,8 +16,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 INCLUDE = os.path.join(ROOT, "include")
-SOURCES = ["nbk_kernels.cu", "nbk_api.cu", "nbk_hermite.cpp"]
-HEADERS = [os.path.join(CSRC, "nbk_kernels.cuh"), os.path.join(INCLUDE, "nbk.h")]
+SOURCES = ["nbk_kernels.cu", "nbk_api.cu", "nbk_hermite_dev.cu", "nbk_batch.cu", "nbk_hermite.cpp"]
+HEADERS = [os.path.join(CSRC, "nbk_kernels.cuh"), os.path.join(CSRC, "nbk_ctx.cuh"), os.path.join(INCLUDE, "nbk.h")]
 LIB = os.path.join(HERE, "libnbk.so")
 
 NVCC_FLAGS = [

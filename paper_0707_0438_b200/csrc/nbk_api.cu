@@ -12,89 +12,11 @@
 #include <new>
 #include <vector>
 
-#include "../../include/nbk.h"
-#include "nbk_kernels.cuh"
+#include "nbk_ctx.cuh"
 
 using namespace nbk;
 
-namespace {
-
-inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
-
-struct DeviceGuard {  // make the context's device current for the call, restore on exit
-    int prev = -1;
-    bool ok = true;
-    explicit DeviceGuard(int dev) {
-        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
-        if (prev != dev) ok = cudaSetDevice(dev) == cudaSuccess;
-    }
-    ~DeviceGuard() {
-        int cur = -1;
-        if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
-    }
-};
-
-}  // namespace
-
-struct nbk_ctx {
-    int device = 0;
-    cudaStream_t stream = nullptr;
-    bool own_stream = false;
-    long long n_max = 0, ni_max = 0, n_cap = 0;
-    int num_sms = 0;
-
-    RawJ raw{};
-    float* pred = nullptr;  // 7 arrays of n_cap floats: x y z m vx vy vz
-    double t = 0.0;
-    bool pred_valid = false;
-    long long pred_nj = -1;
-
-    int32_t* d_iidx = nullptr;
-    float* d_xi = nullptr;
-    float* d_vi = nullptr;
-    float* d_partial = nullptr;
-    size_t partial_bytes = 0;
-    float* d_result = nullptr;  // acc[3 n_i] | jerk[3 n_i] | pot[n_i] of the last call
-    float* h_result = nullptr;  // pinned, mapped into the device address space
-    float* h_result_dev = nullptr;  // device view of h_result
-    unsigned* d_counter = nullptr;  // arrival counter of the fused small-block tail
-    float2* d_nn_partial = nullptr; // nearest neighbour: per partial row (smallest s, its j-tile)
-    float* d_nn_best = nullptr;     // [ni_max]
-    int32_t* d_nn_tile = nullptr;   // [ni_max]
-    int32_t* d_nn_index = nullptr;  // [ni_max] result
-    float* d_nn_r2 = nullptr;       // [ni_max] result
-    bool last_nn = false;           // the last firsthalf asked for nearest neighbours
-    unsigned char* d_batch = nullptr;  // batched calls: one growable device arena
-    size_t batch_bytes = 0;
-    bool batch_ready = false;
-    HermiteState hs{};              // device-resident integrator state (allocated on first use)
-    long long hs_cap = 0;
-    DynHeader* d_hdr = nullptr;
-    DynHeader* h_hdr = nullptr;     // pinned
-    bool host_has_result = false;   // the last firsthalf wrote h_result itself (no D2H needed)
-    InlineJ pending;                // a small set_j not yet on the device (pending.n == 0: none)
-
-    unsigned char* h_stage = nullptr;  // pinned staging for set_j
-    unsigned char* d_stage = nullptr;
-    size_t stage_bytes = 0;
-    cudaEvent_t stage_free = nullptr;  // recorded after the H2D that reads h_stage
-    unsigned char* h_istage = nullptr;  // pinned staging for i_index / xi / vi
-    cudaEvent_t istage_free = nullptr;
-
-    long long last_ni = -1;
-    bool in_flight = false;
-    int variant_scalar = 0;
-    int force_I = 0;
-    bool fused_ok = true;  // nbk_set_variant bit 8 switches the one-launch small-block path off
-    int last_cuda = 0;
-    long long last_launch[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-
-    bool timing = false;
-    cudaEvent_t ev[4][2];
-    bool ev_used[4] = {false, false, false, false};
-};
-
-namespace {
+namespace nbk {
 
 int cuda_fail(nbk_ctx* c, cudaError_t e) {
     c->last_cuda = static_cast<int>(e);
@@ -102,31 +24,26 @@ int cuda_fail(nbk_ctx* c, cudaError_t e) {
     return NBK_ECUDA;
 }
 
-#define NBK_CUDA(c, call)                                   \
-    do {                                                    \
-        cudaError_t e__ = (call);                           \
-        if (e__ != cudaSuccess) return cuda_fail((c), e__); \
-    } while (0)
-
-struct TimeScope {  // CUDA events around one kernel on the context's stream
-    nbk_ctx* c;
-    int slot;
-    TimeScope(nbk_ctx* c_, int slot_) : c(c_), slot(slot_) {
-        if (c->timing) { cudaEventRecord(c->ev[slot][0], c->stream); c->ev_used[slot] = true; }
-    }
-    ~TimeScope() {
-        if (c->timing) cudaEventRecord(c->ev[slot][1], c->stream);
-    }
-};
-
-float* pred_arr(const nbk_ctx* c, int k) { return c->pred + static_cast<size_t>(k) * c->n_cap; }
-
 JPred jpred_of(const nbk_ctx* c) {
     JPred j;
     j.x = pred_arr(c, 0); j.y = pred_arr(c, 1); j.z = pred_arr(c, 2); j.m = pred_arr(c, 3);
     j.vx = pred_arr(c, 4); j.vy = pred_arr(c, 5); j.vz = pred_arr(c, 6);
     return j;
 }
+
+// A pending small set_j goes to the device on its own (before anything else touches the raw state).
+int flush_pending(nbk_ctx* c) {
+    if (c->pending.n > 0) {
+        TimeScope ts(c, 0);
+        NBK_CUDA(c, launch_scatter_inline(c->pending, c->raw, c->stream));
+        c->pending.n = 0;
+    }
+    return NBK_OK;
+}
+
+}  // namespace nbk
+
+namespace {
 
 void free_all(nbk_ctx* c) {
     cudaFree(c->raw.x); cudaFree(c->raw.v); cudaFree(c->raw.a); cudaFree(c->raw.k);
@@ -151,15 +68,6 @@ void free_all(nbk_ctx* c) {
     (void)cudaGetLastError();
 }
 
-// A pending small set_j goes to the device on its own (before anything else touches the raw state).
-int flush_pending(nbk_ctx* c) {
-    if (c->pending.n > 0) {
-        TimeScope ts(c, 0);
-        NBK_CUDA(c, launch_scatter_inline(c->pending, c->raw, c->stream));
-        c->pending.n = 0;
-    }
-    return NBK_OK;
-}
 
 int do_predict(nbk_ctx* c, long long n_j) {
     const long long n_pad = round_up(n_j, kTileJMax);
@@ -713,345 +621,6 @@ int nbk_get_neighbours_dev(nbk_ctx* c, int64_t n_i, int32_t* nn_index, float* nn
     return NBK_OK;
 }
 
-// ---- a8 on the device: the whole block-step loop without host round trips ----
-int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, double* v, double eps,
-                           double t_end, double eta, double dt_max, nbk_hermite_stats* stats) {
-    if (!c || n < 1 || !m || !x || !v || !(eps >= 0.0) || !(t_end >= 0.0) || !(eta > 0.0) ||
-        !(dt_max > 0.0) || n > INT32_MAX)
-        return NBK_EINVAL;
-    if (n > c->n_max || n > c->ni_max) return NBK_ERANGE;
-    int e0;
-    std::frexp(dt_max, &e0);
-    int kmin = -(e0 - 1);            // dt_max rounded down to a power of two
-    if (kmin < -10) kmin = -10;
-    if (kmin < 0 || kmin > kMaxLevel) return NBK_EINVAL;   // dt_max in (2^-48, 1]... 2^0
-    const double dtm = std::ldexp(1.0, -kmin);
-    if (t_end > 2047.0 || std::fmod(t_end, dtm) != 0.0) return NBK_EINVAL;
-    DeviceGuard g(c->device);
-    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
-    const auto wall0 = std::chrono::steady_clock::now();
-    const size_t N = static_cast<size_t>(n);
-    const float eps2 = static_cast<float>(eps * eps);
-    const uint32_t flags = NBK_JERK | NBK_POT;
-    int rc;
-
-    if (c->hs_cap < n) {
-        cudaFree(c->hs.x); cudaFree(c->hs.v); cudaFree(c->hs.a); cudaFree(c->hs.j);
-        cudaFree(c->hs.level); cudaFree(c->hs.act); cudaFree(c->hs.bc_ge);
-        c->hs = HermiteState{};
-        c->hs_cap = 0;
-        NBK_CUDA(c, cudaMalloc(&c->hs.x, sizeof(double) * 3 * N));
-        NBK_CUDA(c, cudaMalloc(&c->hs.v, sizeof(double) * 3 * N));
-        NBK_CUDA(c, cudaMalloc(&c->hs.a, sizeof(double) * 3 * N));
-        NBK_CUDA(c, cudaMalloc(&c->hs.j, sizeof(double) * 3 * N));
-        NBK_CUDA(c, cudaMalloc(&c->hs.level, sizeof(int) * N));
-        NBK_CUDA(c, cudaMalloc(&c->hs.act, sizeof(int32_t) * N));
-        NBK_CUDA(c, cudaMalloc(&c->hs.bc_ge, sizeof(int) * (kMaxLevel + 1) * ((N + 255) / 256)));
-        c->hs_cap = n;
-    }
-    if (!c->d_hdr) NBK_CUDA(c, cudaMalloc(&c->d_hdr, sizeof(DynHeader)));
-    if (!c->h_hdr) NBK_CUDA(c, cudaMallocHost(&c->h_hdr, sizeof(DynHeader)));
-
-    // t = 0 through the ordinary entry points: forces on everybody, first steps (reading R15)
-    std::vector<float> fa(3 * N), fj(3 * N);
-    std::vector<double> a(3 * N), jk(3 * N), tl(N, 0.0);
-    std::vector<int> lev(N);
-    if ((rc = nbk_set_j_particles_f64(c, n, nullptr, nullptr, m, x, v, nullptr, nullptr)) != NBK_OK) return rc;
-    if ((rc = nbk_set_ti(c, 0.0)) != NBK_OK) return rc;
-    if ((rc = nbk_calc_firsthalf(c, n, n, nullptr, nullptr, nullptr, eps2, flags)) != NBK_OK) return rc;
-    if ((rc = nbk_calc_lasthalf(c, n, fa.data(), fj.data(), nullptr)) != NBK_OK) return rc;
-    DynHeader& H = *c->h_hdr;
-    std::memset(&H, 0, sizeof(H));
-    for (size_t i = 0; i < N; ++i) {
-        double na = 0.0, nj = 0.0;
-        for (int q = 0; q < 3; ++q) {
-            a[3 * i + q] = fa[3 * i + q];
-            jk[3 * i + q] = fj[3 * i + q];
-            na += a[3 * i + q] * a[3 * i + q];
-            nj += jk[3 * i + q] * jk[3 * i + q];
-        }
-        na = std::sqrt(na); nj = std::sqrt(nj);
-        double want = dtm;
-        if (nj > 0.0 && na > 0.0) want = std::fmin(0.25 * eta * na / nj, dtm);
-        int k = kMaxLevel;
-        if (want > 0.0) {
-            int e;
-            std::frexp(want, &e);
-            k = -(e - 1);
-            if (k < kmin) k = kmin;
-            if (k > kMaxLevel) k = kMaxLevel;
-        }
-        lev[i] = k;
-        H.level_count[k] += 1;
-    }
-    const int nblk = static_cast<int>((N + 255) / 256);
-    c->hs.nblk = nblk;
-    std::vector<int> bc(static_cast<size_t>(kMaxLevel + 1) * nblk, 0);
-    for (size_t i = 0; i < N; ++i)
-        for (int l = 0; l <= lev[i]; ++l) bc[static_cast<size_t>(l) * nblk + (i >> 8)] += 1;
-    if ((rc = nbk_set_j_particles_f64(c, n, nullptr, tl.data(), m, x, v, a.data(), jk.data())) != NBK_OK) return rc;
-    if ((rc = flush_pending(c)) != NBK_OK) return rc;
-    H.T_now = 0;
-    H.T_end = static_cast<long long>(std::ldexp(t_end, kTickLog2));
-    H.kmin = kmin;
-    H.n = static_cast<int>(n);
-    H.num_sms = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
-    H.max_partial_floats = c->partial_bytes / sizeof(float);
-    H.eta = eta;
-    H.interactions = n * n;
-    NBK_CUDA(c, cudaMemcpyAsync(c->hs.x, x, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
-    NBK_CUDA(c, cudaMemcpyAsync(c->hs.v, v, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
-    NBK_CUDA(c, cudaMemcpyAsync(c->hs.a, a.data(), sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
-    NBK_CUDA(c, cudaMemcpyAsync(c->hs.j, jk.data(), sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
-    NBK_CUDA(c, cudaMemcpyAsync(c->hs.level, lev.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream));
-    NBK_CUDA(c, cudaMemcpyAsync(c->hs.bc_ge, bc.data(), sizeof(int) * bc.size(), cudaMemcpyHostToDevice, c->stream));
-    NBK_CUDA(c, cudaMemcpyAsync(c->d_hdr, &H, sizeof(H), cudaMemcpyHostToDevice, c->stream));
-    NBK_CUDA(c, cudaStreamSynchronize(c->stream));   // the host vectors above may go away
-
-    // one block step = begin, predict + select, force (+ reduce), correct; enqueued in batches with
-    // no host synchronisation inside a batch; steps past t_end return at once (done flag)
-    Variant vv{1, true, eps2 == 0.f, true, false};
-    const long long n_pad = round_up(n, kTileJMax);
-    const size_t ni_max = static_cast<size_t>(c->ni_max);
-    ForceArgs f;
-    std::memset(&f, 0, sizeof(f));
-    f.j = jpred_of(c);
-    f.i_index = c->hs.act;
-    f.partial = c->d_partial;
-    f.eps2 = eps2;
-    f.d.n_j = static_cast<int>(n);
-    f.tail.counter = c->d_counter;
-    f.tail.acc = c->d_result;
-    f.tail.jerk = c->d_result + 3 * ni_max;
-    f.tail.pot = c->d_result + 6 * ni_max;
-    f.dyn = c->d_hdr;
-    f.d.G = H.num_sms;   // grid: one CTA per SM; CTAs beyond the plan's G return
-    ReduceArgs r;
-    std::memset(&r, 0, sizeof(r));
-    r.partial = c->d_partial;
-    r.acc = f.tail.acc; r.jerk = f.tail.jerk; r.pot = f.tail.pot;
-    r.dyn = c->d_hdr;
-    r.n_j = static_cast<int>(n);
-    // the five launches of a block step are captured once into a CUDA graph and replayed
-    const int kBatch = 256;
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t gexec = nullptr;
-    auto enqueue_step = [&]() -> cudaError_t {
-        cudaError_t e;
-        if ((e = launch_hd_begin(c->d_hdr, c->stream)) != cudaSuccess) return e;
-        if ((e = launch_hd_predict(c->raw, c->d_hdr, c->hs, n_pad, pred_arr(c, 0), pred_arr(c, 1),
-                                   pred_arr(c, 2), pred_arr(c, 3), pred_arr(c, 4), pred_arr(c, 5),
-                                   pred_arr(c, 6), c->stream)) != cudaSuccess) return e;
-        if ((e = launch_force(vv, f, c->stream)) != cudaSuccess) return e;
-        if ((e = launch_reduce_dyn(vv, r, static_cast<int>(n), c->stream)) != cudaSuccess) return e;
-        return launch_hd_correct(c->raw, c->d_hdr, c->hs, f.tail.acc, f.tail.jerk,
-                                 static_cast<int>(n), c->stream);
-    };
-    NBK_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
-    cudaError_t ce = enqueue_step();
-    cudaError_t ce2 = cudaStreamEndCapture(c->stream, &graph);
-    if (ce != cudaSuccess || ce2 != cudaSuccess) {
-        if (graph) cudaGraphDestroy(graph);
-        return cuda_fail(c, ce != cudaSuccess ? ce : ce2);
-    }
-    ce = cudaGraphInstantiate(&gexec, graph, 0);
-    if (ce != cudaSuccess) { cudaGraphDestroy(graph); return cuda_fail(c, ce); }
-    for (;;) {
-        for (int s = 0; s < kBatch && ce == cudaSuccess; ++s) ce = cudaGraphLaunch(gexec, c->stream);
-        if (ce == cudaSuccess)
-            ce = cudaMemcpyAsync(c->h_hdr, c->d_hdr, sizeof(DynHeader), cudaMemcpyDeviceToHost, c->stream);
-        if (ce == cudaSuccess) ce = cudaStreamSynchronize(c->stream);
-        if (ce != cudaSuccess || c->h_hdr->done) break;
-    }
-    cudaGraphExecDestroy(gexec);
-    cudaGraphDestroy(graph);
-    if (ce != cudaSuccess) return cuda_fail(c, ce);
-    NBK_CUDA(c, cudaMemcpyAsync(x, c->hs.x, sizeof(double) * 3 * N, cudaMemcpyDeviceToHost, c->stream));
-    NBK_CUDA(c, cudaMemcpyAsync(v, c->hs.v, sizeof(double) * 3 * N, cudaMemcpyDeviceToHost, c->stream));
-    NBK_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->pred_valid = false;
-    c->in_flight = false;
-    if (stats) {
-        std::memset(stats, 0, sizeof(*stats));
-        stats->block_steps = c->h_hdr->block_steps;
-        stats->particle_steps = c->h_hdr->particle_steps;
-        stats->interactions = c->h_hdr->interactions;
-        stats->t_reached = std::ldexp(static_cast<double>(c->h_hdr->T_now), -kTickLog2);
-        for (int b = 0; b < 32; ++b) stats->ni_histogram[b] = c->h_hdr->hist[b];
-        stats->wall_seconds =
-            std::chrono::duration<double>(std::chrono::steady_clock::now() - wall0).count();
-        stats->gpu_call_seconds = stats->wall_seconds;
-    }
-    return NBK_OK;
-}
-
-// ---- batched acc + pot calls -------------------------------------------------
-namespace {
-
-int batch_impl(nbk_ctx* c, int64_t n_groups, const int64_t* i_offset, const float* xi,
-               const int64_t* j_offset, const float* mj, const float* xj, float eps2, uint32_t flags,
-               float* acc, float* pot, bool dev) {
-    if (!c || n_groups < 0 || !(eps2 >= 0.f) || (flags & (NBK_JERK | NBK_NN))) return NBK_EINVAL;
-    if (n_groups == 0) return NBK_OK;
-    if (!i_offset || !j_offset || i_offset[0] != 0 || j_offset[0] != 0) return NBK_EINVAL;
-    for (int64_t g = 0; g < n_groups; ++g)
-        if (i_offset[g + 1] < i_offset[g] || j_offset[g + 1] < j_offset[g]) return NBK_EINVAL;
-    const int64_t ni_tot = i_offset[n_groups], nj_tot = j_offset[n_groups];
-    if (ni_tot > INT32_MAX || n_groups > INT32_MAX) return NBK_ERANGE;
-    if (ni_tot == 0) return NBK_OK;
-    if (!xi || !acc || !pot || (nj_tot > 0 && (!mj || !xj))) return NBK_EINVAL;
-    DeviceGuard g(c->device);
-    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
-    if (!c->batch_ready) {
-        NBK_CUDA(c, batch_prepare());
-        c->batch_ready = true;
-    }
-    // launch form from the mean group size: the i-tile is the power of two >= mean n_i in [32, 512];
-    // the 16 warps that do not fit the i-tile split the j-tiles (wj)
-    std::vector<int> keep;
-    int64_t sum_ni = 0;
-    for (int64_t q = 0; q < n_groups; ++q)
-        if (i_offset[q + 1] > i_offset[q] && j_offset[q + 1] > j_offset[q]) {
-            keep.push_back(static_cast<int>(q));
-            sum_ni += i_offset[q + 1] - i_offset[q];
-        }
-    const size_t ni = static_cast<size_t>(ni_tot);
-    float* d_acc = acc;
-    float* d_pot = pot;
-    const int ng = static_cast<int>(keep.size());
-    int ti = 32;
-    if (ng > 0) while (ti < 512 && ti < sum_ni / ng) ti *= 2;
-    const int wj = 512 / ti, tj = 128;
-    std::vector<long long> pair_prefix(ng + 1, 0), seg_prefix(ng + 1, 0), joff(ng + 1, 0), src_off(ng + 1, 0);
-    std::vector<int> ioff(ng + 1, 0), njt(ng > 0 ? ng : 1, 0);
-    for (int q = 0; q < ng; ++q) {
-        const int64_t gg = keep[q];
-        const long long n_i = i_offset[gg + 1] - i_offset[gg], n_j = j_offset[gg + 1] - j_offset[gg];
-        const long long nit = (n_i + ti - 1) / ti, nt = (n_j + tj - 1) / tj;
-        njt[q] = static_cast<int>(nt);
-        pair_prefix[q + 1] = pair_prefix[q] + nit * nt;
-        seg_prefix[q + 1] = seg_prefix[q] + nit;
-        joff[q + 1] = joff[q] + nt * tj;
-    }
-    const long long P = pair_prefix[ng], n_seg = seg_prefix[ng], n_padded = joff[ng];
-    const int gmax = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
-    const int G = static_cast<int>(P < gmax ? P : gmax);
-    // arena: [x y z m | descriptors | partial | (host entry: xi, mj, xj, acc, pot)]
-    size_t off = 0;
-    auto take = [&](size_t bytes) { const size_t at = off; off += (bytes + 255) & ~static_cast<size_t>(255); return at; };
-    const size_t o_x = take(4 * sizeof(float) * n_padded);
-    const size_t o_pp = take(sizeof(long long) * (ng + 1)), o_sp = take(sizeof(long long) * (ng + 1));
-    const size_t o_jo = take(sizeof(long long) * (ng + 1)), o_so = take(sizeof(long long) * (ng + 1));
-    const size_t o_do = take(sizeof(long long) * (ng + 1));
-    const size_t o_io = take(sizeof(int) * (ng + 1)), o_nt = take(sizeof(int) * (ng + 1));
-    const size_t o_ie = take(sizeof(int) * (ng + 1)), o_sl = take(sizeof(long long) * (ng + 1));
-    const size_t o_part = take(sizeof(float) * 4 * ti * static_cast<size_t>(n_seg + G));
-    size_t o_xi = 0, o_mj = 0, o_xj = 0, o_acc = 0, o_pot = 0;
-    if (!dev) {
-        o_xi = take(sizeof(float) * 3 * ni);
-        o_mj = take(sizeof(float) * nj_tot);
-        o_xj = take(sizeof(float) * 3 * nj_tot);
-        o_acc = take(sizeof(float) * 3 * ni);
-        o_pot = take(sizeof(float) * ni);
-    }
-    if (off > c->batch_bytes) {
-        NBK_CUDA(c, cudaStreamSynchronize(c->stream));
-        cudaFree(c->d_batch);
-        c->d_batch = nullptr;
-        c->batch_bytes = 0;
-        NBK_CUDA(c, cudaMalloc(&c->d_batch, off + off / 4));
-        c->batch_bytes = off + off / 4;
-    }
-    unsigned char* B = c->d_batch;
-    // descriptors of the non-empty groups: i offsets are the caller's (outputs keep the caller's order)
-    std::vector<long long> src_len(ng > 0 ? ng : 1, 0);
-    for (int q = 0; q < ng; ++q) {
-        ioff[q] = static_cast<int>(i_offset[keep[q]]);
-        src_off[q] = j_offset[keep[q]];
-        src_len[q] = j_offset[keep[q] + 1] - j_offset[keep[q]];
-    }
-    std::vector<int> iend(ng > 0 ? ng : 1);
-    for (int q = 0; q < ng; ++q) iend[q] = static_cast<int>(i_offset[keep[q] + 1]);
-    if (ng > 0) src_off[ng] = j_offset[keep[ng - 1] + 1];
-    if (!dev) {
-        NBK_CUDA(c, cudaMemcpyAsync(B + o_xi, xi, sizeof(float) * 3 * ni, cudaMemcpyHostToDevice, c->stream));
-        if (nj_tot > 0) {
-            NBK_CUDA(c, cudaMemcpyAsync(B + o_mj, mj, sizeof(float) * nj_tot, cudaMemcpyHostToDevice, c->stream));
-            NBK_CUDA(c, cudaMemcpyAsync(B + o_xj, xj, sizeof(float) * 3 * nj_tot, cudaMemcpyHostToDevice, c->stream));
-        }
-        d_acc = reinterpret_cast<float*>(B + o_acc);
-        d_pot = reinterpret_cast<float*>(B + o_pot);
-    }
-    NBK_CUDA(c, cudaMemsetAsync(d_acc, 0, sizeof(float) * 3 * ni, c->stream));
-    NBK_CUDA(c, cudaMemsetAsync(d_pot, 0, sizeof(float) * ni, c->stream));
-    if (ng > 0) {
-        // pageable host vectors: these copies complete before the call returns to the vectors' scope end
-        NBK_CUDA(c, cudaMemcpyAsync(B + o_pp, pair_prefix.data(), sizeof(long long) * (ng + 1), cudaMemcpyHostToDevice, c->stream));
-        NBK_CUDA(c, cudaMemcpyAsync(B + o_sp, seg_prefix.data(), sizeof(long long) * (ng + 1), cudaMemcpyHostToDevice, c->stream));
-        NBK_CUDA(c, cudaMemcpyAsync(B + o_jo, joff.data(), sizeof(long long) * (ng + 1), cudaMemcpyHostToDevice, c->stream));
-        NBK_CUDA(c, cudaMemcpyAsync(B + o_so, src_off.data(), sizeof(long long) * (ng + 1), cudaMemcpyHostToDevice, c->stream));
-        NBK_CUDA(c, cudaMemcpyAsync(B + o_io, ioff.data(), sizeof(int) * (ng + 1), cudaMemcpyHostToDevice, c->stream));
-        NBK_CUDA(c, cudaMemcpyAsync(B + o_nt, njt.data(), sizeof(int) * ng, cudaMemcpyHostToDevice, c->stream));
-        NBK_CUDA(c, cudaMemcpyAsync(B + o_ie, iend.data(), sizeof(int) * ng, cudaMemcpyHostToDevice, c->stream));
-        NBK_CUDA(c, cudaMemcpyAsync(B + o_sl, src_len.data(), sizeof(long long) * ng, cudaMemcpyHostToDevice, c->stream));
-        BatchPackArgs pk;
-        pk.mj = dev ? mj : reinterpret_cast<const float*>(B + o_mj);
-        pk.xj = dev ? xj : reinterpret_cast<const float*>(B + o_xj);
-        pk.src_off = reinterpret_cast<const long long*>(B + o_so);
-        pk.dst_off = reinterpret_cast<const long long*>(B + o_jo);
-        pk.src_len = reinterpret_cast<const long long*>(B + o_sl);
-        float* px = reinterpret_cast<float*>(B + o_x);
-        pk.x = px; pk.y = px + n_padded; pk.z = px + 2 * n_padded; pk.m = px + 3 * n_padded;
-        pk.n_groups = ng;
-        pk.n_padded = n_padded;
-        NBK_CUDA(c, launch_batch_pack(pk, c->stream));
-        BatchArgs ba;
-        ba.x = pk.x; ba.y = pk.y; ba.z = pk.z; ba.m = pk.m;
-        ba.xi = dev ? xi : reinterpret_cast<const float*>(B + o_xi);
-        ba.pair_prefix = reinterpret_cast<const long long*>(B + o_pp);
-        ba.seg_prefix = reinterpret_cast<const long long*>(B + o_sp);
-        ba.j_off = reinterpret_cast<const long long*>(B + o_jo);
-        ba.i_off = reinterpret_cast<const int*>(B + o_io);
-        ba.njt = reinterpret_cast<const int*>(B + o_nt);
-        ba.i_end = reinterpret_cast<const int*>(B + o_ie);
-        ba.partial = reinterpret_cast<float*>(B + o_part);
-        ba.acc = d_acc; ba.pot = d_pot;
-        ba.n_groups = ng; ba.ti = ti; ba.tj = tj; ba.wj = wj;
-        ba.P = P; ba.n_seg = n_seg; ba.G = G; ba.eps2 = eps2;
-        {
-            TimeScope ts(c, 2);
-            NBK_CUDA(c, launch_batch(ba, (flags & NBK_EPS0) != 0 || eps2 == 0.f, c->stream));
-        }
-        {
-            TimeScope ts(c, 3);
-            NBK_CUDA(c, launch_batch_reduce(ba, c->stream));
-        }
-        c->last_launch[0] = G; c->last_launch[1] = 512; c->last_launch[2] = 1; c->last_launch[3] = wj;
-        c->last_launch[4] = tj; c->last_launch[5] = c->num_sms;
-        c->last_launch[6] = static_cast<long long>(batch_smem_bytes()); c->last_launch[7] = 3;
-    }
-    if (!dev) {
-        NBK_CUDA(c, cudaMemcpyAsync(acc, d_acc, sizeof(float) * 3 * ni, cudaMemcpyDeviceToHost, c->stream));
-        NBK_CUDA(c, cudaMemcpyAsync(pot, d_pot, sizeof(float) * ni, cudaMemcpyDeviceToHost, c->stream));
-    }
-    // the descriptor vectors live on this stack frame: wait until their copies have been consumed
-    NBK_CUDA(c, cudaStreamSynchronize(c->stream));
-    return NBK_OK;
-}
-
-}  // namespace
-
-int nbk_calc_batch(nbk_ctx* c, int64_t n_groups, const int64_t* i_offset, const float* xi,
-                   const int64_t* j_offset, const float* mj, const float* xj, float eps2,
-                   uint32_t flags, float* acc, float* pot) {
-    return batch_impl(c, n_groups, i_offset, xi, j_offset, mj, xj, eps2, flags, acc, pot, false);
-}
-
-int nbk_calc_batch_dev(nbk_ctx* c, int64_t n_groups, const int64_t* i_offset, const float* xi,
-                       const int64_t* j_offset, const float* mj, const float* xj, float eps2,
-                       uint32_t flags, float* acc, float* pot) {
-    return batch_impl(c, n_groups, i_offset, xi, j_offset, mj, xj, eps2, flags, acc, pot, true);
-}
 
 int nbk_sync(nbk_ctx* c) {
     if (!c) return NBK_EINVAL;

@@ -1,0 +1,191 @@
+// nbk_hermite_dev.cu -- nbk_hermite_evolve_dev: the Hermite block-step loop resident on the device
+// (SURVEY.md 8(f)-1).  Host side only: state upload, CUDA-graph replay of the five launches of a step,
+// termination check; the kernels (hd_*) are in nbk_kernels.cu.
+#include <chrono>
+#include <climits>
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "nbk_ctx.cuh"
+
+using namespace nbk;
+
+namespace {
+inline long long round_up_ll(long long a, long long b) { return (a + b - 1) / b * b; }
+}  // namespace
+
+extern "C" {
+// ---- a8 on the device: the whole block-step loop without host round trips ----
+int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, double* v, double eps,
+                           double t_end, double eta, double dt_max, nbk_hermite_stats* stats) {
+    if (!c || n < 1 || !m || !x || !v || !(eps >= 0.0) || !(t_end >= 0.0) || !(eta > 0.0) ||
+        !(dt_max > 0.0) || n > INT32_MAX)
+        return NBK_EINVAL;
+    if (n > c->n_max || n > c->ni_max) return NBK_ERANGE;
+    int e0;
+    std::frexp(dt_max, &e0);
+    int kmin = -(e0 - 1);            // dt_max rounded down to a power of two
+    if (kmin < -10) kmin = -10;
+    if (kmin < 0 || kmin > kMaxLevel) return NBK_EINVAL;   // dt_max in (2^-48, 1]... 2^0
+    const double dtm = std::ldexp(1.0, -kmin);
+    if (t_end > 2047.0 || std::fmod(t_end, dtm) != 0.0) return NBK_EINVAL;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    const auto wall0 = std::chrono::steady_clock::now();
+    const size_t N = static_cast<size_t>(n);
+    const float eps2 = static_cast<float>(eps * eps);
+    const uint32_t flags = NBK_JERK | NBK_POT;
+    int rc;
+
+    if (c->hs_cap < n) {
+        cudaFree(c->hs.x); cudaFree(c->hs.v); cudaFree(c->hs.a); cudaFree(c->hs.j);
+        cudaFree(c->hs.level); cudaFree(c->hs.act); cudaFree(c->hs.bc_ge);
+        c->hs = HermiteState{};
+        c->hs_cap = 0;
+        NBK_CUDA(c, cudaMalloc(&c->hs.x, sizeof(double) * 3 * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.v, sizeof(double) * 3 * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.a, sizeof(double) * 3 * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.j, sizeof(double) * 3 * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.level, sizeof(int) * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.act, sizeof(int32_t) * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.bc_ge, sizeof(int) * (kMaxLevel + 1) * ((N + 255) / 256)));
+        c->hs_cap = n;
+    }
+    if (!c->d_hdr) NBK_CUDA(c, cudaMalloc(&c->d_hdr, sizeof(DynHeader)));
+    if (!c->h_hdr) NBK_CUDA(c, cudaMallocHost(&c->h_hdr, sizeof(DynHeader)));
+
+    // t = 0 through the ordinary entry points: forces on everybody, first steps (reading R15)
+    std::vector<float> fa(3 * N), fj(3 * N);
+    std::vector<double> a(3 * N), jk(3 * N), tl(N, 0.0);
+    std::vector<int> lev(N);
+    if ((rc = nbk_set_j_particles_f64(c, n, nullptr, nullptr, m, x, v, nullptr, nullptr)) != NBK_OK) return rc;
+    if ((rc = nbk_set_ti(c, 0.0)) != NBK_OK) return rc;
+    if ((rc = nbk_calc_firsthalf(c, n, n, nullptr, nullptr, nullptr, eps2, flags)) != NBK_OK) return rc;
+    if ((rc = nbk_calc_lasthalf(c, n, fa.data(), fj.data(), nullptr)) != NBK_OK) return rc;
+    DynHeader& H = *c->h_hdr;
+    std::memset(&H, 0, sizeof(H));
+    for (size_t i = 0; i < N; ++i) {
+        double na = 0.0, nj = 0.0;
+        for (int q = 0; q < 3; ++q) {
+            a[3 * i + q] = fa[3 * i + q];
+            jk[3 * i + q] = fj[3 * i + q];
+            na += a[3 * i + q] * a[3 * i + q];
+            nj += jk[3 * i + q] * jk[3 * i + q];
+        }
+        na = std::sqrt(na); nj = std::sqrt(nj);
+        double want = dtm;
+        if (nj > 0.0 && na > 0.0) want = std::fmin(0.25 * eta * na / nj, dtm);
+        int k = kMaxLevel;
+        if (want > 0.0) {
+            int e;
+            std::frexp(want, &e);
+            k = -(e - 1);
+            if (k < kmin) k = kmin;
+            if (k > kMaxLevel) k = kMaxLevel;
+        }
+        lev[i] = k;
+        H.level_count[k] += 1;
+    }
+    const int nblk = static_cast<int>((N + 255) / 256);
+    c->hs.nblk = nblk;
+    std::vector<int> bc(static_cast<size_t>(kMaxLevel + 1) * nblk, 0);
+    for (size_t i = 0; i < N; ++i)
+        for (int l = 0; l <= lev[i]; ++l) bc[static_cast<size_t>(l) * nblk + (i >> 8)] += 1;
+    if ((rc = nbk_set_j_particles_f64(c, n, nullptr, tl.data(), m, x, v, a.data(), jk.data())) != NBK_OK) return rc;
+    if ((rc = flush_pending(c)) != NBK_OK) return rc;
+    H.T_now = 0;
+    H.T_end = static_cast<long long>(std::ldexp(t_end, kTickLog2));
+    H.kmin = kmin;
+    H.n = static_cast<int>(n);
+    H.num_sms = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
+    H.max_partial_floats = c->partial_bytes / sizeof(float);
+    H.eta = eta;
+    H.interactions = n * n;
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.x, x, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.v, v, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.a, a.data(), sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.j, jk.data(), sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.level, lev.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.bc_ge, bc.data(), sizeof(int) * bc.size(), cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->d_hdr, &H, sizeof(H), cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaStreamSynchronize(c->stream));   // the host vectors above may go away
+
+    // one block step = begin, predict + select, force (+ reduce), correct; enqueued in batches with
+    // no host synchronisation inside a batch; steps past t_end return at once (done flag)
+    Variant vv{1, true, eps2 == 0.f, true, false};
+    const long long n_pad = round_up_ll(n, kTileJMax);
+    const size_t ni_max = static_cast<size_t>(c->ni_max);
+    ForceArgs f;
+    std::memset(&f, 0, sizeof(f));
+    f.j = jpred_of(c);
+    f.i_index = c->hs.act;
+    f.partial = c->d_partial;
+    f.eps2 = eps2;
+    f.d.n_j = static_cast<int>(n);
+    f.tail.counter = c->d_counter;
+    f.tail.acc = c->d_result;
+    f.tail.jerk = c->d_result + 3 * ni_max;
+    f.tail.pot = c->d_result + 6 * ni_max;
+    f.dyn = c->d_hdr;
+    f.d.G = H.num_sms;   // grid: one CTA per SM; CTAs beyond the plan's G return
+    ReduceArgs r;
+    std::memset(&r, 0, sizeof(r));
+    r.partial = c->d_partial;
+    r.acc = f.tail.acc; r.jerk = f.tail.jerk; r.pot = f.tail.pot;
+    r.dyn = c->d_hdr;
+    r.n_j = static_cast<int>(n);
+    // the five launches of a block step are captured once into a CUDA graph and replayed
+    const int kBatch = 256;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t gexec = nullptr;
+    auto enqueue_step = [&]() -> cudaError_t {
+        cudaError_t e;
+        if ((e = launch_hd_begin(c->d_hdr, c->stream)) != cudaSuccess) return e;
+        if ((e = launch_hd_predict(c->raw, c->d_hdr, c->hs, n_pad, pred_arr(c, 0), pred_arr(c, 1),
+                                   pred_arr(c, 2), pred_arr(c, 3), pred_arr(c, 4), pred_arr(c, 5),
+                                   pred_arr(c, 6), c->stream)) != cudaSuccess) return e;
+        if ((e = launch_force(vv, f, c->stream)) != cudaSuccess) return e;
+        if ((e = launch_reduce_dyn(vv, r, static_cast<int>(n), c->stream)) != cudaSuccess) return e;
+        return launch_hd_correct(c->raw, c->d_hdr, c->hs, f.tail.acc, f.tail.jerk,
+                                 static_cast<int>(n), c->stream);
+    };
+    NBK_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
+    cudaError_t ce = enqueue_step();
+    cudaError_t ce2 = cudaStreamEndCapture(c->stream, &graph);
+    if (ce != cudaSuccess || ce2 != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        return cuda_fail(c, ce != cudaSuccess ? ce : ce2);
+    }
+    ce = cudaGraphInstantiate(&gexec, graph, 0);
+    if (ce != cudaSuccess) { cudaGraphDestroy(graph); return cuda_fail(c, ce); }
+    for (;;) {
+        for (int s = 0; s < kBatch && ce == cudaSuccess; ++s) ce = cudaGraphLaunch(gexec, c->stream);
+        if (ce == cudaSuccess)
+            ce = cudaMemcpyAsync(c->h_hdr, c->d_hdr, sizeof(DynHeader), cudaMemcpyDeviceToHost, c->stream);
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(c->stream);
+        if (ce != cudaSuccess || c->h_hdr->done) break;
+    }
+    cudaGraphExecDestroy(gexec);
+    cudaGraphDestroy(graph);
+    if (ce != cudaSuccess) return cuda_fail(c, ce);
+    NBK_CUDA(c, cudaMemcpyAsync(x, c->hs.x, sizeof(double) * 3 * N, cudaMemcpyDeviceToHost, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(v, c->hs.v, sizeof(double) * 3 * N, cudaMemcpyDeviceToHost, c->stream));
+    NBK_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->pred_valid = false;
+    c->in_flight = false;
+    if (stats) {
+        std::memset(stats, 0, sizeof(*stats));
+        stats->block_steps = c->h_hdr->block_steps;
+        stats->particle_steps = c->h_hdr->particle_steps;
+        stats->interactions = c->h_hdr->interactions;
+        stats->t_reached = std::ldexp(static_cast<double>(c->h_hdr->T_now), -kTickLog2);
+        for (int b = 0; b < 32; ++b) stats->ni_histogram[b] = c->h_hdr->hist[b];
+        stats->wall_seconds =
+            std::chrono::duration<double>(std::chrono::steady_clock::now() - wall0).count();
+        stats->gpu_call_seconds = stats->wall_seconds;
+    }
+    return NBK_OK;
+}
+
+}  // extern "C"

@@ -58,6 +58,11 @@ def test_null_and_bad_arguments(lib):
     assert lib.nbk_calc_firsthalf(None, 1, 1, None, None, None, 0.0, 0) == binding.NBK_EINVAL
     assert lib.nbk_calc_lasthalf(None, 1, None, None, None) == binding.NBK_EINVAL
     assert lib.nbk_hermite_evolve(None, 1, None, None, None, 0.0, 1.0, 0.01, 0.0625, None) == binding.NBK_EINVAL
+    assert lib.nbk_hermite_evolve_dev(None, 1, None, None, None, 0.0, 1.0, 0.01, 0.0625, None) == binding.NBK_EINVAL
+    assert lib.nbk_get_neighbours(None, 1, None, None) == binding.NBK_EINVAL
+    assert lib.nbk_get_neighbours_dev(None, 1, None, None) == binding.NBK_EINVAL
+    assert lib.nbk_calc_batch(None, 1, None, None, None, None, None, 0.0, 0, None, None) == binding.NBK_EINVAL
+    assert lib.nbk_calc_batch_dev(None, 1, None, None, None, None, None, 0.0, 0, None, None) == binding.NBK_EINVAL
 
 
 def test_no_gpu_fails_loudly(lib):
