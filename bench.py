@@ -359,6 +359,77 @@ def run_ours(args, wl):
     return 0
 
 
+def run_sweep(args):
+    """--sweep: the paper's Table 3 / Table 4 shape (kernel-only time against N)
+    plus the block-step i-set sizes of config C2, as a markdown table on stdout.  Not the bench line."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --sweep needs a CUDA device")
+    from paper_0707_0438_b200 import binding as nb
+    from paper_0707_0438_b200 import inputs
+    nb.load()
+    sm = torch.cuda.get_device_properties(0).multi_processor_count
+    peak = sm * 128 * 2 * 1.965e9
+    eps2 = float(np.float32(1.0 / 256.0) ** 2)
+
+    def kernel_ms(ctx, n_j, n_i, idx, flags, e2, reps):
+        ts = []
+        for _ in range(reps + 2):
+            nb.nbk_calc_firsthalf(ctx, n_j, n_i, idx, None, None, e2, flags)
+            t = nb.nbk_get_timing(ctx)
+            ts.append(t["force"] + t["reduce"])
+        return float(np.median(ts[2:]))
+
+    print("| N | acc+jerk+pot ms | interactions/s | TFLOP/s (42) | % FP32 peak | TFLOP/s (k=60) | "
+          "acc+pot ms | interactions/s | TFLOP/s (20) | eps=0 ms | +nearest neighbour ms |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|")
+    seeds = {1024: 1, 16384: 2, 131072: 3, 1048576: 4, 65536: 5}
+    for lg in range(10, 21):
+        n = 1 << lg
+        m, x, v = inputs.plummer_f32(n, seeds.get(n, 100 + lg))
+        ctx = nb.nbk_open(0, n, n)
+        try:
+            nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+            nb.nbk_set_ti(ctx, 0.0)
+            nb.nbk_set_timing(ctx, True)
+            reps = 9 if n <= 131072 else 3
+            full = kernel_ms(ctx, n, n, None, nb.NBK_JERK | nb.NBK_POT, eps2, reps)
+            accp = kernel_ms(ctx, n, n, None, nb.NBK_POT, eps2, reps)
+            e0 = kernel_ms(ctx, n, n, None, nb.NBK_JERK | nb.NBK_POT | nb.NBK_EPS0, 0.0, reps)
+            nn = kernel_ms(ctx, n, n, None, nb.NBK_JERK | nb.NBK_POT | nb.NBK_NN, eps2, reps)
+        finally:
+            nb.nbk_close(ctx)
+        r = n * n / (full * 1e-3)
+        ra = n * n / (accp * 1e-3)
+        print(f"| {n} | {full:.4f} | {r:.3e} | {42 * r / 1e12:.2f} | {100 * 42 * r / peak:.1f} | {60 * r / 1e12:.2f} | "
+              f"{accp:.4f} | {ra:.3e} | {20 * ra / 1e12:.2f} | {e0:.4f} | {nn:.4f} |", flush=True)
+    print()
+    print("| N | n_i (block) | force+reduce kernels us | interactions/s | firsthalf+lasthalf wall us (host API) |")
+    print("|---|---|---|---|---|")
+    for n, seed in ((16384, 2), (65536, 5)):
+        m, x, v = inputs.plummer_f32(n, seed)
+        ctx = nb.nbk_open(0, n, n)
+        try:
+            nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+            for n_i in (1, 32, 256, 2048, 16384):
+                idx = inputs.active_block(n, n_i, seed=2)
+                nb.nbk_set_timing(ctx, True)
+                nb.nbk_set_ti(ctx, 0.0)
+                k = kernel_ms(ctx, n, n_i, idx, nb.NBK_JERK | nb.NBK_POT, eps2, 9)
+                nb.nbk_set_timing(ctx, False)
+                reps = 100 if n_i <= 2048 else 20
+                t0 = time.perf_counter()
+                for q in range(reps):
+                    nb.nbk_set_ti(ctx, 1e-4 * (q + 1))     # forces a new prediction, as a block step does
+                    nb.nbk_calc_firsthalf(ctx, n, n_i, idx, None, None, eps2, nb.NBK_JERK | nb.NBK_POT)
+                    nb.nbk_calc_lasthalf(ctx, n_i)
+                w = (time.perf_counter() - t0) / reps
+                print(f"| {n} | {n_i} | {k * 1e3:.1f} | {n * n_i / (k * 1e-3):.3e} | {w * 1e6:.1f} |", flush=True)
+        finally:
+            nb.nbk_close(ctx)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -368,7 +439,11 @@ def main(argv=None):
     ap.add_argument("--workload", choices=sorted(WORKLOADS), default="C3")
     ap.add_argument("--skip-cpu-baseline", action="store_true",
                     help="do not time the oracle (for runs under ncu); cpu_baseline is then null")
+    ap.add_argument("--sweep", action="store_true",
+                    help="print kernel time against N (1K..1M) and the block-step sweep as markdown tables")
     args = ap.parse_args(argv)
+    if args.sweep:
+        return run_sweep(args)
     wl = WORKLOADS[args.workload]
     if args.impl == "reference":
         return run_reference(args, wl)
