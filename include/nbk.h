@@ -200,10 +200,10 @@ int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, double* x, doub
 
 /* The same integration with the whole block-step loop on the device (PAPER.md
  * L346, L368 name it as what fp64 GPUs make possible): after the forces at t = 0, every block step
- * is five stream-ordered launches -- scheduler (next block time from per-level particle counts),
- * predictor + selection of the particles due, i x j force kernel planned on the device, reduction,
- * fp64 corrector + Aarseth step + block rule -- enqueued in batches of 256 steps with no host
- * synchronisation in between.  Same scheme, formulas and arguments as nbk_hermite_evolve (dt_max
+ * is four stream-ordered launches -- predictor + selection of the particles due, i x j force kernel
+ * planned on the device, reduction, fp64 corrector + Aarseth step + block rule whose last block also
+ * schedules the next step (next block time from per-level particle counts) -- replayed from a CUDA
+ * graph in batches of 256 steps with no host synchronisation in between.  Same scheme, formulas and arguments as nbk_hermite_evolve (dt_max
  * <= 1); stats->gpu_call_seconds equals wall_seconds. */
 int nbk_hermite_evolve_dev(nbk_ctx* ctx, int64_t n, const double* m, double* x, double* v,
                            double eps, double t_end, double eta, double dt_max,

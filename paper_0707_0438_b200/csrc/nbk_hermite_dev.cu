@@ -111,7 +111,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     NBK_CUDA(c, cudaMemcpyAsync(c->d_hdr, &H, sizeof(H), cudaMemcpyHostToDevice, c->stream));
     NBK_CUDA(c, cudaStreamSynchronize(c->stream));   // the host vectors above may go away
 
-    // one block step = begin, predict + select, force (+ reduce), correct; enqueued in batches with
+    // one block step = predict + select, force (+ reduce), correct + next step's header; enqueued in batches with
     // no host synchronisation inside a batch; steps past t_end return at once (done flag)
     Variant vv{1, true, eps2 == 0.f, true, false};
     const long long n_pad = round_up_ll(n, kTileJMax);
@@ -135,13 +135,13 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     r.acc = f.tail.acc; r.jerk = f.tail.jerk; r.pot = f.tail.pot;
     r.dyn = c->d_hdr;
     r.n_j = static_cast<int>(n);
-    // the five launches of a block step are captured once into a CUDA graph and replayed
+    // the four launches of a block step are captured once into a CUDA graph and replayed
     const int kBatch = 256;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t gexec = nullptr;
+    NBK_CUDA(c, launch_hd_begin(c->d_hdr, c->stream));   // first step; later ones: hd_correct's tail
     auto enqueue_step = [&]() -> cudaError_t {
         cudaError_t e;
-        if ((e = launch_hd_begin(c->d_hdr, c->stream)) != cudaSuccess) return e;
         if ((e = launch_hd_predict(c->raw, c->d_hdr, c->hs, n_pad, pred_arr(c, 0), pred_arr(c, 1),
                                    pred_arr(c, 2), pred_arr(c, 3), pred_arr(c, 4), pred_arr(c, 5),
                                    pred_arr(c, 6), c->stream)) != cudaSuccess) return e;

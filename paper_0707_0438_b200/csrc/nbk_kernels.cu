@@ -727,8 +727,9 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
     const int ix = 1 << ix_log2, ry = 256 >> ix_log2;
     const int tid = threadIdx.x;
     const int tx = tid & (ix - 1), ty = tid >> ix_log2;
-    const long long i0 = static_cast<long long>(blockIdx.x) * ix;
-    if (i0 >= d.n_i) return;
+    // grid-stride over blocks of ix i-particles (the dyn launch has a fixed grid)
+    for (long long i0 = static_cast<long long>(blockIdx.x) * ix; i0 < d.n_i;
+         i0 += static_cast<long long>(gridDim.x) * ix) {
     const long long i = i0 + tx;
     const bool valid = i < d.n_i;
     const int it = static_cast<int>(i0 / d.ti);
@@ -802,6 +803,8 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
         a.jerk[3 * i + 0] = static_cast<float>(sh[4][tid]);
         a.jerk[3 * i + 1] = static_cast<float>(sh[5][tid]);
         a.jerk[3 * i + 2] = static_cast<float>(sh[6][tid]);
+    }
+    __syncthreads();   // shared arrays are reused by the next block of i-particles
     }
 }
 
@@ -1038,7 +1041,9 @@ __global__ void batch_pack_kernel(const BatchPackArgs a) {
 // Particles sit in one list per power-of-two level k (step 2^-k); all particles of a level share
 // their last-update time, so the next block time follows from the finest occupied level and the
 // particles due are those with level >= kstar: no pass over N to find them.
-__global__ void hd_begin_kernel(DynHeader* h) {   // one CTA of 64 threads
+// Called by every thread of one CTA (>= 64 threads): hd_begin_kernel for the first step, the last
+// block of hd_correct_kernel for all later ones.
+__device__ void hd_begin_body(DynHeader* h) {
     __shared__ long long cnt[kMaxLevel + 1];
     __shared__ long long cost[kPlanCandidates];
     __shared__ Decomp cand[kPlanCandidates];
@@ -1087,6 +1092,10 @@ __global__ void hd_begin_kernel(DynHeader* h) {   // one CTA of 64 threads
         h->plan = cand[bc];
         h->fused = cand[bc].nit == 1 && cand[bc].n_i <= kFusedMaxI;
     }
+}
+
+__global__ void hd_begin_kernel(DynHeader* h) {   // one CTA of 64 threads
+    hd_begin_body(h);
 }
 
 // a3 for the device-resident integrator: predict every j to t_next and, in the same pass, list the
@@ -1162,9 +1171,8 @@ __device__ __forceinline__ int level_for_dev(double want, int kmin) {
 __global__ void hd_correct_kernel(const RawJ raw, DynHeader* h, const HermiteState hs,
                                   const float* acc, const float* jerk) {
     if (h->done) return;
-    const int q = blockIdx.x * blockDim.x + threadIdx.x;
     const int n_act = h->n_act;
-    if (q >= n_act) return;
+    for (int q = blockIdx.x * blockDim.x + threadIdx.x; q < n_act; q += gridDim.x * blockDim.x) {
     const int i = hs.act[q];
     const int k0 = hs.level[i];
     const double dt = ldexp(1.0, -k0);
@@ -1223,6 +1231,22 @@ __global__ void hd_correct_kernel(const RawJ raw, DynHeader* h, const HermiteSta
         int b = 0;
         while ((2LL << b) <= n_act && b < 31) ++b;
         h->hist[b] += 1;
+    }
+    }
+    // the last block to finish prepares the next step (T_next, who is due, launch plan): one launch
+    // less per block step than a separate hd_begin_kernel
+    __shared__ int is_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned ticket = atomicAdd(&h->ticket, 1u);
+        is_last = (ticket == gridDim.x - 1u);
+        if (is_last) h->ticket = 0u;
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        hd_begin_body(h);
     }
 }
 
@@ -1458,12 +1482,15 @@ cudaError_t launch_hd_predict(const RawJ& raw, DynHeader* h, const HermiteState&
 
 cudaError_t launch_hd_correct(const RawJ& raw, DynHeader* h, const HermiteState& hs, const float* acc,
                               const float* jerk, int n, cudaStream_t st) {
-    hd_correct_kernel<<<(n + 127) / 128, 128, 0, st>>>(raw, h, hs, acc, jerk);
+    int grid = (n + 127) / 128;
+    if (grid > 64) grid = 64;   // grid-stride over the due particles; most steps hold a handful
+    hd_correct_kernel<<<grid, 128, 0, st>>>(raw, h, hs, acc, jerk);
     return cudaGetLastError();
 }
 
 cudaError_t launch_reduce_dyn(const Variant& v, const ReduceArgs& a, int ni_max, cudaStream_t s) {
-    const unsigned grid = static_cast<unsigned>((ni_max + 31) / 32);
+    unsigned grid = static_cast<unsigned>((ni_max + 31) / 32);
+    if (grid > 296) grid = 296;   // grid-stride: most steps return at once (reduced by the force kernel)
     if (v.jerk) reduce_kernel<true, false><<<grid, 256, 0, s>>>(a, 5);
     else reduce_kernel<false, false><<<grid, 256, 0, s>>>(a, 5);
     return cudaGetLastError();

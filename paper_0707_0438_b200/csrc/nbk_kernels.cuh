@@ -125,6 +125,7 @@ struct DynHeader {
     long long hist[32];
     Decomp plan;                        // launch plan of the current step (made once, hd_begin_kernel)
     int fused;                          // the force kernel's last CTA reduces (small block)
+    unsigned ticket;                    // arrival counter of hd_correct_kernel's blocks
 };
 struct HermiteState {        // fp64 integrator state, [n][3] row-major; level[n]
     double* x;
