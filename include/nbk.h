@@ -68,6 +68,16 @@ typedef enum nbk_status {
  * All device and pinned memory is allocated here, none later. */
 int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cuda_stream);
 
+/* The same with the context's device buffers carved out of ONE caller-owned device buffer (e.g. a
+ * torch tensor), so that the caller's allocator owns the memory: `workspace` is a device pointer
+ * aligned to 256 bytes holding at least nbk_workspace_bytes(device, n_max, ni_max) bytes; it must
+ * outlive the context and is not freed by nbk_close.  Pinned host staging, and the buffers that
+ * nbk_hermite_evolve_dev and nbk_calc_batch allocate on first use, stay the library's. */
+int nbk_open_ws(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cuda_stream,
+                void* workspace, int64_t workspace_bytes);
+/* Bytes of workspace nbk_open_ws needs on `device` (depends on its SM count), or a negative status. */
+int64_t nbk_workspace_bytes(int device, int64_t n_max, int64_t ni_max);
+
 /* Free everything the context owns (waits for its stream first).  NULL is accepted. */
 int nbk_close(nbk_ctx* ctx);
 
@@ -135,6 +145,8 @@ int nbk_calc_firsthalf_dev(nbk_ctx* ctx, int64_t n_j, int64_t n_i, const int32_t
 /* Wait for the last firsthalf and copy acc[n_i][3], jerk[n_i][3], pot[n_i] to HOST arrays
  * (any may be NULL; jerk is zero if NBK_JERK was not set).  n_i must equal firsthalf's. */
 int nbk_calc_lasthalf(nbk_ctx* ctx, int64_t n_i, float* acc, float* jerk, float* pot);
+/* Same into double arrays (GRAPE-style callers keep doubles); the values are the fp32 results. */
+int nbk_calc_lasthalf_f64(nbk_ctx* ctx, int64_t n_i, double* acc, double* jerk, double* pot);
 /* Same to DEVICE arrays, asynchronous on the stream, no synchronisation. */
 int nbk_calc_lasthalf_dev(nbk_ctx* ctx, int64_t n_i, float* acc, float* jerk, float* pot);
 

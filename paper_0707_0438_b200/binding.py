@@ -18,9 +18,9 @@ NBK_OK, NBK_EINVAL, NBK_ERANGE, NBK_ENOMEM, NBK_ECUDA, NBK_ESTATE = 0, -1, -2, -
 NBK_JERK, NBK_POT, NBK_EPS0, NBK_NN = 1, 2, 4, 8
 
 EXPORTS = [
-    "nbk_open", "nbk_close", "nbk_npipes", "nbk_set_j_particles", "nbk_set_j_particles_f64",
+    "nbk_open", "nbk_open_ws", "nbk_workspace_bytes", "nbk_close", "nbk_npipes", "nbk_set_j_particles", "nbk_set_j_particles_f64",
     "nbk_set_j_particles_dev", "nbk_set_ti", "nbk_predict", "nbk_get_predicted",
-    "nbk_calc_firsthalf", "nbk_calc_firsthalf_dev", "nbk_calc_lasthalf", "nbk_calc_lasthalf_dev",
+    "nbk_calc_firsthalf", "nbk_calc_firsthalf_dev", "nbk_calc_lasthalf", "nbk_calc_lasthalf_f64", "nbk_calc_lasthalf_dev",
     "nbk_get_neighbours", "nbk_get_neighbours_dev", "nbk_calc_batch", "nbk_calc_batch_dev",
     "nbk_hermite_evolve", "nbk_hermite_evolve_dev", "nbk_sync", "nbk_set_timing", "nbk_get_timing", "nbk_last_launch",
     "nbk_plan", "nbk_set_variant", "nbk_last_cuda_error", "nbk_strerror", "nbk_version",
@@ -38,6 +38,8 @@ class HermiteStats(ctypes.Structure):
 
 _SIGS = {
     "nbk_open": (_i32, [ctypes.POINTER(_vp), _i32, _i64, _i64, _vp]),
+    "nbk_open_ws": (_i32, [ctypes.POINTER(_vp), _i32, _i64, _i64, _vp, _vp, _i64]),
+    "nbk_workspace_bytes": (_i64, [_i32, _i64, _i64]),
     "nbk_close": (_i32, [_vp]),
     "nbk_npipes": (_i32, [_vp]),
     "nbk_set_j_particles": (_i32, [_vp, _i64] + [_vp] * 7),
@@ -49,6 +51,7 @@ _SIGS = {
     "nbk_calc_firsthalf": (_i32, [_vp, _i64, _i64, _vp, _vp, _vp, _f32, _u32]),
     "nbk_calc_firsthalf_dev": (_i32, [_vp, _i64, _i64, _vp, _vp, _vp, _f32, _u32]),
     "nbk_calc_lasthalf": (_i32, [_vp, _i64, _vp, _vp, _vp]),
+    "nbk_calc_lasthalf_f64": (_i32, [_vp, _i64, _vp, _vp, _vp]),
     "nbk_calc_lasthalf_dev": (_i32, [_vp, _i64, _vp, _vp, _vp]),
     "nbk_calc_batch": (_i32, [_vp, _i64, _vp, _vp, _vp, _vp, _vp, _f32, _u32, _vp, _vp]),
     "nbk_calc_batch_dev": (_i32, [_vp, _i64, _vp, _vp, _vp, _vp, _vp, _f32, _u32, _vp, _vp]),
@@ -120,6 +123,21 @@ def _host(a, dtype, shape_tail=None):
 def nbk_open(device: int, n_max: int, ni_max: int, cuda_stream: int = 0):
     ctx = _vp()
     _check("nbk_open", load().nbk_open(ctypes.byref(ctx), device, n_max, ni_max, cuda_stream or None))
+    return ctx
+
+
+def nbk_workspace_bytes(device: int, n_max: int, ni_max: int) -> int:
+    n = load().nbk_workspace_bytes(device, n_max, ni_max)
+    if n < 0:
+        raise NbkError("nbk_workspace_bytes", int(n))
+    return int(n)
+
+
+def nbk_open_ws(device: int, n_max: int, ni_max: int, cuda_stream: int, workspace: int, workspace_bytes: int):
+    """workspace: device address (e.g. tensor.data_ptr()) the caller keeps alive."""
+    ctx = _vp()
+    _check("nbk_open_ws", load().nbk_open_ws(ctypes.byref(ctx), device, n_max, ni_max, cuda_stream or None,
+                                             workspace or None, workspace_bytes))
     return ctx
 
 
@@ -200,6 +218,15 @@ def nbk_calc_lasthalf(ctx, n_i):
     pot = np.empty(n_i, np.float32)
     _check("nbk_calc_lasthalf",
            load().nbk_calc_lasthalf(ctx, n_i, acc.ctypes.data, jerk.ctypes.data, pot.ctypes.data), ctx)
+    return acc, jerk, pot
+
+
+def nbk_calc_lasthalf_f64(ctx, n_i):
+    acc = np.empty((n_i, 3), np.float64)
+    jerk = np.empty((n_i, 3), np.float64)
+    pot = np.empty(n_i, np.float64)
+    _check("nbk_calc_lasthalf_f64",
+           load().nbk_calc_lasthalf_f64(ctx, n_i, acc.ctypes.data, jerk.ctypes.data, pot.ctypes.data), ctx)
     return acc, jerk, pot
 
 

@@ -46,16 +46,18 @@ int flush_pending(nbk_ctx* c) {
 namespace {
 
 void free_all(nbk_ctx* c) {
-    cudaFree(c->raw.x); cudaFree(c->raw.v); cudaFree(c->raw.a); cudaFree(c->raw.k);
-    cudaFree(c->raw.m); cudaFree(c->raw.t); cudaFree(c->pred);
-    cudaFree(c->d_iidx); cudaFree(c->d_xi); cudaFree(c->d_vi);
-    cudaFree(c->d_partial); cudaFree(c->d_result); cudaFree(c->d_stage); cudaFree(c->d_counter);
+    if (!c->caller_workspace) {   // otherwise these are pieces of the caller's buffer
+        cudaFree(c->raw.x); cudaFree(c->raw.v); cudaFree(c->raw.a); cudaFree(c->raw.k);
+        cudaFree(c->raw.m); cudaFree(c->raw.t); cudaFree(c->pred);
+        cudaFree(c->d_iidx); cudaFree(c->d_xi); cudaFree(c->d_vi);
+        cudaFree(c->d_partial); cudaFree(c->d_result); cudaFree(c->d_stage); cudaFree(c->d_counter);
+        cudaFree(c->d_nn_partial); cudaFree(c->d_nn_best); cudaFree(c->d_nn_tile);
+        cudaFree(c->d_nn_index); cudaFree(c->d_nn_r2);
+    }
     cudaFree(c->d_batch);
     cudaFree(c->hs.x); cudaFree(c->hs.v); cudaFree(c->hs.a); cudaFree(c->hs.j);
     cudaFree(c->hs.level); cudaFree(c->hs.act); cudaFree(c->hs.bc_ge); cudaFree(c->d_hdr);
     if (c->h_hdr) cudaFreeHost(c->h_hdr);
-    cudaFree(c->d_nn_partial); cudaFree(c->d_nn_best); cudaFree(c->d_nn_tile);
-    cudaFree(c->d_nn_index); cudaFree(c->d_nn_r2);
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_stage) cudaFreeHost(c->h_stage);
     if (c->h_istage) cudaFreeHost(c->h_istage);
@@ -317,12 +319,48 @@ int set_j_host(nbk_ctx* c, long long n, const int32_t* addr, const double* tj, c
 
 extern "C" {
 
-int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cuda_stream) {
+namespace {
+
+// Device memory of a context comes either from cudaMalloc (nbk_open) or, piece by piece and
+// 256-byte aligned, from one caller-owned buffer (nbk_open_ws; nbk_workspace_bytes adds up the
+// same pieces in the same order).
+struct DeviceArena {
+    unsigned char* base = nullptr;
+    size_t cap = 0, off = 0;
+    cudaError_t take(void** p, size_t bytes) {
+        if (!base) return cudaMalloc(p, bytes);
+        const size_t at = (off + 255) & ~static_cast<size_t>(255);
+        off = at + bytes;
+        if (off > cap) return cudaErrorMemoryAllocation;
+        *p = base + at;
+        return cudaSuccess;
+    }
+};
+
+size_t workspace_total(long long n_max, long long ni_max, int num_sms) {
+    const size_t cap = static_cast<size_t>(round_up(n_max, kTileJMax)), ni = static_cast<size_t>(ni_max);
+    const size_t pb = sizeof(float) * plan_partial_floats_bound(ni_max, num_sms);
+    const size_t sb = static_cast<size_t>(n_max) * (8 + 8 + 4 * 24 + 4) + 16 * 8;
+    const size_t pieces[] = {24 * cap, 12 * cap, 12 * cap, 12 * cap, 4 * cap, 8 * cap, 28 * cap,   // raw, pred
+                             4 * ni, 12 * ni, 12 * ni, 28 * ni, sizeof(unsigned),                   // i staging, result
+                             pb, pb / 4, 4 * ni, 4 * ni, 4 * ni, 4 * ni, sb};                       // partial, nn, stage
+    size_t off = 0;
+    for (size_t b : pieces) off = ((off + 255) & ~static_cast<size_t>(255)) + b;
+    return off;
+}
+
+int open_impl(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cuda_stream,
+              void* workspace, size_t workspace_bytes) {
     if (!out || n_max < 1 || ni_max < 1 || n_max > (1LL << 30) || ni_max > (1LL << 30))
         return NBK_EINVAL;
     *out = nullptr;
     nbk_ctx* c = new (std::nothrow) nbk_ctx();
     if (!c) return NBK_ENOMEM;
+    DeviceArena arena;
+    arena.base = static_cast<unsigned char*>(workspace);
+    arena.cap = workspace_bytes;
+    c->caller_workspace = workspace != nullptr;
+    auto dalloc = [&](void** p, size_t bytes) { return arena.take(p, bytes); };
     std::memset(c->ev, 0, sizeof(c->ev));
     c->pending.n = 0;
     c->device = device;
@@ -358,13 +396,13 @@ int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cud
                     }
         if (e != cudaSuccess) break;
         const size_t cap = static_cast<size_t>(c->n_cap);
-        if ((e = cudaMalloc(&c->raw.x, sizeof(double) * 3 * cap)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->raw.v, sizeof(float) * 3 * cap)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->raw.a, sizeof(float) * 3 * cap)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->raw.k, sizeof(float) * 3 * cap)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->raw.m, sizeof(float) * cap)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->raw.t, sizeof(double) * cap)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->pred, sizeof(float) * 7 * cap)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->raw.x), sizeof(double) * 3 * cap)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->raw.v), sizeof(float) * 3 * cap)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->raw.a), sizeof(float) * 3 * cap)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->raw.k), sizeof(float) * 3 * cap)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->raw.m), sizeof(float) * cap)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->raw.t), sizeof(double) * cap)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->pred), sizeof(float) * 7 * cap)) != cudaSuccess) break;
         if ((e = cudaMemsetAsync(c->raw.x, 0, sizeof(double) * 3 * cap, c->stream)) != cudaSuccess) break;
         if ((e = cudaMemsetAsync(c->raw.v, 0, sizeof(float) * 3 * cap, c->stream)) != cudaSuccess) break;
         if ((e = cudaMemsetAsync(c->raw.a, 0, sizeof(float) * 3 * cap, c->stream)) != cudaSuccess) break;
@@ -373,24 +411,24 @@ int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cud
         if ((e = cudaMemsetAsync(c->raw.t, 0, sizeof(double) * cap, c->stream)) != cudaSuccess) break;
         if ((e = cudaMemsetAsync(c->pred, 0, sizeof(float) * 7 * cap, c->stream)) != cudaSuccess) break;
         const size_t ni = static_cast<size_t>(ni_max);
-        if ((e = cudaMalloc(&c->d_iidx, sizeof(int32_t) * ni)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_xi, sizeof(float) * 3 * ni)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_vi, sizeof(float) * 3 * ni)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_result, sizeof(float) * 7 * ni)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_iidx), sizeof(int32_t) * ni)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_xi), sizeof(float) * 3 * ni)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_vi), sizeof(float) * 3 * ni)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_result), sizeof(float) * 7 * ni)) != cudaSuccess) break;
         if ((e = cudaHostAlloc(&c->h_result, sizeof(float) * 9 * ni, cudaHostAllocMapped)) != cudaSuccess) break;
         if ((e = cudaHostGetDevicePointer(&c->h_result_dev, c->h_result, 0)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_counter, sizeof(unsigned))) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_counter), sizeof(unsigned))) != cudaSuccess) break;
         if ((e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned), c->stream)) != cudaSuccess) break;
         c->partial_bytes = sizeof(float) * plan_partial_floats_bound(ni_max, c->num_sms);
-        if ((e = cudaMalloc(&c->d_partial, c->partial_bytes)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_nn_partial, c->partial_bytes / 4)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_nn_best, sizeof(float) * ni)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_nn_tile, sizeof(int32_t) * ni)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_nn_index, sizeof(int32_t) * ni)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_nn_r2, sizeof(float) * ni)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_partial), c->partial_bytes)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_nn_partial), c->partial_bytes / 4)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_nn_best), sizeof(float) * ni)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_nn_tile), sizeof(int32_t) * ni)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_nn_index), sizeof(int32_t) * ni)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_nn_r2), sizeof(float) * ni)) != cudaSuccess) break;
         c->stage_bytes = static_cast<size_t>(n_max) * (8 + 8 + 4 * 24 + 4) + 16 * 8;
         if ((e = cudaMallocHost(&c->h_stage, c->stage_bytes)) != cudaSuccess) break;
-        if ((e = cudaMalloc(&c->d_stage, c->stage_bytes)) != cudaSuccess) break;
+        if ((e = dalloc(reinterpret_cast<void**>(&c->d_stage), c->stage_bytes)) != cudaSuccess) break;
         if ((e = cudaMallocHost(&c->h_istage, ni * 28 + 64)) != cudaSuccess) break;
         if ((e = cudaEventCreateWithFlags(&c->stage_free, cudaEventDisableTiming)) != cudaSuccess) break;
         if ((e = cudaEventCreateWithFlags(&c->istage_free, cudaEventDisableTiming)) != cudaSuccess) break;
@@ -410,6 +448,28 @@ int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cud
     }
     *out = c;
     return NBK_OK;
+}
+
+}  // namespace
+
+int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cuda_stream) {
+    return open_impl(out, device, n_max, ni_max, cuda_stream, nullptr, 0);
+}
+
+int nbk_open_ws(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cuda_stream,
+                void* workspace, int64_t workspace_bytes) {
+    if (!workspace || workspace_bytes <= 0 || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return NBK_EINVAL;
+    return open_impl(out, device, n_max, ni_max, cuda_stream, workspace, static_cast<size_t>(workspace_bytes));
+}
+
+int64_t nbk_workspace_bytes(int device, int64_t n_max, int64_t ni_max) {
+    if (n_max < 1 || ni_max < 1 || n_max > (1LL << 30) || ni_max > (1LL << 30)) return NBK_EINVAL;
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return NBK_ECUDA;
+    }
+    return static_cast<int64_t>(workspace_total(n_max, ni_max, sms));
 }
 
 int nbk_close(nbk_ctx* c) {
@@ -575,6 +635,22 @@ int nbk_calc_lasthalf(nbk_ctx* c, int64_t n_i, float* acc, float* jerk, float* p
     if (acc) std::memcpy(acc, c->h_result, sizeof(float) * 3 * ni);
     if (jerk) std::memcpy(jerk, c->h_result + 3 * ni, sizeof(float) * 3 * ni);
     if (pot) std::memcpy(pot, c->h_result + 6 * ni, sizeof(float) * ni);
+    return NBK_OK;
+}
+
+int nbk_calc_lasthalf_f64(nbk_ctx* c, int64_t n_i, double* acc, double* jerk, double* pot) {
+    if (!c || n_i < 0) return NBK_EINVAL;
+    if (!c->in_flight || n_i != c->last_ni) return NBK_ESTATE;
+    const int rc = nbk_calc_lasthalf(c, n_i, nullptr, nullptr, nullptr);   // waits, fills h_result
+    if (rc != NBK_OK) return rc;
+    const size_t ni = static_cast<size_t>(n_i);
+    const float* h = c->h_result;
+    for (size_t k = 0; k < 3 * ni; ++k) {
+        if (acc) acc[k] = h[k];
+        if (jerk) jerk[k] = h[3 * ni + k];
+    }
+    if (pot)
+        for (size_t k = 0; k < ni; ++k) pot[k] = h[6 * ni + k];
     return NBK_OK;
 }
 

@@ -33,6 +33,7 @@ struct nbk_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
     bool own_stream = false;
+    bool caller_workspace = false;  // device buffers of nbk_open live in the caller's workspace
     long long n_max = 0, ni_max = 0, n_cap = 0;
     int num_sms = 0;
 

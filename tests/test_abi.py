@@ -51,6 +51,9 @@ def test_null_and_bad_arguments(lib):
     ctx = ctypes.c_void_p()
     assert lib.nbk_open(ctypes.byref(ctx), 0, 0, 16, None) == binding.NBK_EINVAL
     assert lib.nbk_open(ctypes.byref(ctx), 0, 16, -1, None) == binding.NBK_EINVAL
+    assert lib.nbk_open_ws(ctypes.byref(ctx), 0, 16, 16, None, None, 1024) == binding.NBK_EINVAL
+    assert lib.nbk_workspace_bytes(0, 0, 16) == binding.NBK_EINVAL
+    assert lib.nbk_calc_lasthalf_f64(None, 1, None, None, None) == binding.NBK_EINVAL
     assert lib.nbk_close(None) == binding.NBK_OK
     assert lib.nbk_npipes(None) == binding.NBK_EINVAL
     assert lib.nbk_set_ti(None, 0.0) == binding.NBK_EINVAL

@@ -617,3 +617,34 @@ def test_batched_calls_device_pointers(gpu, c_oracle):
         nb.nbk_calc_batch_dev(ctx, io, dxi.data_ptr(), jo, dmj.data_ptr(), dxj.data_ptr(), np.float32(EPS) ** 2,
                               nb.NBK_POT, acc.data_ptr(), pot.data_ptr())
     assert_parity((acc.cpu().numpy(), None, pot.cpu().numpy()), (racc, None, rpot), jerk=False, what="batch dev")
+
+
+def test_caller_owned_workspace_and_double_readback(gpu, c_oracle):
+    """nbk_open_ws: every device buffer of the context lives in one torch tensor the caller owns
+    (PyTorch is the allocator); nbk_calc_lasthalf_f64 returns the same fp32 results widened."""
+    torch = gpu
+    n = 5000
+    m, x, v = inputs.plummer_f32(n, seed=301)
+    need = nb.nbk_workspace_bytes(0, n, n)
+    assert need > 0
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    assert ws.data_ptr() % 256 == 0
+    with pytest.raises(nb.NbkError):
+        nb.nbk_open_ws(0, n, n, 0, ws.data_ptr(), need - 1)
+    ctx = nb.nbk_open_ws(0, n, n, 0, ws.data_ptr(), need)
+    try:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, n, n, None, None, None, np.float32(EPS) ** 2, FULL | nb.NBK_NN)
+        got = nb.nbk_calc_lasthalf(ctx, n)
+        got64 = nb.nbk_calc_lasthalf_f64(ctx, n)
+        nn, r2 = nb.nbk_get_neighbours(ctx, n)
+    finally:
+        nb.nbk_close(ctx)
+    ws.zero_()          # still the caller's: close did not free it
+    torch.cuda.synchronize()
+    assert_parity(got, c_oracle.force(m, x, v, EPS), what="workspace ctx")
+    for a, b in zip(got, got64):
+        assert b.dtype == np.float64 and np.array_equal(a.astype(np.float64), b)
+    ref_nn, ref_r2 = c_oracle.nearest_neighbour(x)
+    _check_nn(nn, r2, ref_nn, ref_r2, x, np.arange(n), what="workspace ctx nn")
