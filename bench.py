@@ -316,9 +316,17 @@ def run_ours(args, wl):
     force_ms = float(np.mean(kern_ms["force"]))
     kint = n * n / (force_ms * 1e-3)
     achieved = FLOPS_EXECUTED[jerk] * kint / 1e12
+    # DRAM bytes of one launch of the kernel from the committed ncu --set full capture (bench.py cannot
+    # run under ncu itself); null for workloads that were not captured
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "force_kernel_traffic.json")) as f:
+            traffic = json.load(f).get(args.workload)
+    except Exception:
+        pass
     roofline = {
         "bound": "alu", "kernel": "nbk::force_kernel", "achieved": achieved, "peak": peak_tflops,
-        "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
+        "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": traffic,
         "peak_source": f"{sm_count} SMs x 128 fp32 lanes x 2 x {sm_max_mhz:.0f} MHz ({peak_src}); "
                        "DESIGN.md 'Roofline'",
         "flops_per_interaction": FLOPS_EXECUTED[jerk],
@@ -403,6 +411,22 @@ def run_sweep(args):
         ra = n * n / (accp * 1e-3)
         print(f"| {n} | {full:.4f} | {r:.3e} | {42 * r / 1e12:.2f} | {100 * 42 * r / peak:.1f} | {60 * r / 1e12:.2f} | "
               f"{accp:.4f} | {ra:.3e} | {20 * ra / 1e12:.2f} | {e0:.4f} | {nn:.4f} |", flush=True)
+    # launch + synchronise floor of this box: one 1-particle predictor launch and a stream sync
+    ctx = nb.nbk_open(0, 256, 256)
+    try:
+        nb.nbk_set_j_particles(ctx, None, None, np.ones(1, np.float32), np.zeros((1, 3), np.float32))
+        for q in range(20):
+            nb.nbk_predict(ctx, 1)
+            nb.nbk_sync(ctx)
+        t0 = time.perf_counter()
+        for q in range(500):
+            nb.nbk_predict(ctx, 1)
+            nb.nbk_sync(ctx)
+        floor_us = (time.perf_counter() - t0) / 500 * 1e6
+    finally:
+        nb.nbk_close(ctx)
+    print()
+    print(f"Launch + synchronise floor (one 1-thread-block kernel, stream sync, through the binding): {floor_us:.1f} us")
     print()
     print("| N | n_i (block) | force+reduce kernels us | interactions/s | firsthalf+lasthalf wall us (host API) |")
     print("|---|---|---|---|---|")
