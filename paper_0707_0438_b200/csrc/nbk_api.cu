@@ -1,5 +1,5 @@
 // nbk_api.cu -- the C ABI of include/nbk.h: context, workspaces, staging and launch logic.
-// Every step of the path runs in the kernels of nbk_kernels.cu; this file only moves
+// Every step of the path runs in the kernels of nbk_force.cu / nbk_state_kernels.cu; this file only moves
 // arguments, picks the launch shape and enqueues.  There is no CPU fallback: without a CUDA
 // device nbk_open fails with NBK_ECUDA.
 #include <cuda_runtime.h>

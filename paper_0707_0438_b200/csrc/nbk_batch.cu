@@ -1,5 +1,5 @@
 // nbk_batch.cu -- nbk_calc_batch[_dev]: many (i-group, interaction-list) acc + pot problems in one
-// launch.  Host side only: descriptors, arena, launches; kernels in nbk_kernels.cu.
+// launch.  Host side only: descriptors, arena, launches; kernels in nbk_batch_kernels.cu.
 #include <chrono>
 #include <climits>
 #include <cmath>

@@ -1,0 +1,333 @@
+// nbk_device.cuh -- device-side building blocks shared by the kernel sources: packed f32x2
+// arithmetic, mbarrier / TMA bulk-copy helpers, the shared-memory tile ring's shape, and the
+// i x j tile loops with the nearest-neighbour re-scan (L126-L128).
+// Internal to the CUDA path.
+#pragma once
+#include "nbk_kernels.cuh"
+
+#ifndef NBK_USE_RCP
+#define NBK_USE_RCP 0
+#endif
+#ifndef NBK_UNROLL
+#define NBK_UNROLL 1   // trips of the 4-j step of the packed tile loop unrolled together
+#endif
+
+namespace nbk {
+
+typedef unsigned long long u64;
+
+// ---------------------------------------------------------------- packed fp32 pair helpers
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
+    u64 d;
+    asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ u64 add2(u64 a, u64 b) {
+    u64 d;
+    asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) {
+    u64 d;
+    asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ u64 pack(float lo, float hi) {
+    u64 d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ void unpack(u64 d, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(d));
+}
+__device__ __forceinline__ float rsq(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// ---------------------------------------------------------------- mbarrier / TMA bulk helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            " selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes,
+                                         uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+
+
+__host__ __device__ __forceinline__ long long pair_start(long long k, long long P, int G) {
+    return (k * P) / G;
+}
+
+// Shared memory of force_kernel:
+//   [kStages full mbarriers | kStages empty mbarriers | pad to 128 B]
+//   [kStages x narr x kTileJMax floats]  [nacc*I x threads doubles]
+template <bool JERK>
+struct Shape {
+    static constexpr int narr = JERK ? 7 : 4;   // x y z m [vx vy vz]
+    static constexpr int nacc = JERK ? 10 : 4;  // ax ay az pot [j1 xyz, j2 xyz]
+    static constexpr int stage_floats = narr * kTileJMax;
+};
+
+template <int I, bool JERK>
+constexpr size_t smem_bytes_of() {
+    return 128 + sizeof(float) * kStages * Shape<JERK>::stage_floats +
+           sizeof(double) * Shape<JERK>::nacc * I * warps_of(I) * 32 +
+           8 * I * warps_of(I) * 32;   // nearest-neighbour (distance, tile) per thread and i
+}
+
+// One elected thread: bring j-tile `jt` (tj particles) into a ring slot.
+template <bool JERK>
+__device__ __forceinline__ void issue_tile(const JPred& j, int jt, int tj, float* stage,
+                                           uint32_t bar) {
+    const uint32_t bytes = tj * sizeof(float);
+    constexpr uint32_t stride = kTileJMax * sizeof(float);
+    const size_t off = static_cast<size_t>(jt) * tj;
+    mbar_expect_tx(bar, bytes * Shape<JERK>::narr);
+    const uint32_t dst = smem_u32(stage);
+    bulk_g2s(dst + 0 * stride, j.x + off, bytes, bar);
+    bulk_g2s(dst + 1 * stride, j.y + off, bytes, bar);
+    bulk_g2s(dst + 2 * stride, j.z + off, bytes, bar);
+    bulk_g2s(dst + 3 * stride, j.m + off, bytes, bar);
+    if (JERK) {
+        bulk_g2s(dst + 4 * stride, j.vx + off, bytes, bar);
+        bulk_g2s(dst + 5 * stride, j.vy + off, bytes, bar);
+        bulk_g2s(dst + 6 * stride, j.vz + off, bytes, bar);
+    }
+}
+
+// ------------------------------------------------------------------- the i x j tile loops
+// PAPER.md L91-L96 (kernel steps 1-4).  Per ordered pair (i, j), r = x_j - x_i, w = v_j - v_i,
+// s = r.r + eps2:
+//   pot  += m s^-1/2            (sign applied in reduce_kernel)
+//   acc  += m s^-3/2 r
+//   j1   += m s^-3/2 w ;  j2 += m s^-5/2 (r.w) r ;  jerk = j1 - 3 j2 (formed per partial row)
+// The i-state is held negated (r = x_j + (-x_i) is one add).  sl[q] is the position of the
+// i-particle's own j entry inside this tile (anything outside [0, tj) if it is elsewhere);
+// MASK instantiations zero the mass of that entry.
+// NN instantiations also keep, per i, the smallest s seen in this tile ("a
+// comparison is added with each force calculation to maintain the particle with the minimum
+// distance"); which j it was is found afterwards by re-scanning the one winning tile (nn_scan).
+template <int I, bool JERK, bool EPS0, bool MASK, bool NN>
+__device__ __forceinline__ void tile_packed(const float* __restrict__ sx, int jbeg, int jend,
+                                            const float (&ni)[I][6], const int (&sl)[I],
+                                            u64 (&acc)[I][Shape<JERK>::nacc], float eps2,
+                                            float (&tmin)[I]) {
+    const u64 e2p = pack(eps2, eps2);
+    constexpr int kUnroll = NBK_UNROLL;
+#pragma unroll kUnroll
+    for (int jj = jbeg; jj < jend; jj += 4) {
+        const ulonglong2 X = *reinterpret_cast<const ulonglong2*>(sx + jj);
+        const ulonglong2 Y = *reinterpret_cast<const ulonglong2*>(sx + kTileJMax + jj);
+        const ulonglong2 Z = *reinterpret_cast<const ulonglong2*>(sx + 2 * kTileJMax + jj);
+        const ulonglong2 M = *reinterpret_cast<const ulonglong2*>(sx + 3 * kTileJMax + jj);
+        ulonglong2 VX, VY, VZ;
+        if (JERK) {
+            VX = *reinterpret_cast<const ulonglong2*>(sx + 4 * kTileJMax + jj);
+            VY = *reinterpret_cast<const ulonglong2*>(sx + 5 * kTileJMax + jj);
+            VZ = *reinterpret_cast<const ulonglong2*>(sx + 6 * kTileJMax + jj);
+        }
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const u64 xj = h ? X.y : X.x, yj = h ? Y.y : Y.x, zj = h ? Z.y : Z.x;
+            const u64 mj0 = h ? M.y : M.x;
+#pragma unroll
+            for (int q = 0; q < I; ++q) {
+                u64 mj = mj0;
+                if (MASK) {  // the i-particle's own entry contributes nothing
+                    float mlo, mhi;
+                    unpack(mj0, mlo, mhi);
+                    mlo = (jj + 2 * h == sl[q]) ? 0.f : mlo;
+                    mhi = (jj + 2 * h + 1 == sl[q]) ? 0.f : mhi;
+                    mj = pack(mlo, mhi);
+                }
+                const u64 dx = add2(xj, pack(ni[q][0], ni[q][0]));
+                const u64 dy = add2(yj, pack(ni[q][1], ni[q][1]));
+                const u64 dz = add2(zj, pack(ni[q][2], ni[q][2]));
+                u64 r2 = fma2(dx, dx, e2p);
+                r2 = fma2(dy, dy, r2);
+                r2 = fma2(dz, dz, r2);
+                float r2a, r2b;
+                unpack(r2, r2a, r2b);
+                if (NN) {
+                    float qa = r2a, qb = r2b;
+                    if (MASK) {  // the own entry is nobody's neighbour
+                        qa = (jj + 2 * h == sl[q]) ? __int_as_float(0x7f800000) : qa;
+                        qb = (jj + 2 * h + 1 == sl[q]) ? __int_as_float(0x7f800000) : qb;
+                    }
+                    tmin[q] = fminf(tmin[q], fminf(qa, qb));
+                }
+                float ra = rsq(r2a), rb = rsq(r2b);
+                u64 rinv, rinv2;
+                if (EPS0) {  // zero-distance pairs contribute nothing
+                    ra = r2a > 0.f ? ra : 0.f;
+                    rb = r2b > 0.f ? rb : 0.f;
+                    rinv = pack(ra, rb);
+                    rinv2 = mul2(rinv, rinv);
+                } else if (NBK_USE_RCP) {
+                    rinv = pack(ra, rb);
+                    rinv2 = pack(rcp(r2a), rcp(r2b));
+                } else {
+                    rinv = pack(ra, rb);
+                    rinv2 = mul2(rinv, rinv);
+                }
+                const u64 mrinv = mul2(mj, rinv);
+                acc[q][3] = add2(acc[q][3], mrinv);
+                const u64 mrinv3 = mul2(mrinv, rinv2);
+                acc[q][0] = fma2(mrinv3, dx, acc[q][0]);
+                acc[q][1] = fma2(mrinv3, dy, acc[q][1]);
+                acc[q][2] = fma2(mrinv3, dz, acc[q][2]);
+                if (JERK) {
+                    const u64 vxj = h ? VX.y : VX.x, vyj = h ? VY.y : VY.x, vzj = h ? VZ.y : VZ.x;
+                    const u64 dvx = add2(vxj, pack(ni[q][3], ni[q][3]));
+                    const u64 dvy = add2(vyj, pack(ni[q][4], ni[q][4]));
+                    const u64 dvz = add2(vzj, pack(ni[q][5], ni[q][5]));
+                    u64 rv = mul2(dx, dvx);
+                    rv = fma2(dy, dvy, rv);
+                    rv = fma2(dz, dvz, rv);
+                    acc[q][4] = fma2(mrinv3, dvx, acc[q][4]);
+                    acc[q][5] = fma2(mrinv3, dvy, acc[q][5]);
+                    acc[q][6] = fma2(mrinv3, dvz, acc[q][6]);
+                    const u64 beta = mul2(mul2(rv, rinv2), mrinv3);
+                    acc[q][7] = fma2(beta, dx, acc[q][7]);
+                    acc[q][8] = fma2(beta, dy, acc[q][8]);
+                    acc[q][9] = fma2(beta, dz, acc[q][9]);
+                }
+            }
+        }
+    }
+}
+
+template <int I, bool JERK, bool EPS0, bool MASK>
+__device__ __forceinline__ void tile_scalar(const float* __restrict__ sx, int jbeg, int jend,
+                                            const float (&ni)[I][6], const int (&sl)[I],
+                                            float (&acc)[I][Shape<JERK>::nacc], float eps2) {
+#pragma unroll 2
+    for (int jj = jbeg; jj < jend; ++jj) {
+        const float xj = sx[jj], yj = sx[kTileJMax + jj], zj = sx[2 * kTileJMax + jj];
+        const float mj0 = sx[3 * kTileJMax + jj];
+        float vxj = 0.f, vyj = 0.f, vzj = 0.f;
+        if (JERK) {
+            vxj = sx[4 * kTileJMax + jj]; vyj = sx[5 * kTileJMax + jj]; vzj = sx[6 * kTileJMax + jj];
+        }
+#pragma unroll
+        for (int q = 0; q < I; ++q) {
+            const float mj = (MASK && jj == sl[q]) ? 0.f : mj0;
+            const float dx = xj + ni[q][0], dy = yj + ni[q][1], dz = zj + ni[q][2];
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
+            float rinv = rsq(r2);
+            if (EPS0) rinv = r2 > 0.f ? rinv : 0.f;
+            const float rinv2 = (!EPS0 && NBK_USE_RCP) ? rcp(r2) : rinv * rinv;
+            const float mrinv = mj * rinv;
+            acc[q][3] += mrinv;
+            const float mrinv3 = mrinv * rinv2;
+            acc[q][0] = fmaf(mrinv3, dx, acc[q][0]);
+            acc[q][1] = fmaf(mrinv3, dy, acc[q][1]);
+            acc[q][2] = fmaf(mrinv3, dz, acc[q][2]);
+            if (JERK) {
+                const float dvx = vxj + ni[q][3], dvy = vyj + ni[q][4], dvz = vzj + ni[q][5];
+                const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+                acc[q][4] = fmaf(mrinv3, dvx, acc[q][4]);
+                acc[q][5] = fmaf(mrinv3, dvy, acc[q][5]);
+                acc[q][6] = fmaf(mrinv3, dvz, acc[q][6]);
+                const float beta = (rv * rinv2) * mrinv3;
+                acc[q][7] = fmaf(beta, dx, acc[q][7]);
+                acc[q][8] = fmaf(beta, dy, acc[q][8]);
+                acc[q][9] = fmaf(beta, dz, acc[q][9]);
+            }
+        }
+    }
+}
+
+// Nearest neighbour, second step: one warp re-scans the one j-tile whose minimum won, with the
+// arithmetic of the tile loop (same s for the same pair), and returns the lowest j that attains the
+// tile's minimum, the own entry left out by index (reading R20: ties go to the lowest index).
+// r2out is the unsoftened squared distance of that pair in fp32.
+__device__ __forceinline__ float sfma(float a, float b, float c) {
+    float d;
+    asm("fma.rn.ftz.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
+}
+__device__ __forceinline__ float sadd(float a, float b) {
+    float d;
+    asm("add.rn.ftz.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+    return d;
+}
+__device__ __forceinline__ void nn_scan(const JPred& j, int n_j, int tile, int tj, float nx,
+                                        float ny, float nz, int self, float eps2, int lane,
+                                        int* nn_out, float* r2_out) {
+    float best = __int_as_float(0x7f800000);
+    int bj = 0x7fffffff;
+    if (tile >= 0) {
+        const int j0 = tile * tj;
+        for (int jj = j0 + lane; jj < j0 + tj && jj < n_j; jj += 32) {
+            const float dx = sadd(j.x[jj], nx), dy = sadd(j.y[jj], ny), dz = sadd(j.z[jj], nz);
+            const float s = sfma(dz, dz, sfma(dy, dy, sfma(dx, dx, eps2)));
+            if (jj != self && s < best) { best = s; bj = jj; }   // ascending jj: first minimum kept
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float ob = __shfl_xor_sync(0xffffffffu, best, o);
+        const int oj = __shfl_xor_sync(0xffffffffu, bj, o);
+        if (ob < best || (ob == best && oj < bj)) { best = ob; bj = oj; }
+    }
+    if (lane == 0) {
+        if (bj == 0x7fffffff) {
+            *nn_out = -1;
+            *r2_out = __int_as_float(0x7f800000);
+        } else {
+            const float dx = sadd(j.x[bj], nx), dy = sadd(j.y[bj], ny), dz = sadd(j.z[bj], nz);
+            *nn_out = bj;
+            *r2_out = sfma(dz, dz, sfma(dy, dy, dx * dx));
+        }
+    }
+}
+
+template <bool PACKED> struct AccT { typedef float type; };
+template <> struct AccT<true> { typedef u64 type; };
+
+__device__ __forceinline__ float acc_take(u64& a) {
+    float lo, hi;
+    unpack(a, lo, hi);
+    a = 0ull;
+    return lo + hi;
+}
+__device__ __forceinline__ float acc_take(float& a) {
+    const float s = a;
+    a = 0.f;
+    return s;
+}
+
+
+}  // namespace nbk

@@ -1,6 +1,6 @@
 // nbk_hermite_dev.cu -- nbk_hermite_evolve_dev: the Hermite block-step loop resident on the device
 // (SURVEY.md 8(f)-1).  Host side only: state upload, CUDA-graph replay of the five launches of a step,
-// termination check; the kernels (hd_*) are in nbk_kernels.cu.
+// termination check; the kernels (hd_*) are in nbk_hermite_kernels.cu.
 #include <chrono>
 #include <climits>
 #include <cmath>

@@ -1,4 +1,5 @@
-// nbk_kernels.cuh -- launch-side declarations shared by nbk_kernels.cu and nbk_api.cu.
+// nbk_kernels.cuh -- launch-side declarations shared by the kernel sources (nbk_force.cu, nbk_*_kernels.cu)
+// and the host sources (nbk_api.cu, nbk_hermite_dev.cu, nbk_batch.cu).
 // Internal to the CUDA path; nothing here is part of the C ABI (include/nbk.h).
 #pragma once
 #include <cuda_runtime.h>
