@@ -8,6 +8,9 @@
 #ifndef NBK_USE_RCP
 #define NBK_USE_RCP 0
 #endif
+#ifndef NBK_FOLD
+#define NBK_FOLD 2     // j-tiles between folds of the fp32 accumulators into fp64 (power of two)
+#endif
 #ifndef NBK_UNROLL
 #define NBK_UNROLL 1   // trips of the 4-j step of the packed tile loop unrolled together
 #endif

@@ -195,15 +195,17 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
         __syncwarp();
         if (lane == 0) mbar_arrive(empty0 + 8 * slot);
 
-        // second level: fold this tile's fp32 sums into the thread's private fp64 slots
-#pragma unroll
-        for (int q = 0; q < I; ++q) {
-#pragma unroll
-            for (int v = 0; v < NACC; ++v)
-                sacc[(q * NACC + v) * T + tid] += static_cast<double>(acc_take(acc[q][v]));
-        }
-
+        // second level: fold the fp32 sums into the thread's private fp64 slots, every NBK_FOLD tiles
+        // (fp32 stays within <= NBK_FOLD * 128 terms per packed half) and at the end of a segment
         const bool last_of_tile = (jt == d.njt - 1) || (n == n_local - 1);
+        if (last_of_tile || (jt & (NBK_FOLD - 1)) == NBK_FOLD - 1) {
+#pragma unroll
+            for (int q = 0; q < I; ++q) {
+#pragma unroll
+                for (int v = 0; v < NACC; ++v)
+                    sacc[(q * NACC + v) * T + tid] += static_cast<double>(acc_take(acc[q][v]));
+            }
+        }
         if (last_of_tile) {
             // one partial row per (CTA, i-tile touched): 8 floats per i.  When wjn warps split
             // the j-tiles, the warp with slice 0 adds the wjn private sums of each i (fixed order).
