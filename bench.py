@@ -367,6 +367,93 @@ def run_ours(args, wl):
     return 0
 
 
+def run_sharded(args, wl):
+    """--shard j: the j-sharded path (paper_0707_0438_b200/sharded.py): every rank
+    holds N/G j-particles, computes partial sums for all N i-particles, two all-reduces per step.
+    Total work is fixed as G grows ("strong").  Not the default multi-GPU mode."""
+    import torch
+    rank, local, world = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    from paper_0707_0438_b200 import binding as nb
+    from paper_0707_0438_b200 import inputs
+    from paper_0707_0438_b200.sharded import ShardedForce
+    nb.load()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    cfg, eps, jerk, desc = wl
+    m, x, v = inputs.config_inputs(cfg)
+    n = m.shape[0]
+    eps2 = float(np.float32(eps) ** 2)
+    flags = (nb.NBK_JERK if jerk else 0) | nb.NBK_POT
+    sf = ShardedForce(n, n, device=local)
+    try:
+        sf.set_j_particles(None, None, m, x, v)
+        sf.set_ti(0.0)
+        ig = torch.arange(n, dtype=torch.int32, device=dev)
+        out = (torch.empty((n, 3), dtype=torch.float32, device=dev), torch.empty((n, 3), dtype=torch.float32, device=dev),
+               torch.empty((n,), dtype=torch.float32, device=dev))
+        flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+
+        def barrier():
+            if world > 1:
+                import torch.distributed as dist
+                dist.barrier()
+            torch.cuda.synchronize(dev)
+
+        nb.nbk_set_timing(sf.ops.ctx, True)
+        for _ in range(max(args.warmup, 0)):
+            flush.zero_()
+            sf.calc(ig, eps2, flags, out)
+        barrier()
+        sampler = ClockSampler(physical_gpu_index(local))
+        sampler.start()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        force_ms = []
+        for k in range(args.steps):
+            flush.zero_()
+            evs[k][0].record()
+            sf.calc(ig, eps2, flags, out)
+            evs[k][1].record()
+            force_ms.append(nb.nbk_get_timing(sf.ops.ctx)["force"])
+        barrier()
+        clocks = sampler.stop()
+        local_ms = float(np.sum([a.elapsed_time(b) for a, b in evs]))
+        # strong scaling: the job's units are N x N per step whatever G is; time = max over ranks
+        total_ms, units_sum = aggregate(local_ms, float(args.steps) * n * sf.n_local, world, str(dev))
+        launch = nb.nbk_last_launch(sf.ops.ctx)
+        assert bool(torch.isfinite(out[0]).all()) and bool(torch.isfinite(out[2]).all())
+    finally:
+        sf.close()
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    if rank != 0:
+        return 0
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak_tflops = sm_count * 128 * 2 * 1.965e9 / 1e12
+    kint = n * sf.n_local / (float(np.mean(force_ms)) * 1e-3)
+    achieved = FLOPS_EXECUTED[jerk] * kint / 1e12
+    line = {
+        "metric": METRIC, "value": units_sum / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": desc, "n_i": n, "n_j": n, "parallelism": f"j-sharded x{world}",
+                   "n_j_per_rank": sf.n_local, "collectives_per_step": 2 if world > 1 else 0,
+                   "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB write)", "launch": launch},
+        "clocks": clocks, "gpu_launches": int(args.steps * 5),
+        "roofline": {"bound": "alu", "kernel": "nbk::force_kernel (rank 0)", "achieved": achieved, "peak": peak_tflops,
+                     "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
+                     "kernel_ms": float(np.mean(force_ms))},
+        "cpu_baseline": None,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def run_sweep(args):
     """--sweep: the paper's Table 3 / Table 4 shape (kernel-only time against N)
     plus the block-step i-set sizes of config C2, as a markdown table on stdout.  Not the bench line."""
@@ -465,12 +552,17 @@ def main(argv=None):
                     help="do not time the oracle (for runs under ncu); cpu_baseline is then null")
     ap.add_argument("--sweep", action="store_true",
                     help="print kernel time against N (1K..1M) and the block-step sweep as markdown tables")
+    ap.add_argument("--shard", choices=["none", "j"], default="none",
+                    help="j: shard the j-particles over the ranks with two all-reduces per step (strong scaling); "
+                         "default: independent replicas (weak)")
     args = ap.parse_args(argv)
     if args.sweep:
         return run_sweep(args)
     wl = WORKLOADS[args.workload]
     if args.impl == "reference":
         return run_reference(args, wl)
+    if args.shard == "j":
+        return run_sharded(args, wl)
     return run_ours(args, wl)
 
 

@@ -223,6 +223,37 @@ int nbk_hermite_evolve_dev(nbk_ctx* ctx, int64_t n, const double* m, double* x, 
 
 /* ---- utilities --------------------------------------------------------------------------- */
 
+/* ---- j-sharding over several GPUs --------------------------------------
+ * "the j-particles are divided in blocks ... the partial forces are stored ...
+ * after which they are summed".  Stretched over devices: rank r of G holds the j-particles with
+ * global addresses [j0_r, j0_r + n_local_r) in its own context (local address = global - j0_r),
+ * every rank computes the partial sums of ALL active i-particles against its own j-particles, and
+ * one all-reduce(sum) of n_i x 8 doubles gives every rank the total.  The library does the three
+ * device steps; the two all-reduces between them are the caller's (torch.distributed / NCCL; the
+ * Python class ShardedForce in paper_0707_0438_b200/sharded.py strings them together).  All
+ * pointers are DEVICE pointers; everything is enqueued on the context's stream, nothing waits.
+ *
+ * 1. nbk_shard_gather_i_dev: predict (if stale), then for each i-particle k with global address
+ *    i_global[k]: i_local[k] = its local address if this rank owns it, else -1;
+ *    xv[k][0..7] = (x, y, z, 0, vx, vy, vz, 0) of its predicted fp32 state if owned, else zeros.
+ *    Exactly one rank owns each i-particle, so all-reduce(sum) of xv over the ranks is an exact
+ *    copy of the owner's state to everybody.
+ * 2. nbk_shard_calc_partial_dev: the force kernel and split-j reduction of i-particles with the
+ *    state xv (after the exchange) against local j-particles [0, n_local), the own entry of an
+ *    owned i-particle (i_local[k] >= 0) left out; writes sum64[k][0..7] = (acc(3), -pot, jerk(3),
+ *    0) as the fp64 sums BEFORE the rounding to fp32 (the fp32 results of this rank alone remain
+ *    readable with nbk_calc_lasthalf*).  flags as nbk_calc_firsthalf; NBK_NN is refused
+ *    (NBK_EINVAL).  n_local == 0 is allowed (sums are zero).
+ * 3. nbk_shard_finish_dev: after all-reduce(sum) of sum64: acc, jerk, pot in fp32 (one rounding;
+ *    pot = -sum64[k][3]); any output may be NULL.  Every rank gets bit-identical results because
+ *    an all-reduce returns the same bits on every rank. */
+int nbk_shard_gather_i_dev(nbk_ctx* ctx, int64_t n_local, int64_t j0, int64_t n_i,
+                           const int32_t* i_global, int32_t* i_local, float* xv);
+int nbk_shard_calc_partial_dev(nbk_ctx* ctx, int64_t n_local, int64_t n_i, const int32_t* i_local,
+                               const float* xv, float eps2, uint32_t flags, double* sum64);
+int nbk_shard_finish_dev(nbk_ctx* ctx, int64_t n_i, const double* sum64, float* acc, float* jerk,
+                         float* pot);
+
 /* Block until everything enqueued on the context's stream has run. */
 int nbk_sync(nbk_ctx* ctx);
 

@@ -22,6 +22,7 @@ EXPORTS = [
     "nbk_set_j_particles_dev", "nbk_set_ti", "nbk_predict", "nbk_get_predicted",
     "nbk_calc_firsthalf", "nbk_calc_firsthalf_dev", "nbk_calc_lasthalf", "nbk_calc_lasthalf_f64", "nbk_calc_lasthalf_dev",
     "nbk_get_neighbours", "nbk_get_neighbours_dev", "nbk_calc_batch", "nbk_calc_batch_dev",
+    "nbk_shard_gather_i_dev", "nbk_shard_calc_partial_dev", "nbk_shard_finish_dev",
     "nbk_hermite_evolve", "nbk_hermite_evolve_dev", "nbk_sync", "nbk_set_timing", "nbk_get_timing", "nbk_last_launch",
     "nbk_plan", "nbk_set_variant", "nbk_last_cuda_error", "nbk_strerror", "nbk_version",
 ]
@@ -57,6 +58,9 @@ _SIGS = {
     "nbk_calc_batch_dev": (_i32, [_vp, _i64, _vp, _vp, _vp, _vp, _vp, _f32, _u32, _vp, _vp]),
     "nbk_get_neighbours": (_i32, [_vp, _i64, _vp, _vp]),
     "nbk_get_neighbours_dev": (_i32, [_vp, _i64, _vp, _vp]),
+    "nbk_shard_gather_i_dev": (_i32, [_vp, _i64, _i64, _i64, _vp, _vp, _vp]),
+    "nbk_shard_calc_partial_dev": (_i32, [_vp, _i64, _i64, _vp, _vp, _f32, _u32, _vp]),
+    "nbk_shard_finish_dev": (_i32, [_vp, _i64, _vp, _vp, _vp, _vp]),
     "nbk_hermite_evolve": (_i32, [_vp, _i64, _vp, _vp, _vp, _f64, _f64, _f64, _f64,
                                   ctypes.POINTER(HermiteStats)]),
     "nbk_hermite_evolve_dev": (_i32, [_vp, _i64, _vp, _vp, _vp, _f64, _f64, _f64, _f64,
@@ -270,6 +274,23 @@ def nbk_get_neighbours(ctx, n_i):
 def nbk_get_neighbours_dev(ctx, n_i, nn_index=0, nn_r2=0):
     _check("nbk_get_neighbours_dev",
            load().nbk_get_neighbours_dev(ctx, n_i, nn_index or None, nn_r2 or None), ctx)
+
+
+def nbk_shard_gather_i_dev(ctx, n_local, j0, n_i, i_global, i_local, xv):
+    """All array arguments are device addresses (see include/nbk.h, j-sharding)."""
+    _check("nbk_shard_gather_i_dev",
+           load().nbk_shard_gather_i_dev(ctx, n_local, j0, n_i, i_global or None, i_local or None, xv or None), ctx)
+
+
+def nbk_shard_calc_partial_dev(ctx, n_local, n_i, i_local, xv, eps2, flags, sum64):
+    _check("nbk_shard_calc_partial_dev",
+           load().nbk_shard_calc_partial_dev(ctx, n_local, n_i, i_local or None, xv or None, float(eps2), flags,
+                                             sum64 or None), ctx)
+
+
+def nbk_shard_finish_dev(ctx, n_i, sum64, acc=0, jerk=0, pot=0):
+    _check("nbk_shard_finish_dev",
+           load().nbk_shard_finish_dev(ctx, n_i, sum64 or None, acc or None, jerk or None, pot or None), ctx)
 
 
 def nbk_hermite_evolve_dev(ctx, m, x, v, eps, t_end, eta=0.01, dt_max=1.0 / 16.0):

@@ -138,7 +138,8 @@ namespace {
 // point; d_iidx is then unused); to_host: also write the results into the mapped host buffer.
 int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iidx,
                   const float* d_xi, const float* d_vi, float eps2, uint32_t flags,
-                  const int32_t* h_inline = nullptr, bool to_host = false) {
+                  const int32_t* h_inline = nullptr, bool to_host = false,
+                  double* sum64 = nullptr) {
     if (!c->pred_valid || c->pred_nj != n_j) {
         const int rc = do_predict(c, n_j);
         if (rc != NBK_OK) return rc;
@@ -152,6 +153,7 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     if (n_i == 0) return NBK_OK;
     if (n_j == 0) {
         NBK_CUDA(c, cudaMemsetAsync(acc, 0, sizeof(float) * 7 * n_i, c->stream));
+        if (sum64) NBK_CUDA(c, cudaMemsetAsync(sum64, 0, sizeof(double) * 8 * n_i, c->stream));
         c->last_launch[7] = 0;
         return NBK_OK;
     }
@@ -177,7 +179,7 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     fa.eps2 = eps2;
     fa.d = d;
     std::memset(&fa.tail, 0, sizeof(fa.tail));
-    const bool fused = v.I == 1 && d.nit == 1 && n_i <= kFusedMaxI && c->fused_ok;
+    const bool fused = v.I == 1 && d.nit == 1 && n_i <= kFusedMaxI && c->fused_ok && !sum64;
     if (h_inline && !fused) {  // planner chose another shape: stage the indices after all
         NBK_CUDA(c, cudaEventSynchronize(c->istage_free));
         std::memcpy(c->h_istage, h_inline, sizeof(int32_t) * n_i);
@@ -226,6 +228,7 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     ra.nn_best = c->d_nn_best;
     ra.nn_tile = c->d_nn_tile;
     ra.acc = acc; ra.jerk = jerk; ra.pot = pot;
+    ra.sum64 = sum64;
     ra.d = d;
     {
         TimeScope ts(c, 3);
@@ -664,6 +667,50 @@ int nbk_calc_lasthalf_dev(nbk_ctx* c, int64_t n_i, float* acc, float* jerk, floa
     if (acc) NBK_CUDA(c, cudaMemcpyAsync(acc, c->d_result, sizeof(float) * 3 * ni, cudaMemcpyDeviceToDevice, c->stream));
     if (jerk) NBK_CUDA(c, cudaMemcpyAsync(jerk, c->d_result + 3 * ni, sizeof(float) * 3 * ni, cudaMemcpyDeviceToDevice, c->stream));
     if (pot) NBK_CUDA(c, cudaMemcpyAsync(pot, c->d_result + 6 * ni, sizeof(float) * ni, cudaMemcpyDeviceToDevice, c->stream));
+    return NBK_OK;
+}
+
+// ---- j-sharding over several GPUs -----------------
+int nbk_shard_gather_i_dev(nbk_ctx* c, int64_t n_local, int64_t j0, int64_t n_i,
+                           const int32_t* i_global, int32_t* i_local, float* xv) {
+    if (!c || n_local < 0 || n_i < 0 || j0 < 0) return NBK_EINVAL;
+    if (n_i > 0 && (!i_global || !i_local || !xv)) return NBK_EINVAL;
+    if (n_local > c->n_max || n_i > c->ni_max) return NBK_ERANGE;
+    if (n_i == 0) return NBK_OK;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    if (n_local > 0 && (!c->pred_valid || c->pred_nj != n_local)) {
+        const int rc = do_predict(c, n_local);
+        if (rc != NBK_OK) return rc;
+    }
+    ShardGatherArgs a;
+    a.j = jpred_of(c);
+    a.i_global = i_global; a.i_local = i_local; a.xv = xv;
+    a.n_i = n_i; a.j0 = j0; a.n_local = n_local;
+    NBK_CUDA(c, launch_shard_gather(a, c->stream));
+    return NBK_OK;
+}
+
+int nbk_shard_calc_partial_dev(nbk_ctx* c, int64_t n_local, int64_t n_i, const int32_t* i_local,
+                               const float* xv, float eps2, uint32_t flags, double* sum64) {
+    if (!c || n_local < 0 || n_i < 0 || !(eps2 >= 0.f)) return NBK_EINVAL;
+    if (flags & NBK_NN) return NBK_EINVAL;   // the neighbour search is per shard: not combined here
+    if (n_i > 0 && (!i_local || !xv || !sum64)) return NBK_EINVAL;
+    if (n_local > c->n_max || n_i > c->ni_max) return NBK_ERANGE;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    NBK_CUDA(c, launch_shard_split(xv, n_i, c->d_xi, c->d_vi, c->stream));
+    return enqueue_force(c, n_local, n_i, i_local, c->d_xi, c->d_vi, eps2, flags, nullptr, false,
+                         sum64);
+}
+
+int nbk_shard_finish_dev(nbk_ctx* c, int64_t n_i, const double* sum64, float* acc, float* jerk,
+                         float* pot) {
+    if (!c || n_i < 0) return NBK_EINVAL;
+    if (n_i > 0 && !sum64) return NBK_EINVAL;
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    NBK_CUDA(c, launch_shard_finish(sum64, n_i, acc, jerk, pot, c->stream));
     return NBK_OK;
 }
 

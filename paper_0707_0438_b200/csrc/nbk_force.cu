@@ -487,6 +487,11 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
         a.jerk[3 * i + 0] = static_cast<float>(sh[4][tid]);
         a.jerk[3 * i + 1] = static_cast<float>(sh[5][tid]);
         a.jerk[3 * i + 2] = static_cast<float>(sh[6][tid]);
+        if (a.sum64) {   // j-shard: the caller adds the ranks' sums before the one rounding
+#pragma unroll
+            for (int v = 0; v < 7; ++v) a.sum64[8 * i + v] = sh[v][tid];
+            a.sum64[8 * i + 7] = 0.0;
+        }
     }
     __syncthreads();   // shared arrays are reused by the next block of i-particles
     }

@@ -134,6 +134,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     r.partial = c->d_partial;
     r.acc = f.tail.acc; r.jerk = f.tail.jerk; r.pot = f.tail.pot;
     r.dyn = c->d_hdr;
+    r.sum64 = nullptr;
     r.n_j = static_cast<int>(n);
     // the four launches of a block step are captured once into a CUDA graph and replayed
     const int kBatch = 256;

@@ -181,6 +181,7 @@ struct ReduceArgs {
     float* acc;   // [n_i][3]
     float* jerk;  // [n_i][3]
     float* pot;   // [n_i]
+    double* sum64;  // nullable [n_i][8]: the fp64 sums before rounding (acc3, -pot, jerk3, 0): j-shards
     Decomp d;
     const DynHeader* dyn;    // non-null: plan on the device (and return if the force kernel reduced)
     int n_j;                 // dyn only
@@ -214,6 +215,21 @@ struct NnScanArgs {
     float eps2;
 };
 cudaError_t launch_nn_scan(const NnScanArgs& a, cudaStream_t s);
+
+// j-sharding over several GPUs: nbk_shard_kernels.cu
+struct ShardGatherArgs {
+    JPred j;                  // this rank's predicted j-state (addresses are local)
+    const int32_t* i_global;  // [n_i] global j address of each i-particle
+    int32_t* i_local;         // [n_i] out: address in this shard, or -1 if another rank owns it
+    float* xv;                // [n_i][8] out: x y z 0 vx vy vz 0 of owned i-particles, 0 elsewhere
+    long long n_i;
+    long long j0;             // global address of local address 0
+    long long n_local;
+};
+cudaError_t launch_shard_gather(const ShardGatherArgs& a, cudaStream_t s);
+cudaError_t launch_shard_split(const float* xv, long long n_i, float* xi, float* vi, cudaStream_t s);
+cudaError_t launch_shard_finish(const double* sum64, long long n_i, float* acc, float* jerk,
+                                float* pot, cudaStream_t s);
 
 // set_j scatter: staged particles -> raw SoA at addr (nullptr: identity).  x, v as fp32 or fp64.
 struct ScatterArgs {

@@ -1,0 +1,214 @@
+"""GPU parity of the j-sharded path (include/nbk.h "j-sharding") against the
+fp64 oracle on the whole system.  The box has one GPU, so the G shards are G contexts of one
+process run one after the other (no kernel waits on another); the two all-reduces are replaced, in
+the test only, by a sum over the G buffers.  What is under test is the kernel side: ownership
+mapping, zero-filled state exchange, external i-state with the own entry left out by local address,
+fp64 partial sums, the single rounding."""
+import numpy as np
+import pytest
+
+from paper_0707_0438_b200 import binding as nb
+from paper_0707_0438_b200 import inputs
+from paper_0707_0438_b200.sharded import ShardedForce, shard_bounds
+from parity import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+EPS = inputs.EPS_PAPER
+FULL = nb.NBK_JERK | nb.NBK_POT
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests have no fallback")
+    nb.load()
+    return torch
+
+
+def run_shards(torch, world, m, x, v, eps, ii, flags=FULL, tj=None, a=None, k=None, t=0.0):
+    """G contexts on one GPU, run in turn; sums over the G buffers stand in for the all-reduces."""
+    n, n_i = m.shape[0], ii.shape[0]
+    dev = torch.device("cuda", 0)
+    ts = torch.cuda.Stream(device=dev)   # one stream for the G contexts and the torch sums between them
+    stream = ts.cuda_stream
+    ig = torch.from_numpy(ii.astype(np.int32)).to(dev)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(ts):
+        return _run_shards_on(torch, dev, stream, ig, world, m, x, v, eps, ii, flags, tj, a, k, t)
+
+
+def _run_shards_on(torch, dev, stream, ig, world, m, x, v, eps, ii, flags, tj, a, k, t):
+    n, n_i = m.shape[0], ii.shape[0]
+    ctxs, bounds = [], []
+    for r in range(world):
+        j0, j1 = shard_bounds(n, world, r)
+        c = nb.nbk_open(0, max(j1 - j0, 1), max(n_i, 1), stream)
+        if j1 > j0:
+            cut = lambda arr: None if arr is None else arr[j0:j1]
+            nb.nbk_set_j_particles(c, None, cut(tj), m[j0:j1], x[j0:j1], v[j0:j1], cut(a), cut(k))
+        nb.nbk_set_ti(c, t)
+        ctxs.append(c)
+        bounds.append((j0, j1))
+    try:
+        il = [torch.empty(n_i, dtype=torch.int32, device=dev) for _ in range(world)]
+        xv = [torch.empty((n_i, 8), dtype=torch.float32, device=dev) for _ in range(world)]
+        for r, c in enumerate(ctxs):
+            j0, j1 = bounds[r]
+            nb.nbk_shard_gather_i_dev(c, j1 - j0, j0, n_i, ig.data_ptr(), il[r].data_ptr(), xv[r].data_ptr())
+        owners = torch.stack([(t_ >= 0).to(torch.int32) for t_ in il]).sum(0)
+        assert bool((owners == 1).all()), "every i-particle has exactly one owner"
+        xv_all = torch.stack(xv).sum(0).contiguous()       # stands in for all-reduce #1
+        s64 = [torch.empty((n_i, 8), dtype=torch.float64, device=dev) for _ in range(world)]
+        for r, c in enumerate(ctxs):
+            j0, j1 = bounds[r]
+            nb.nbk_shard_calc_partial_dev(c, j1 - j0, n_i, il[r].data_ptr(), xv_all.data_ptr(),
+                                          np.float32(eps) ** 2, flags, s64[r].data_ptr())
+        tot = torch.stack(s64).sum(0).contiguous()         # stands in for all-reduce #2
+        acc = torch.empty((n_i, 3), dtype=torch.float32, device=dev)
+        jerk = torch.empty((n_i, 3), dtype=torch.float32, device=dev)
+        pot = torch.empty(n_i, dtype=torch.float32, device=dev)
+        nb.nbk_shard_finish_dev(ctxs[0], n_i, tot.data_ptr(), acc.data_ptr(), jerk.data_ptr(), pot.data_ptr())
+        torch.cuda.synchronize()
+        return acc.cpu().numpy(), jerk.cpu().numpy(), pot.cpu().numpy(), xv_all.cpu().numpy()
+    finally:
+        for c in ctxs:
+            nb.nbk_close(c)
+
+
+@pytest.mark.parametrize("world", [1, 2, 3, 8])
+@pytest.mark.parametrize("n,n_i", [(16384, 16384), (16384, 37), (4099, 1031)])
+def test_sharded_parity_vs_whole_system_oracle(gpu, c_oracle, world, n, n_i):
+    m, x, v = inputs.plummer_f32(n, 2)
+    ii = np.arange(n, dtype=np.int32) if n_i == n else inputs.active_block(n, n_i, 21)
+    ref = c_oracle.force(m, x, v, EPS, i_index=ii)
+    acc, jerk, pot, xv = run_shards(gpu, world, m, x, v, EPS, ii)
+    assert np.array_equal(xv[:, 0:3], x[ii]) and np.array_equal(xv[:, 4:7], v[ii])   # exact copy
+    assert_parity((acc, jerk, pot), ref, what=f"sharded G={world} n={n} n_i={n_i}")
+
+
+def test_sharded_eps0_and_acc_only(gpu, c_oracle):
+    n = 8192
+    m, x, v = inputs.plummer_f32(n, 7)
+    ii = inputs.active_block(n, 2048, 22)
+    ref = c_oracle.force(m, x, v, 0.0, i_index=ii)
+    acc, jerk, pot, _ = run_shards(gpu, 4, m, x, v, 0.0, ii, flags=FULL | nb.NBK_EPS0)
+    assert_parity((acc, jerk, pot), ref, what="sharded eps=0")
+    ref = c_oracle.force(m, x, v, EPS, i_index=ii, want_jerk=False)
+    acc, jerk, pot, _ = run_shards(gpu, 4, m, x, v, EPS, ii, flags=nb.NBK_POT)
+    assert_parity((acc, jerk, pot), ref, jerk=False, what="sharded acc+pot")
+    assert not jerk.any()
+
+
+def test_sharded_with_prediction_and_more_ranks_than_particles(gpu, c_oracle):
+    """Predicted state is what is exchanged; shards may be empty (G > n)."""
+    n, t = 5, 0.01
+    m, x, v = inputs.plummer_f32(n, 9)
+    a, k = inputs.gaussian_derivatives(n, 10)
+    tj = inputs.particle_times(n, t, 11)
+    ii = np.arange(n, dtype=np.int32)
+    xp, vp = c_oracle.predict(t, tj, x, v, a, k)
+    xp, vp = xp.astype(np.float32), vp.astype(np.float32)
+    ref = c_oracle.force(m, xp, vp, EPS, i_index=ii)
+    acc, jerk, pot, xv = run_shards(gpu, 8, m, x, v, EPS, ii, tj=tj, a=a, k=k, t=t)
+    assert np.max(np.abs(xv[:, 0:3] - xp)) <= 1.2e-7 * np.max(np.abs(xp))
+    assert_parity((acc, jerk, pot), ref, what="sharded G=8 n=5")
+
+
+def test_sharded_world1_class_equals_plain_path_bitwise(gpu, c_oracle):
+    """ShardedForce at world size 1 (no collective): same bits as firsthalf/lasthalf, because the
+    fp64 sums are rounded once either way."""
+    n, n_i = 16384, 2048
+    m, x, v = inputs.plummer_f32(n, 2)
+    ii = inputs.active_block(n, n_i, 23)
+    sf = ShardedForce(n, n_i, device=0)
+    try:
+        assert (sf.world, sf.j0, sf.j1) == (1, 0, n)
+        sf.set_j_particles(None, None, m, x, v)
+        sf.set_ti(0.0)
+        ig = gpu.from_numpy(ii).to("cuda:0")
+        acc, jerk, pot = sf.calc(ig, np.float32(EPS) ** 2)
+        gpu.cuda.synchronize()
+        got = (acc.cpu().numpy(), jerk.cpu().numpy(), pot.cpu().numpy())
+        assert sf.collectives == 0
+    finally:
+        sf.close()
+    c = nb.nbk_open(0, n, n_i)
+    try:
+        nb.nbk_set_j_particles(c, None, None, m, x, v)
+        nb.nbk_set_ti(c, 0.0)
+        nb.nbk_calc_firsthalf(c, n, n_i, ii, None, None, np.float32(EPS) ** 2, FULL)
+        plain = nb.nbk_calc_lasthalf(c, n_i)
+    finally:
+        nb.nbk_close(c)
+    for g, p in zip(got, plain):
+        assert np.array_equal(g, p)
+    assert_parity(got, c_oracle.force(m, x, v, EPS, i_index=ii), what="ShardedForce world 1")
+
+
+NCCL_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+import numpy as np, torch
+import torch.distributed as dist
+from paper_0707_0438_b200 import binding as nb, inputs
+from paper_0707_0438_b200.sharded import ShardedForce
+torch.cuda.set_device(0)
+dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+n, n_i = 16384, 4096
+m, x, v = inputs.plummer_f32(n, 2)
+ii = inputs.active_block(n, n_i, 24)
+e2 = float(np.float32(inputs.EPS_PAPER) ** 2)
+sf = ShardedForce(n, n_i, device=0, always_reduce=True)
+sf.set_j_particles(None, None, m, x, v)
+sf.set_ti(0.0)
+ig = torch.from_numpy(ii).to("cuda:0")
+outs = [tuple(t.clone() for t in sf.calc(ig, e2)) for _ in range(3)]
+torch.cuda.synchronize()
+assert sf.collectives == 6
+c = nb.nbk_open(0, n, n_i)
+nb.nbk_set_j_particles(c, None, None, m, x, v)
+nb.nbk_set_ti(c, 0.0)
+nb.nbk_calc_firsthalf(c, n, n_i, ii, None, None, e2, nb.NBK_JERK | nb.NBK_POT)
+plain = nb.nbk_calc_lasthalf(c, n_i)
+nb.nbk_close(c)
+for o in outs:
+    for g, p in zip(o, plain):
+        assert np.array_equal(g.cpu().numpy(), p)
+sf.close()
+dist.destroy_process_group()
+print("NCCL_OK")
+"""
+
+
+def test_sharded_class_with_nccl_collectives_at_world1(gpu, tmp_path):
+    """The real collectives (NCCL all-reduce of fp32 state and fp64 sums on the library's stream) at
+    world size 1, where a sum over ranks is the identity: results equal the plain path bit for bit."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "nccl_worker.py"
+    script.write_text(NCCL_WORKER.format(root=root))
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29541", RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
+    p = subprocess.run([sys.executable, str(script)], env=env, capture_output=True, text=True, timeout=600)
+    assert p.returncode == 0 and "NCCL_OK" in p.stdout, p.stdout + p.stderr
+
+
+def test_sharded_refused_calls(gpu):
+    c = nb.nbk_open(0, 64, 64)
+    try:
+        buf = gpu.zeros(64 * 8, dtype=gpu.float64, device="cuda:0")
+        with pytest.raises(nb.NbkError) as e:
+            nb.nbk_shard_calc_partial_dev(c, 64, 8, buf.data_ptr(), buf.data_ptr(), 0.0, FULL | nb.NBK_NN,
+                                          buf.data_ptr())
+        assert e.value.status == nb.NBK_EINVAL
+        with pytest.raises(nb.NbkError) as e:
+            nb.nbk_shard_gather_i_dev(c, 65, 0, 8, buf.data_ptr(), buf.data_ptr(), buf.data_ptr())
+        assert e.value.status == nb.NBK_ERANGE
+        with pytest.raises(nb.NbkError) as e:
+            nb.nbk_shard_calc_partial_dev(c, 64, 8, 0, buf.data_ptr(), 0.0, FULL, buf.data_ptr())
+        assert e.value.status == nb.NBK_EINVAL
+    finally:
+        nb.nbk_close(c)
