@@ -498,6 +498,35 @@ def run_sweep(args):
         ra = n * n / (accp * 1e-3)
         print(f"| {n} | {full:.4f} | {r:.3e} | {42 * r / 1e12:.2f} | {100 * 42 * r / peak:.1f} | {60 * r / 1e12:.2f} | "
               f"{accp:.4f} | {ra:.3e} | {20 * ra / 1e12:.2f} | {e0:.4f} | {nn:.4f} |", flush=True)
+    # a3 predictor (HBM-bound: 72 B read + 28 B written per particle)
+    hbm_peak = 6549.1
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            hbm_peak = float(json.load(f)["hbm_gbs"])
+    except Exception:
+        pass
+    print()
+    print(f"| N | predict_kernel us | GB/s (100 B per particle) | fraction of measured HBM copy peak ({hbm_peak:.0f} GB/s) |")
+    print("|---|---|---|---|")
+    for n in (131072, 1048576, 4194304):
+        rng = np.random.default_rng(n)
+        m = np.full(n, 1.0 / n, np.float32)
+        x = rng.standard_normal((n, 3)).astype(np.float32)
+        v = rng.standard_normal((n, 3)).astype(np.float32)
+        ctx = nb.nbk_open(0, n, 1024)
+        try:
+            nb.nbk_set_j_particles(ctx, None, np.zeros(n), m, x, v, v, v)
+            nb.nbk_set_timing(ctx, True)
+            ts = []
+            for q in range(12):
+                nb.nbk_set_ti(ctx, 1e-3 * (q + 1))
+                nb.nbk_predict(ctx, n)
+                ts.append(nb.nbk_get_timing(ctx)["predict"])
+            us = float(np.median(ts[2:])) * 1e3
+        finally:
+            nb.nbk_close(ctx)
+        gbs = 100.0 * n / (us * 1e-6) / 1e9
+        print(f"| {n} | {us:.1f} | {gbs:.0f} | {gbs / hbm_peak:.2f} |", flush=True)
     # launch + synchronise floor of this box: one 1-particle predictor launch and a stream sync
     ctx = nb.nbk_open(0, 256, 256)
     try:
