@@ -498,6 +498,36 @@ def run_sweep(args):
         ra = n * n / (accp * 1e-3)
         print(f"| {n} | {full:.4f} | {r:.3e} | {42 * r / 1e12:.2f} | {100 * 42 * r / peak:.1f} | {60 * r / 1e12:.2f} | "
               f"{accp:.4f} | {ra:.3e} | {20 * ra / 1e12:.2f} | {e0:.4f} | {nn:.4f} |", flush=True)
+    # Small N: one call's events include ~7 us of launch and event overhead (NBK_TRACE in-kernel spans are
+    # that much shorter), so also time 32 calls queued back to back between two events
+    print()
+    print("| N | acc+jerk+pot, events per call us | 32 calls back to back, us per call | interactions/s (back to back) |")
+    print("|---|---|---|---|")
+    dev = torch.device("cuda", 0)
+    ts_stream = torch.cuda.Stream(device=dev)
+    for lg in range(10, 16):
+        n = 1 << lg
+        m, x, v = inputs.plummer_f32(n, seeds.get(n, 100 + lg))
+        ctx = nb.nbk_open(0, n, n, ts_stream.cuda_stream)
+        try:
+            nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+            nb.nbk_set_ti(ctx, 0.0)
+            nb.nbk_set_timing(ctx, True)
+            single = kernel_ms(ctx, n, n, None, nb.NBK_JERK | nb.NBK_POT, eps2, 9)
+            nb.nbk_set_timing(ctx, False)
+            per = []
+            for rep in range(5):
+                e0_, e1_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0_.record(ts_stream)
+                for q in range(32):
+                    nb.nbk_calc_firsthalf_dev(ctx, n, n, 0, 0, 0, eps2, nb.NBK_JERK | nb.NBK_POT)
+                e1_.record(ts_stream)
+                ts_stream.synchronize()
+                per.append(e0_.elapsed_time(e1_) / 32.0)
+            b2b = float(np.median(per[1:]))
+        finally:
+            nb.nbk_close(ctx)
+        print(f"| {n} | {single * 1e3:.1f} | {b2b * 1e3:.1f} | {n * n / (b2b * 1e-3):.3e} |", flush=True)
     # a3 predictor (HBM-bound: 72 B read + 28 B written per particle)
     hbm_peak = 6549.1
     try:

@@ -18,6 +18,14 @@ using namespace nbk;
 
 namespace nbk {
 
+bool pdl_enabled() {
+    static const bool on = [] {
+        const char* e = std::getenv("NBK_PDL");
+        return !(e && e[0] == '0');
+    }();
+    return on;
+}
+
 int cuda_fail(nbk_ctx* c, cudaError_t e) {
     c->last_cuda = static_cast<int>(e);
     (void)cudaGetLastError();

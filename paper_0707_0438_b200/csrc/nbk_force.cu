@@ -60,6 +60,8 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
     float* snn_best = reinterpret_cast<float*>(sacc + NACC * I * T);   // [I][T]
     int* snn_tile = reinterpret_cast<int*>(snn_best + I * T);          // [I][T]
 
+    pdl_trigger();
+    pdl_wait();   // before anything the predictor (or the step header) wrote is read
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const int warp = tid >> 5;
@@ -401,6 +403,8 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
     __shared__ int sht[NN ? 256 : 1];
     __shared__ int krange[2];
     __shared__ int s_first[kMaxCtas], s_last[kMaxCtas];
+    pdl_trigger();
+    pdl_wait();   // every thread, also those of a launch that returns at once (the successor waits on us)
     Decomp dplan = a.d;
     if (a.dyn) {   // device-resident integrator: same plan as the force kernel made
         if (a.dyn->done || a.dyn->n_act <= 0 || a.dyn->fused) return;   // fused: already reduced
@@ -499,6 +503,8 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
 
 // One warp per i-particle: find the index inside the winning tile (two-kernel path).
 __global__ void __launch_bounds__(256) nn_scan_kernel(const NnScanArgs a) {
+    pdl_trigger();
+    pdl_wait();
     const int lane = threadIdx.x & 31;
     const int i = blockIdx.x * 8 + (threadIdx.x >> 5);
     if (i >= a.n_i) return;
@@ -544,13 +550,11 @@ static cudaError_t launch_of(const ForceArgs& a, bool nn, cudaStream_t s) {
     const size_t smem = smem_bytes_of<I, JERK>();
     if constexpr (JERK && PACKED) {
         if (nn) {
-            force_kernel<I, JERK, EPS0, PACKED, true><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
-            return cudaGetLastError();
+            return launch_pdl(force_kernel<I, JERK, EPS0, PACKED, true>, a.d.G, warps_of(I) * 32, smem, s, a);
         }
     }
     if (nn) return cudaErrorInvalidValue;
-    force_kernel<I, JERK, EPS0, PACKED, false><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
-    return cudaGetLastError();
+    return launch_pdl(force_kernel<I, JERK, EPS0, PACKED, false>, a.d.G, warps_of(I) * 32, smem, s, a);
 }
 
 #define NBK_DISPATCH(CALL, ...)                                                         \
@@ -602,25 +606,22 @@ cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s)
     while (ix_log2 > 0 && (1 << (ix_log2 - 1)) >= a.d.n_i) --ix_log2;
     const int ix = 1 << ix_log2;
     const unsigned grid = static_cast<unsigned>((a.d.n_i + ix - 1) / ix);
-    if (v.jerk && v.nn) reduce_kernel<true, true><<<grid, 256, 0, s>>>(a, ix_log2);
-    else if (v.jerk) reduce_kernel<true, false><<<grid, 256, 0, s>>>(a, ix_log2);
-    else reduce_kernel<false, false><<<grid, 256, 0, s>>>(a, ix_log2);
-    return cudaGetLastError();
+    if (v.jerk && v.nn) return launch_pdl(reduce_kernel<true, true>, grid, 256, 0, s, a, ix_log2);
+    if (v.jerk) return launch_pdl(reduce_kernel<true, false>, grid, 256, 0, s, a, ix_log2);
+    return launch_pdl(reduce_kernel<false, false>, grid, 256, 0, s, a, ix_log2);
 }
 
 
 cudaError_t launch_reduce_dyn(const Variant& v, const ReduceArgs& a, int ni_max, cudaStream_t s) {
     unsigned grid = static_cast<unsigned>((ni_max + 31) / 32);
     if (grid > 296) grid = 296;   // grid-stride: most steps return at once (reduced by the force kernel)
-    if (v.jerk) reduce_kernel<true, false><<<grid, 256, 0, s>>>(a, 5);
-    else reduce_kernel<false, false><<<grid, 256, 0, s>>>(a, 5);
-    return cudaGetLastError();
+    if (v.jerk) return launch_pdl(reduce_kernel<true, false>, grid, 256, 0, s, a, 5);
+    return launch_pdl(reduce_kernel<false, false>, grid, 256, 0, s, a, 5);
 }
 
 cudaError_t launch_nn_scan(const NnScanArgs& a, cudaStream_t s) {
     if (a.n_i <= 0) return cudaSuccess;
-    nn_scan_kernel<<<(a.n_i + 7) / 8, 256, 0, s>>>(a);
-    return cudaGetLastError();
+    return launch_pdl(nn_scan_kernel, static_cast<unsigned>((a.n_i + 7) / 8), 256, 0, s, a);
 }
 
 

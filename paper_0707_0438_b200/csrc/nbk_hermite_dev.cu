@@ -136,7 +136,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     r.dyn = c->d_hdr;
     r.sum64 = nullptr;
     r.n_j = static_cast<int>(n);
-    // the four launches of a block step are captured once into a CUDA graph and replayed
+    // the four launches of a block step are captured into a CUDA graph and replayed
     const int kBatch = 256;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t gexec = nullptr;
@@ -151,8 +151,12 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
         return launch_hd_correct(c->raw, c->d_hdr, c->hs, f.tail.acc, f.tail.jerk,
                                  static_cast<int>(n), c->stream);
     };
+    // kStepsPerGraph steps per graph: inside a graph consecutive kernels are joined by programmatic
+    // dependent-launch edges (nbk_kernels.cuh), between graph launches the stream serialises fully
+    const int kStepsPerGraph = 8;
     NBK_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
-    cudaError_t ce = enqueue_step();
+    cudaError_t ce = cudaSuccess;
+    for (int s = 0; s < kStepsPerGraph && ce == cudaSuccess; ++s) ce = enqueue_step();
     cudaError_t ce2 = cudaStreamEndCapture(c->stream, &graph);
     if (ce != cudaSuccess || ce2 != cudaSuccess) {
         if (graph) cudaGraphDestroy(graph);
@@ -161,7 +165,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     ce = cudaGraphInstantiate(&gexec, graph, 0);
     if (ce != cudaSuccess) { cudaGraphDestroy(graph); return cuda_fail(c, ce); }
     for (;;) {
-        for (int s = 0; s < kBatch && ce == cudaSuccess; ++s) ce = cudaGraphLaunch(gexec, c->stream);
+        for (int s = 0; s < kBatch / kStepsPerGraph && ce == cudaSuccess; ++s) ce = cudaGraphLaunch(gexec, c->stream);
         if (ce == cudaSuccess)
             ce = cudaMemcpyAsync(c->h_hdr, c->d_hdr, sizeof(DynHeader), cudaMemcpyDeviceToHost, c->stream);
         if (ce == cudaSuccess) ce = cudaStreamSynchronize(c->stream);

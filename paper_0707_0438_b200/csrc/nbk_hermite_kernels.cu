@@ -67,6 +67,8 @@ __device__ void hd_begin_body(DynHeader* h) {
 }
 
 __global__ void hd_begin_kernel(DynHeader* h) {   // one CTA of 64 threads
+    pdl_trigger();
+    pdl_wait();
     hd_begin_body(h);
 }
 
@@ -78,6 +80,8 @@ __global__ void __launch_bounds__(256) hd_predict_kernel(const RawJ raw, DynHead
                                                          float* px, float* py, float* pz, float* pm,
                                                          float* pvx, float* pvy, float* pvz) {
     __shared__ int red[8];
+    pdl_trigger();
+    pdl_wait();
     __shared__ int wsum[8];
     if (h->done) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -142,6 +146,8 @@ __device__ __forceinline__ int level_for_dev(double want, int kmin) {
 // writes the fp64 state, the level lists' counts and the raw j-state the predictor reads.
 __global__ void hd_correct_kernel(const RawJ raw, DynHeader* h, const HermiteState hs,
                                   const float* acc, const float* jerk) {
+    pdl_trigger();
+    pdl_wait();
     if (h->done) return;
     const int n_act = h->n_act;
     for (int q = blockIdx.x * blockDim.x + threadIdx.x; q < n_act; q += gridDim.x * blockDim.x) {
@@ -224,24 +230,21 @@ __global__ void hd_correct_kernel(const RawJ raw, DynHeader* h, const HermiteSta
 
 
 cudaError_t launch_hd_begin(DynHeader* h, cudaStream_t st) {
-    hd_begin_kernel<<<1, 64, 0, st>>>(h);
-    return cudaGetLastError();
+    return launch_pdl(hd_begin_kernel, 1, 64, 0, st, h);
 }
 
 cudaError_t launch_hd_predict(const RawJ& raw, DynHeader* h, const HermiteState& hs, long long n_pad,
                               float* px, float* py, float* pz, float* pm, float* pvx, float* pvy,
                               float* pvz, cudaStream_t st) {
     const unsigned grid = static_cast<unsigned>((n_pad + 255) / 256);
-    hd_predict_kernel<<<grid, 256, 0, st>>>(raw, h, hs, n_pad, px, py, pz, pm, pvx, pvy, pvz);
-    return cudaGetLastError();
+    return launch_pdl(hd_predict_kernel, grid, 256, 0, st, raw, h, hs, n_pad, px, py, pz, pm, pvx, pvy, pvz);
 }
 
 cudaError_t launch_hd_correct(const RawJ& raw, DynHeader* h, const HermiteState& hs, const float* acc,
                               const float* jerk, int n, cudaStream_t st) {
     int grid = (n + 127) / 128;
     if (grid > 64) grid = 64;   // grid-stride over the due particles; most steps hold a handful
-    hd_correct_kernel<<<grid, 128, 0, st>>>(raw, h, hs, acc, jerk);
-    return cudaGetLastError();
+    return launch_pdl(hd_correct_kernel, static_cast<unsigned>(grid), 128, 0, st, raw, h, hs, acc, jerk);
 }
 
 

@@ -14,6 +14,36 @@ constexpr int kMaxI = 4;        // max i-particles per thread
 constexpr int kMaxRowI = 1024;  // max (warps * 32 * I): i-rows one CTA writes per (segment)
 constexpr int kMaxCtas = 256;   // max CTAs of a force launch (one per SM; B200 has 148)
 
+// ---- programmatic dependent launch (sm_90+).  A block step is a chain of short kernels (predict ->
+// force -> reduce -> correct): each kernel of the chain is launched with programmatic stream
+// serialisation, lets its successor be scheduled as soon as all of its own CTAs are resident
+// (pdl_trigger at entry) and waits for its predecessor's completion and memory flush before it
+// touches global memory (pdl_wait).  That hides the launch and CTA-scheduling latency between
+// dependent kernels (2-3 us per edge), which is what a small block step is made of.
+// Without the launch attribute both instructions do nothing.  NBK_PDL=0 in the environment turns
+// the attribute off.
+bool pdl_enabled();
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem,
+                              cudaStream_t s, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = pdl_enabled() ? 1 : 0;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+#endif
+
 // warps per CTA for each i-per-thread count: one CTA per SM, registers decide the warp count
 __host__ __device__ constexpr int warps_of(int I) { return I == 4 ? 8 : (I == 2 ? 12 : 16); }
 

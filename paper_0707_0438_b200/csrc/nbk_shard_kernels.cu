@@ -12,6 +12,8 @@
 namespace nbk {
 
 __global__ void __launch_bounds__(256) shard_gather_kernel(const ShardGatherArgs a) {
+    pdl_trigger();
+    pdl_wait();
     const long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (k >= a.n_i) return;
     const long long l = static_cast<long long>(a.i_global[k]) - a.j0;
@@ -29,6 +31,8 @@ __global__ void __launch_bounds__(256) shard_gather_kernel(const ShardGatherArgs
 
 __global__ void __launch_bounds__(256) shard_split_kernel(const float* xv, long long n_i, float* xi,
                                                           float* vi) {
+    pdl_trigger();
+    pdl_wait();
     const long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (k >= n_i) return;
     const float4* s = reinterpret_cast<const float4*>(xv + 8 * k);
@@ -40,6 +44,8 @@ __global__ void __launch_bounds__(256) shard_split_kernel(const float* xv, long 
 // sum64 row: acc(3), -pot, jerk(3), 0 -- the layout reduce_kernel writes
 __global__ void __launch_bounds__(256) shard_finish_kernel(const double* sum64, long long n_i,
                                                            float* acc, float* jerk, float* pot) {
+    pdl_trigger();
+    pdl_wait();
     const long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (k >= n_i) return;
     const double* s = sum64 + 8 * k;
@@ -60,22 +66,19 @@ static unsigned grid_of(long long n) { return static_cast<unsigned>((n + 255) / 
 
 cudaError_t launch_shard_gather(const ShardGatherArgs& a, cudaStream_t s) {
     if (a.n_i <= 0) return cudaSuccess;
-    shard_gather_kernel<<<grid_of(a.n_i), 256, 0, s>>>(a);
-    return cudaGetLastError();
+    return launch_pdl(shard_gather_kernel, grid_of(a.n_i), 256, 0, s, a);
 }
 
 cudaError_t launch_shard_split(const float* xv, long long n_i, float* xi, float* vi,
                                cudaStream_t s) {
     if (n_i <= 0) return cudaSuccess;
-    shard_split_kernel<<<grid_of(n_i), 256, 0, s>>>(xv, n_i, xi, vi);
-    return cudaGetLastError();
+    return launch_pdl(shard_split_kernel, grid_of(n_i), 256, 0, s, xv, n_i, xi, vi);
 }
 
 cudaError_t launch_shard_finish(const double* sum64, long long n_i, float* acc, float* jerk,
                                 float* pot, cudaStream_t s) {
     if (n_i <= 0) return cudaSuccess;
-    shard_finish_kernel<<<grid_of(n_i), 256, 0, s>>>(sum64, n_i, acc, jerk, pot);
-    return cudaGetLastError();
+    return launch_pdl(shard_finish_kernel, grid_of(n_i), 256, 0, s, sum64, n_i, acc, jerk, pot);
 }
 
 }  // namespace nbk

@@ -6,6 +6,8 @@ namespace nbk {
 // ------------------------------------------------------------------ scatter (a1) / predict (a3)
 template <typename T>
 __global__ void scatter_kernel(const ScatterArgs s, const RawJ raw) {
+    pdl_trigger();
+    pdl_wait();
     const long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (k >= s.n) return;
     const long long ad = s.addr ? static_cast<long long>(s.addr[k]) : k;
@@ -31,6 +33,8 @@ __global__ void scatter_kernel(const ScatterArgs s, const RawJ raw) {
 __global__ void predict_kernel(const RawJ raw, double t, long long n_j, long long n_pad, float* px,
                                float* py, float* pz, float* pm, float* pvx, float* pvy,
                                float* pvz) {
+    pdl_trigger();
+    pdl_wait();
     const long long j = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (j >= n_pad) return;
     // padding (n_j <= j < n_pad): massless and far away, so that it is nobody's neighbour
@@ -58,6 +62,8 @@ __global__ void predict_kernel(const RawJ raw, double t, long long n_j, long lon
 __global__ void predict_upd_kernel(const RawJ raw, double t, long long n_j, long long n_pad,
                                    float* px, float* py, float* pz, float* pm, float* pvx,
                                    float* pvy, float* pvz, const InlineJ upd) {
+    pdl_trigger();
+    pdl_wait();
     const long long j = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (j >= n_pad) return;
     // padding (n_j <= j < n_pad): massless and far away, so that it is nobody's neighbour
@@ -101,6 +107,8 @@ __global__ void predict_upd_kernel(const RawJ raw, double t, long long n_j, long
 
 
 __global__ void scatter_inline_kernel(const InlineJ p, const RawJ raw) {
+    pdl_trigger();
+    pdl_wait();
     const int k = threadIdx.x;
     if (k >= p.n) return;
     const long long ad = p.addr[k];
@@ -117,16 +125,14 @@ __global__ void scatter_inline_kernel(const InlineJ p, const RawJ raw) {
 
 cudaError_t launch_scatter_inline(const InlineJ& p, const RawJ& raw, cudaStream_t st) {
     if (p.n <= 0) return cudaSuccess;
-    scatter_inline_kernel<<<1, kInlineMaxJ, 0, st>>>(p, raw);
-    return cudaGetLastError();
+    return launch_pdl(scatter_inline_kernel, 1, kInlineMaxJ, 0, st, p, raw);
 }
 
 cudaError_t launch_scatter(const ScatterArgs& s, const RawJ& raw, cudaStream_t st) {
     if (s.n <= 0) return cudaSuccess;
     const unsigned grid = static_cast<unsigned>((s.n + 255) / 256);
-    if (s.f64) scatter_kernel<double><<<grid, 256, 0, st>>>(s, raw);
-    else scatter_kernel<float><<<grid, 256, 0, st>>>(s, raw);
-    return cudaGetLastError();
+    if (s.f64) return launch_pdl(scatter_kernel<double>, grid, 256, 0, st, s, raw);
+    return launch_pdl(scatter_kernel<float>, grid, 256, 0, st, s, raw);
 }
 
 cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n_pad, float* px,
@@ -135,10 +141,9 @@ cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n
     if (n_pad <= 0) return cudaSuccess;
     const unsigned grid = static_cast<unsigned>((n_pad + 255) / 256);
     if (upd && upd->n > 0)
-        predict_upd_kernel<<<grid, 256, 0, st>>>(raw, t, n_j, n_pad, px, py, pz, pm, pvx, pvy, pvz, *upd);
-    else
-        predict_kernel<<<grid, 256, 0, st>>>(raw, t, n_j, n_pad, px, py, pz, pm, pvx, pvy, pvz);
-    return cudaGetLastError();
+        return launch_pdl(predict_upd_kernel, grid, 256, 0, st, raw, t, n_j, n_pad, px, py, pz, pm, pvx, pvy,
+                          pvz, *upd);
+    return launch_pdl(predict_kernel, grid, 256, 0, st, raw, t, n_j, n_pad, px, py, pz, pm, pvx, pvy, pvz);
 }
 
 
