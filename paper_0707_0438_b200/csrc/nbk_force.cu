@@ -60,8 +60,13 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
     float* snn_best = reinterpret_cast<float*>(sacc + NACC * I * T);   // [I][T]
     int* snn_tile = reinterpret_cast<int*>(snn_best + I * T);          // [I][T]
 
-    pdl_trigger();
-    pdl_wait();   // before anything the predictor (or the step header) wrote is read
+    // Small-block form only (I == 1: block steps, the device-resident integrator): the I = 2 and 4
+    // forms run for milliseconds, are launched without the attribute, and their code is left as it
+    // was (two more instructions ahead of the tile loop cost 1 % at C3 -- code placement).
+    if constexpr (I == 1) {
+        pdl_trigger();
+        pdl_wait();   // before anything the predictor (or the step header) wrote is read
+    }
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const int warp = tid >> 5;
@@ -550,11 +555,17 @@ static cudaError_t launch_of(const ForceArgs& a, bool nn, cudaStream_t s) {
     const size_t smem = smem_bytes_of<I, JERK>();
     if constexpr (JERK && PACKED) {
         if (nn) {
-            return launch_pdl(force_kernel<I, JERK, EPS0, PACKED, true>, a.d.G, warps_of(I) * 32, smem, s, a);
+            if constexpr (I == 1)
+                return launch_pdl(force_kernel<I, JERK, EPS0, PACKED, true>, a.d.G, warps_of(I) * 32, smem, s, a);
+            force_kernel<I, JERK, EPS0, PACKED, true><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
+            return cudaGetLastError();
         }
     }
     if (nn) return cudaErrorInvalidValue;
-    return launch_pdl(force_kernel<I, JERK, EPS0, PACKED, false>, a.d.G, warps_of(I) * 32, smem, s, a);
+    if constexpr (I == 1)
+        return launch_pdl(force_kernel<I, JERK, EPS0, PACKED, false>, a.d.G, warps_of(I) * 32, smem, s, a);
+    force_kernel<I, JERK, EPS0, PACKED, false><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
+    return cudaGetLastError();
 }
 
 #define NBK_DISPATCH(CALL, ...)                                                         \
