@@ -389,7 +389,9 @@ def run_sharded(args, wl):
     n = m.shape[0]
     eps2 = float(np.float32(eps) ** 2)
     flags = (nb.NBK_JERK if jerk else 0) | nb.NBK_POT
-    sf = ShardedForce(n, n, device=local)
+    sf = ShardedForce(n, n, device=local, mode=args.shard)
+    ci = -(-n // world)   # i-particles this rank's force kernel handles
+    n_i_rank = n if args.shard == "j" else max(0, min((rank + 1) * ci, n) - min(rank * ci, n))
     try:
         sf.set_j_particles(None, None, m, x, v)
         sf.set_ti(0.0)
@@ -423,7 +425,7 @@ def run_sharded(args, wl):
         clocks = sampler.stop()
         local_ms = float(np.sum([a.elapsed_time(b) for a, b in evs]))
         # strong scaling: the job's units are N x N per step whatever G is; time = max over ranks
-        total_ms, units_sum = aggregate(local_ms, float(args.steps) * n * sf.n_local, world, str(dev))
+        total_ms, units_sum = aggregate(local_ms, float(args.steps) * n_i_rank * sf.n_local, world, str(dev))
         launch = nb.nbk_last_launch(sf.ops.ctx)
         assert bool(torch.isfinite(out[0]).all()) and bool(torch.isfinite(out[2]).all())
     finally:
@@ -435,14 +437,15 @@ def run_sharded(args, wl):
         return 0
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     peak_tflops = sm_count * 128 * 2 * 1.965e9 / 1e12
-    kint = n * sf.n_local / (float(np.mean(force_ms)) * 1e-3)
+    kint = n_i_rank * sf.n_local / (float(np.mean(force_ms)) * 1e-3)
     achieved = FLOPS_EXECUTED[jerk] * kint / 1e12
     line = {
         "metric": METRIC, "value": units_sum / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": desc, "n_i": n, "n_j": n, "parallelism": f"j-sharded x{world}",
-                   "n_j_per_rank": sf.n_local, "collectives_per_step": 2 if world > 1 else 0,
+        "config": {"workload": desc, "n_i": n, "n_j": n, "parallelism": f"{args.shard}-sharded x{world}",
+                   "n_j_per_rank": sf.n_local, "n_i_per_rank": n_i_rank,
+                   "collectives_per_step": (2 if args.shard == "j" else 3) if world > 1 else 0,
                    "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB write)", "launch": launch},
         "clocks": clocks, "gpu_launches": int(args.steps * 5),
         "roofline": {"bound": "alu", "kernel": "nbk::force_kernel (rank 0)", "achieved": achieved, "peak": peak_tflops,
@@ -611,8 +614,9 @@ def main(argv=None):
                     help="do not time the oracle (for runs under ncu); cpu_baseline is then null")
     ap.add_argument("--sweep", action="store_true",
                     help="print kernel time against N (1K..1M) and the block-step sweep as markdown tables")
-    ap.add_argument("--shard", choices=["none", "j"], default="none",
-                    help="j: shard the j-particles over the ranks with two all-reduces per step (strong scaling); "
+    ap.add_argument("--shard", choices=["none", "j", "i"], default="none",
+                    help="j: shard the j-particles over the ranks with two all-reduces per step; i: replicate j, shard "
+                         "each i-list, all-gather the results (both strong scaling); "
                          "default: independent replicas (weak)")
     args = ap.parse_args(argv)
     if args.sweep:
@@ -620,7 +624,7 @@ def main(argv=None):
     wl = WORKLOADS[args.workload]
     if args.impl == "reference":
         return run_reference(args, wl)
-    if args.shard == "j":
+    if args.shard in ("j", "i"):
         return run_sharded(args, wl)
     return run_ours(args, wl)
 

@@ -10,6 +10,10 @@ global addresses [j0_r, j1_r) in its own nbk context; a force call on a block of
     all-reduce    (NCCL)     n_i x 8 fp64 partial sums
     finish        (kernel)   one rounding to fp32
 
+mode="i" is the other cut of SURVEY.md 8(e): every rank holds all j-particles, takes a slice of
+each i-list through the ordinary firsthalf/lasthalf calls, and the result arrays are all-gathered
+(no partial sums; suited to full evaluations at large N, e.g. config C4).
+
 This module holds no arithmetic of the method: it computes the shard bounds, owns the exchange
 buffers and strings the three C-ABI calls (include/nbk.h, "j-sharding") and the two collectives
 together on one stream.  `ops` is the object that runs the three device steps; the default is
@@ -81,6 +85,12 @@ class NbkShardOps:
     def finish(self, n_i, sum64, acc, jerk, pot):
         B.nbk_shard_finish_dev(self.ctx, n_i, sum64.data_ptr(), acc.data_ptr(), jerk.data_ptr(), pot.data_ptr())
 
+    def calc_slice(self, n_j, i_index, eps2, flags, acc, jerk, pot):
+        """i-sharding: the plain firsthalf / lasthalf pair on this rank's slice of the i-list."""
+        n_i = int(i_index.shape[0])
+        B.nbk_calc_firsthalf_dev(self.ctx, n_j, n_i, i_index.data_ptr(), 0, 0, eps2, flags)
+        B.nbk_calc_lasthalf_dev(self.ctx, n_i, acc.data_ptr(), jerk.data_ptr(), pot.data_ptr())
+
     def sync(self):
         B.nbk_sync(self.ctx)
 
@@ -89,20 +99,32 @@ class ShardedForce:
     """One rank's end of the j-sharded path.  Every rank makes the same calls in the same order."""
 
     def __init__(self, n_total: int, ni_max: int, device: int = 0, group=None, ops=None,
-                 world: int | None = None, rank: int | None = None, always_reduce: bool = False):
+                 world: int | None = None, rank: int | None = None, always_reduce: bool = False,
+                 mode: str = "j"):
         live = dist.is_available() and dist.is_initialized()
         self.group = group
         self.world = world if world is not None else (dist.get_world_size(group) if live else 1)
         self.rank = rank if rank is not None else (dist.get_rank(group) if live else 0)
         if self.world > 1 and not live:
             raise RuntimeError("ShardedForce with world > 1 needs an initialised process group")
+        if mode not in ("j", "i"):
+            raise ValueError("mode must be 'j' (j-particles sharded) or 'i' (i-particles sharded, j replicated)")
+        self.mode = mode
         self.n_total, self.ni_max = int(n_total), int(ni_max)
-        self.j0, self.j1 = shard_bounds(self.n_total, self.world, self.rank)
+        # mode "i": every rank holds all j-particles and takes a slice of each i-list
+        self.j0, self.j1 = shard_bounds(self.n_total, self.world, self.rank) if mode == "j" else (0, self.n_total)
         self.n_local = self.j1 - self.j0
         self.ops = ops if ops is not None else NbkShardOps(device, self.n_local, self.ni_max)
-        self.i_local = self.ops.alloc((self.ni_max,), torch.int32)
-        self.xv = self.ops.alloc((self.ni_max, 8), torch.float32)
-        self.sum64 = self.ops.alloc((self.ni_max, 8), torch.float64)
+        if mode == "j":
+            self.i_local = self.ops.alloc((self.ni_max,), torch.int32)
+            self.xv = self.ops.alloc((self.ni_max, 8), torch.float32)
+            self.sum64 = self.ops.alloc((self.ni_max, 8), torch.float64)
+        else:   # gather buffers: world equal chunks, the last one padded
+            self.chunk_max = -(-self.ni_max // self.world)
+            rows = self.chunk_max * self.world
+            self.g_acc = self.ops.alloc((rows, 3), torch.float32)
+            self.g_jerk = self.ops.alloc((rows, 3), torch.float32)
+            self.g_pot = self.ops.alloc((rows,), torch.float32)
         self.collectives = 0   # all-reduces issued so far (for tests and bench)
         # issue the collectives at world size 1 too (needs a process group): lets a one-GPU box run
         # the NCCL calls, their dtypes and their stream ordering
@@ -146,12 +168,15 @@ class ShardedForce:
     def calc(self, i_global, eps2: float, flags: int = B.NBK_JERK | B.NBK_POT, out=None):
         """i_global: int32 tensor [n_i] of global addresses, on the ops' device, the same on every
         rank.  Returns (acc [n_i,3], jerk [n_i,3], pot [n_i]) fp32 tensors, bit-identical on every
-        rank; asynchronous on the stream for the CUDA ops."""
+        rank; asynchronous on the stream for the CUDA ops.  In mode "i" without `out` the tensors are
+        views of the gather buffers and stay valid until the next call."""
         n_i = int(i_global.shape[0])
         if n_i > self.ni_max:
             raise ValueError("calc: n_i > ni_max")
         if flags & B.NBK_NN:
             raise ValueError("calc: the neighbour search is not combined across shards")
+        if self.mode == "i" and n_i > 0:
+            return self._calc_i_sharded(i_global, n_i, float(eps2), int(flags), out)
         if out is None:
             out = (self.ops.alloc((n_i, 3), torch.float32), self.ops.alloc((n_i, 3), torch.float32),
                    self.ops.alloc((n_i,), torch.float32))
@@ -166,6 +191,38 @@ class ShardedForce:
             self.ops.calc_partial(self.n_local, n_i, il, xv, float(eps2), int(flags), s64)
             self._all_reduce(s64)
             self.ops.finish(n_i, s64, *out)
+        finally:
+            if hasattr(self.ops, "leave"):
+                self.ops.leave()
+        return out
+
+    # ---- i-sharding: j replicated, rank r takes rows [r c, (r+1) c) of the i-list,
+    # c = ceil(n_i / G); no partial sums, one all-gather of each result array
+    def _all_gather(self, full, chunk_rows):
+        if self.world > 1 or self.always_reduce:
+            parts = [full[r * chunk_rows:(r + 1) * chunk_rows] for r in range(self.world)]
+            dist.all_gather(parts, parts[self.rank], group=self.group)
+            self.collectives += 1
+
+    def _calc_i_sharded(self, i_global, n_i, eps2, flags, out):
+        c = -(-n_i // self.world)
+        lo, hi = min(self.rank * c, n_i), min((self.rank + 1) * c, n_i)
+        rows = c * self.world
+        g_acc, g_jerk, g_pot = self.g_acc[:rows], self.g_jerk[:rows], self.g_pot[:rows]
+        if hasattr(self.ops, "enter"):
+            self.ops.enter()
+        try:
+            if hi > lo:
+                sl = slice(self.rank * c, self.rank * c + (hi - lo))
+                self.ops.calc_slice(self.n_total, i_global[lo:hi], eps2, flags, g_acc[sl], g_jerk[sl], g_pot[sl])
+            for full in (g_acc, g_jerk, g_pot):
+                self._all_gather(full, c)
+            if out is None:   # views of the gather buffers: valid until the next call
+                out = (g_acc[:n_i], g_jerk[:n_i], g_pot[:n_i])
+            else:
+                out[0].copy_(g_acc[:n_i])
+                out[1].copy_(g_jerk[:n_i])
+                out[2].copy_(g_pot[:n_i])
         finally:
             if hasattr(self.ops, "leave"):
                 self.ops.leave()

@@ -177,6 +177,16 @@ for o in outs:
     for g, p in zip(o, plain):
         assert np.array_equal(g.cpu().numpy(), p)
 sf.close()
+si = ShardedForce(n, n_i, device=0, always_reduce=True, mode="i")   # i-sharding: three all-gathers per call
+si.set_j_particles(None, None, m, x, v)
+si.set_ti(0.0)
+for rep in range(2):
+    o = si.calc(ig, e2)
+    torch.cuda.synchronize()
+    for g, p in zip(o, plain):
+        assert np.array_equal(g.cpu().numpy(), p)
+assert si.collectives == 6
+si.close()
 dist.destroy_process_group()
 print("NCCL_OK")
 """
@@ -191,9 +201,37 @@ def test_sharded_class_with_nccl_collectives_at_world1(gpu, tmp_path):
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     script = tmp_path / "nccl_worker.py"
     script.write_text(NCCL_WORKER.format(root=root))
-    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29541", RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
     p = subprocess.run([sys.executable, str(script)], env=env, capture_output=True, text=True, timeout=600)
     assert p.returncode == 0 and "NCCL_OK" in p.stdout, p.stdout + p.stderr
+
+
+def test_i_sharded_world1_class_equals_plain_path_bitwise(gpu, c_oracle):
+    """mode="i" at world size 1: the slice is the whole i-list, so the results are the plain path's."""
+    n, n_i = 8192, 1000
+    m, x, v = inputs.plummer_f32(n, 4)
+    ii = inputs.active_block(n, n_i, 25)
+    sf = ShardedForce(n, n_i, device=0, mode="i")
+    try:
+        sf.set_j_particles(None, None, m, x, v)
+        sf.set_ti(0.0)
+        ig = gpu.from_numpy(ii).to("cuda:0")
+        out = (gpu.empty((n_i, 3), device="cuda:0"), gpu.empty((n_i, 3), device="cuda:0"), gpu.empty(n_i, device="cuda:0"))
+        got = sf.calc(ig, np.float32(EPS) ** 2, out=out)
+        gpu.cuda.synchronize()
+        got = tuple(t.cpu().numpy() for t in got)
+        view = sf.calc(ig, np.float32(EPS) ** 2)
+        gpu.cuda.synchronize()
+        for g, w in zip(got, view):
+            assert np.array_equal(g, w.cpu().numpy())
+        assert sf.collectives == 0
+    finally:
+        sf.close()
+    assert_parity(got, c_oracle.force(m, x, v, EPS, i_index=ii), what="i-sharded world 1")
 
 
 def test_sharded_refused_calls(gpu):

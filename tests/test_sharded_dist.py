@@ -61,6 +61,12 @@ class OracleOps:   # test stand-in for the three device steps: oracle on the loc
                                     i_index=i_local.numpy(), xi=xvn[:, 0:3], vi=xvn[:, 4:7])
             s[:, 0:3] = acc; s[:, 3] = -pot; s[:, 4:7] = jrk
         sum64.copy_(torch.from_numpy(s))
+    def calc_slice(self, n_j, i_index, eps2, flags, acc, jerk, pot):
+        xp, vp = self._pred(n_j)
+        a_, j_, p_ = O.force(self.m[:n_j].astype(np.float32), xp, vp, np.sqrt(eps2), i_index=i_index.numpy())
+        acc.copy_(torch.from_numpy(a_.astype(np.float32)))
+        jerk.copy_(torch.from_numpy(j_.astype(np.float32)))
+        pot.copy_(torch.from_numpy(p_.astype(np.float32)))
     def finish(self, n_i, sum64, acc, jerk, pot):
         s = sum64.numpy()
         acc.copy_(torch.from_numpy(s[:, 0:3].astype(np.float32)))
@@ -73,11 +79,12 @@ n, n_i, eps, t = {n}, {n_i}, 1.0 / 256.0, 0.01
 m, x, v = inputs.plummer_f32(n, 11)
 a, k = inputs.gaussian_derivatives(n, 12)
 tj = inputs.particle_times(n, t, 13)
-sf = ShardedForce(n, n_i, ops=OracleOps((n + world - 1) // world + 1))
+mode = {mode!r}
+sf = ShardedForce(n, n_i, ops=OracleOps(n + 1 if mode == "i" else (n + world - 1) // world + 1), mode=mode)
 kept = sf.set_j_particles(None, tj, m, x, v, a, k)
 sf.set_ti(t)
 ii = inputs.active_block(n, n_i, 14).astype(np.int32)
-acc, jerk, pot = sf.calc(torch.from_numpy(ii), eps * eps)
+acc, jerk, pot = (t.clone() for t in sf.calc(torch.from_numpy(ii), eps * eps))
 # a second call after updating two particles owned by different ranks (global addresses 1 and n-2)
 upd = np.array([1, n - 2])
 sf.set_j_particles(upd, np.full(2, t), m[upd], x[upd] + np.float32(0.25), v[upd], a[upd], k[upd])
@@ -108,14 +115,15 @@ def test_shard_bounds_cover_and_balance():
         shard_bounds(10, 2, 2)
 
 
-def test_sharded_force_world2_matches_whole_system_oracle(tmp_path):
+@pytest.mark.parametrize("mode", ["j", "i"])
+def test_sharded_force_world2_matches_whole_system_oracle(tmp_path, mode):
     from oracle import nbody_oracle as O
     from paper_0707_0438_b200 import inputs
     from parity import assert_parity
 
     n, n_i = 301, 97   # odd sizes: unequal shards, i-particles owned by both ranks
     script = tmp_path / "worker.py"
-    script.write_text(WORKER.format(root=ROOT, n=n, n_i=n_i))
+    script.write_text(WORKER.format(root=ROOT, n=n, n_i=n_i, mode=mode))
     port = _free_port()
     procs = []
     for rank in range(2):
@@ -129,9 +137,14 @@ def test_sharded_force_world2_matches_whole_system_oracle(tmp_path):
         assert p.returncode == 0, err
         outs.append(json.loads(out.strip().splitlines()[-1]))
     outs.sort(key=lambda o: o["rank"])
-    assert (outs[0]["j0"], outs[0]["j1"], outs[1]["j0"], outs[1]["j1"]) == (0, 150, 150, 301)
-    assert outs[0]["kept"] == 150 and outs[1]["kept"] == 151
-    assert outs[0]["collectives"] == 4 and outs[1]["collectives"] == 4   # two per call
+    if mode == "j":
+        assert (outs[0]["j0"], outs[0]["j1"], outs[1]["j0"], outs[1]["j1"]) == (0, 150, 150, 301)
+        assert outs[0]["kept"] == 150 and outs[1]["kept"] == 151
+        assert outs[0]["collectives"] == 4 and outs[1]["collectives"] == 4   # two all-reduces per call
+    else:   # j replicated, i-list cut in two (49 + 48 of 97), three all-gathers per call
+        assert (outs[0]["j0"], outs[0]["j1"], outs[1]["j0"], outs[1]["j1"]) == (0, 301, 0, 301)
+        assert outs[0]["kept"] == 301 and outs[1]["kept"] == 301
+        assert outs[0]["collectives"] == 6 and outs[1]["collectives"] == 6
     for key in ("acc", "jerk", "pot", "acc2", "pot2"):   # an all-reduce gives every rank the same bits
         assert outs[0][key] == outs[1][key], key
 
