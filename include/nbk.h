@@ -64,7 +64,10 @@ typedef enum nbk_status {
 
 /* Create a context on CUDA device `device` able to hold n_max j-particles and to serve up to
  * ni_max i-particles per call.  `cuda_stream` is a cudaStream_t (e.g. a torch stream's
- * .cuda_stream) on which all work is enqueued; NULL = the library creates its own stream.
+ * .cuda_stream) on which all work is enqueued; NULL = the library creates its own non-blocking
+ * stream.  Note that the handle of CUDA's legacy default stream IS NULL (torch's default stream has
+ * .cuda_stream == 0): a caller that mixes its own work on the default stream with _dev calls must
+ * pass a real stream here or order the two with events.
  * All device and pinned memory is allocated here, none later. */
 int nbk_open(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cuda_stream);
 
