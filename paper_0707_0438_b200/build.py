@@ -24,7 +24,7 @@ LIB = os.path.join(HERE, "libnbk.so")
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC,-O2,-fvisibility=default",
+    "-Xcompiler", "-fPIC,-O2,-fvisibility=default,-fopenmp",
     "-shared", "-cudart", "static",
 ]
 
@@ -51,7 +51,7 @@ def build(force: bool = False, lib: str = LIB, defines=(), verbose: bool = False
     cmd += [f"-D{d}" for d in defines]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-o", lib]
+    cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-lgomp", "-o", lib]
     proc = subprocess.run(cmd, capture_output=True, text=True)
     if proc.returncode != 0:
         raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + proc.stdout + proc.stderr)

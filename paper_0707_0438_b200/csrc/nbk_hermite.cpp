@@ -98,6 +98,8 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
     std::vector<float> fa(3 * N), fj(3 * N);
     std::vector<int32_t> act;
     act.reserve(N);
+    std::vector<int> knew(N);
+    const int64_t kParallelMin = 2048;   // blocks smaller than this are corrected by the calling thread
     // packed per-block buffers for set_j
     std::vector<double> bt(N), bm(N), bx(3 * N), bv(3 * N), ba(3 * N), bj(3 * N), xp(3 * N), vp(3 * N);
     Levels L(n);
@@ -148,6 +150,7 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
         NBK_TIMED(nbk_set_ti(ctx, t_new));
         NBK_TIMED(nbk_calc_firsthalf(ctx, n, ni, act.data(), nullptr, nullptr, eps2, flags));
         // host predictor (fp64) for the block's own particles, overlapped with the device
+#pragma omp parallel for schedule(static) if (ni >= kParallelMin)
         for (int64_t q = 0; q < ni; ++q) {
             const size_t i = static_cast<size_t>(act[q]);
             const double dt = t_new - tl[i], dt2 = dt * dt / 2.0, dt3 = dt * dt * dt / 6.0;
@@ -160,6 +163,10 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
         slot = 1;
         NBK_TIMED(nbk_calc_lasthalf(ctx, ni, fa.data(), fj.data(), nullptr));
 
+        // corrector, Aarseth step and block rule: independent per particle (large blocks run on all
+        // host cores); the level lists are updated afterwards in block order, so the result does
+        // not depend on the thread count
+#pragma omp parallel for schedule(static) if (ni >= kParallelMin)
         for (int64_t q = 0; q < ni; ++q) {
             const int32_t ii = act[q];
             const size_t i = static_cast<size_t>(ii);
@@ -197,10 +204,7 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
                        T_new % (int64_t(1) << (kTickLog2 - (k - 1))) == 0) {
                 k -= 1;
             }
-            if (k != L.lev[i]) {
-                L.remove(ii);
-                L.insert(ii, k);
-            }
+            knew[q] = k;
             bt[q] = t_new;
             bm[q] = m[i];
             for (int c = 0; c < 3; ++c) {
@@ -208,6 +212,13 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
                 bv[3 * q + c] = v[3 * i + c];
                 ba[3 * q + c] = a1[c];
                 bj[3 * q + c] = j1[c];
+            }
+        }
+        for (int64_t q = 0; q < ni; ++q) {
+            const int32_t ii = act[q];
+            if (knew[q] != L.lev[ii]) {
+                L.remove(ii);
+                L.insert(ii, knew[q]);
             }
         }
         slot = 2;
