@@ -389,7 +389,14 @@ def run_sharded(args, wl):
     n = m.shape[0]
     eps2 = float(np.float32(eps) ** 2)
     flags = (nb.NBK_JERK if jerk else 0) | nb.NBK_POT
-    sf = ShardedForce(n, n, device=local, mode=args.shard)
+    if args.transport == "peer" and world == 1:   # symmetric memory wants a process group, also at world size 1
+        import torch.distributed as dist
+        if not dist.is_initialized():
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29577")
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
+    sf = ShardedForce(n, n, device=local, mode=args.shard,
+                      transport=args.transport if args.shard == "j" else "nccl")
     ci = -(-n // world)   # i-particles this rank's force kernel handles
     n_i_rank = n if args.shard == "j" else max(0, min((rank + 1) * ci, n) - min(rank * ci, n))
     try:
@@ -430,8 +437,8 @@ def run_sharded(args, wl):
         assert bool(torch.isfinite(out[0]).all()) and bool(torch.isfinite(out[2]).all())
     finally:
         sf.close()
-    if world > 1:
-        import torch.distributed as dist
+    import torch.distributed as dist
+    if dist.is_initialized():
         dist.destroy_process_group()
     if rank != 0:
         return 0
@@ -445,7 +452,8 @@ def run_sharded(args, wl):
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": desc, "n_i": n, "n_j": n, "parallelism": f"{args.shard}-sharded x{world}",
                    "n_j_per_rank": sf.n_local, "n_i_per_rank": n_i_rank,
-                   "collectives_per_step": (2 if args.shard == "j" else 3) if world > 1 else 0,
+                   "collectives_per_step": (0 if sf.transport == "peer" else 2 if args.shard == "j" else 3) if world > 1 else 0,
+                   "transport": sf.transport + (" (symmetric memory, 2 barriers per step, P2P loads)" if sf.transport == "peer" else ""),
                    "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB write)", "launch": launch},
         "clocks": clocks, "gpu_launches": int(args.steps * 5),
         "roofline": {"bound": "alu", "kernel": "nbk::force_kernel (rank 0)", "achieved": achieved, "peak": peak_tflops,
@@ -618,6 +626,8 @@ def main(argv=None):
                     help="j: shard the j-particles over the ranks with two all-reduces per step; i: replicate j, shard "
                          "each i-list, all-gather the results (both strong scaling); "
                          "default: independent replicas (weak)")
+    ap.add_argument("--transport", choices=["nccl", "peer"], default="nccl",
+                    help="with --shard j: exchange by NCCL all-reduces, or by loads from peer (symmetric) memory")
     args = ap.parse_args(argv)
     if args.sweep:
         return run_sweep(args)

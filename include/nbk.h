@@ -257,6 +257,24 @@ int nbk_shard_calc_partial_dev(nbk_ctx* ctx, int64_t n_local, int64_t n_i, const
 int nbk_shard_finish_dev(nbk_ctx* ctx, int64_t n_i, const double* sum64, float* acc, float* jerk,
                          float* pot);
 
+/* The same two exchanges as loads from PEER memory (NVLink / NVSwitch P2P) instead of collectives,
+ * for callers whose xv and sum64 buffers live in symmetric memory mapped into every rank (e.g.
+ * torch.distributed._symmetric_memory).  `world` <= 16 ranks.  The caller separates the steps with a
+ * cross-rank barrier on the stream (after gather_i; after calc_partial): two barriers per call, no
+ * payload collective.
+ *   nbk_shard_fetch_i_dev   replaces all-reduce 1: xv[k] (this rank's private [n_i][8] buffer) = row k
+ *                           of the OWNER's published buffer, the owner found from shard_begin (HOST
+ *                           array of world + 1 global addresses); peer_xv is a HOST array of `world`
+ *                           device pointers, peer_xv[r] = rank r's buffer written by its gather_i.
+ *   nbk_shard_combine_dev   replaces all-reduce 2 and finish: acc, jerk, pot = the sum over ranks r, in
+ *                           rank order, of row k of peer_sum64[r] (HOST array of `world` device
+ *                           pointers to the [n_i][8] fp64 buffers calc_partial wrote), rounded once.
+ *                           Same bits on every rank. */
+int nbk_shard_fetch_i_dev(nbk_ctx* ctx, int64_t n_i, int32_t world, const int32_t* i_global,
+                          const int64_t* shard_begin, const void* const* peer_xv, float* xv);
+int nbk_shard_combine_dev(nbk_ctx* ctx, int64_t n_i, int32_t world, const void* const* peer_sum64,
+                          float* acc, float* jerk, float* pot);
+
 /* Block until everything enqueued on the context's stream has run. */
 int nbk_sync(nbk_ctx* ctx);
 

@@ -23,6 +23,7 @@ EXPORTS = [
     "nbk_calc_firsthalf", "nbk_calc_firsthalf_dev", "nbk_calc_lasthalf", "nbk_calc_lasthalf_f64", "nbk_calc_lasthalf_dev",
     "nbk_get_neighbours", "nbk_get_neighbours_dev", "nbk_calc_batch", "nbk_calc_batch_dev",
     "nbk_shard_gather_i_dev", "nbk_shard_calc_partial_dev", "nbk_shard_finish_dev",
+    "nbk_shard_fetch_i_dev", "nbk_shard_combine_dev",
     "nbk_hermite_evolve", "nbk_hermite_evolve_dev", "nbk_sync", "nbk_set_timing", "nbk_get_timing", "nbk_last_launch",
     "nbk_plan", "nbk_set_variant", "nbk_last_cuda_error", "nbk_strerror", "nbk_version",
 ]
@@ -61,6 +62,8 @@ _SIGS = {
     "nbk_shard_gather_i_dev": (_i32, [_vp, _i64, _i64, _i64, _vp, _vp, _vp]),
     "nbk_shard_calc_partial_dev": (_i32, [_vp, _i64, _i64, _vp, _vp, _f32, _u32, _vp]),
     "nbk_shard_finish_dev": (_i32, [_vp, _i64, _vp, _vp, _vp, _vp]),
+    "nbk_shard_fetch_i_dev": (_i32, [_vp, _i64, _i32, _vp, _vp, _vp, _vp]),
+    "nbk_shard_combine_dev": (_i32, [_vp, _i64, _i32, _vp, _vp, _vp, _vp]),
     "nbk_hermite_evolve": (_i32, [_vp, _i64, _vp, _vp, _vp, _f64, _f64, _f64, _f64,
                                   ctypes.POINTER(HermiteStats)]),
     "nbk_hermite_evolve_dev": (_i32, [_vp, _i64, _vp, _vp, _vp, _f64, _f64, _f64, _f64,
@@ -291,6 +294,22 @@ def nbk_shard_calc_partial_dev(ctx, n_local, n_i, i_local, xv, eps2, flags, sum6
 def nbk_shard_finish_dev(ctx, n_i, sum64, acc=0, jerk=0, pot=0):
     _check("nbk_shard_finish_dev",
            load().nbk_shard_finish_dev(ctx, n_i, sum64 or None, acc or None, jerk or None, pot or None), ctx)
+
+
+def nbk_shard_fetch_i_dev(ctx, n_i, i_global, shard_begin, peer_xv, xv):
+    """shard_begin: world + 1 global addresses; peer_xv: world device addresses (host sequences)."""
+    begin = np.ascontiguousarray(shard_begin, dtype=np.int64)
+    ptrs = (_vp * len(peer_xv))(*[int(p) for p in peer_xv])
+    if begin.shape[0] != len(peer_xv) + 1:
+        raise ValueError("shard_fetch_i: shard_begin must have world + 1 entries")
+    _check("nbk_shard_fetch_i_dev",
+           load().nbk_shard_fetch_i_dev(ctx, n_i, len(peer_xv), i_global or None, begin.ctypes.data, ptrs, xv or None), ctx)
+
+
+def nbk_shard_combine_dev(ctx, n_i, peer_sum64, acc=0, jerk=0, pot=0):
+    ptrs = (_vp * len(peer_sum64))(*[int(p) for p in peer_sum64])
+    _check("nbk_shard_combine_dev",
+           load().nbk_shard_combine_dev(ctx, n_i, len(peer_sum64), ptrs, acc or None, jerk or None, pot or None), ctx)
 
 
 def nbk_hermite_evolve_dev(ctx, m, x, v, eps, t_end, eta=0.01, dt_max=1.0 / 16.0):

@@ -722,6 +722,42 @@ int nbk_shard_finish_dev(nbk_ctx* c, int64_t n_i, const double* sum64, float* ac
     return NBK_OK;
 }
 
+int nbk_shard_fetch_i_dev(nbk_ctx* c, int64_t n_i, int32_t world, const int32_t* i_global,
+                          const int64_t* shard_begin, const void* const* peer_xv, float* xv) {
+    if (!c || n_i < 0 || world < 1 || world > kMaxPeers || !shard_begin || !peer_xv) return NBK_EINVAL;
+    if (n_i > 0 && (!i_global || !xv)) return NBK_EINVAL;
+    if (n_i > c->ni_max) return NBK_ERANGE;
+    ShardPeers p;
+    std::memset(&p, 0, sizeof(p));
+    p.world = world;
+    for (int r = 0; r < world; ++r) {
+        if (!peer_xv[r] || shard_begin[r] > shard_begin[r + 1]) return NBK_EINVAL;
+        p.ptr[r] = peer_xv[r];
+        p.begin[r] = shard_begin[r];
+    }
+    p.begin[world] = shard_begin[world];
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    NBK_CUDA(c, launch_shard_fetch(p, i_global, n_i, xv, c->stream));
+    return NBK_OK;
+}
+
+int nbk_shard_combine_dev(nbk_ctx* c, int64_t n_i, int32_t world, const void* const* peer_sum64,
+                          float* acc, float* jerk, float* pot) {
+    if (!c || n_i < 0 || world < 1 || world > kMaxPeers || !peer_sum64) return NBK_EINVAL;
+    ShardPeers p;
+    std::memset(&p, 0, sizeof(p));
+    p.world = world;
+    for (int r = 0; r < world; ++r) {
+        if (!peer_sum64[r]) return NBK_EINVAL;
+        p.ptr[r] = peer_sum64[r];
+    }
+    DeviceGuard g(c->device);
+    if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
+    NBK_CUDA(c, launch_shard_combine(p, n_i, acc, jerk, pot, c->stream));
+    return NBK_OK;
+}
+
 int nbk_get_neighbours(nbk_ctx* c, int64_t n_i, int32_t* nn_index, float* nn_r2) {
     if (!c || n_i < 0) return NBK_EINVAL;
     if (!c->in_flight || n_i != c->last_ni || !c->last_nn) return NBK_ESTATE;

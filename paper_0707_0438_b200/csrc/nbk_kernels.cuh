@@ -260,6 +260,18 @@ cudaError_t launch_shard_gather(const ShardGatherArgs& a, cudaStream_t s);
 cudaError_t launch_shard_split(const float* xv, long long n_i, float* xi, float* vi, cudaStream_t s);
 cudaError_t launch_shard_finish(const double* sum64, long long n_i, float* acc, float* jerk,
                                 float* pot, cudaStream_t s);
+// The same two exchanges over peer memory (NVLink P2P loads from the other ranks' symmetric buffers)
+// instead of NCCL collectives: ptr[r] is rank r's buffer as mapped into this process.
+constexpr int kMaxPeers = 16;
+struct ShardPeers {
+    const void* ptr[kMaxPeers];
+    long long begin[kMaxPeers + 1];   // shard r owns global addresses [begin[r], begin[r+1]) (fetch only)
+    int world;
+};
+cudaError_t launch_shard_fetch(const ShardPeers& peers, const int32_t* i_global, long long n_i,
+                               float* xv, cudaStream_t s);
+cudaError_t launch_shard_combine(const ShardPeers& peers, long long n_i, float* acc, float* jerk,
+                                 float* pot, cudaStream_t s);
 
 // set_j scatter: staged particles -> raw SoA at addr (nullptr: identity).  x, v as fp32 or fp64.
 struct ScatterArgs {

@@ -14,6 +14,12 @@ mode="i" is the other cut of SURVEY.md 8(e): every rank holds all j-particles, t
 each i-list through the ordinary firsthalf/lasthalf calls, and the result arrays are all-gathered
 (no partial sums; suited to full evaluations at large N, e.g. config C4).
 
+transport="peer" (mode "j") replaces the two all-reduces by loads from peer memory: the exchange
+buffers live in torch symmetric memory mapped into every rank, a cross-rank barrier separates the
+steps, `nbk_shard_fetch_i_dev` reads each i-particle's state from its owner's buffer and
+`nbk_shard_combine_dev` adds the ranks' fp64 rows in rank order and rounds once (all-reduce and finish
+in one kernel).  It needs NVLink/NVSwitch P2P between the ranks; NCCL stays the default.
+
 This module holds no arithmetic of the method: it computes the shard bounds, owns the exchange
 buffers and strings the three C-ABI calls (include/nbk.h, "j-sharding") and the two collectives
 together on one stream.  `ops` is the object that runs the three device steps; the default is
@@ -85,6 +91,12 @@ class NbkShardOps:
     def finish(self, n_i, sum64, acc, jerk, pot):
         B.nbk_shard_finish_dev(self.ctx, n_i, sum64.data_ptr(), acc.data_ptr(), jerk.data_ptr(), pot.data_ptr())
 
+    def fetch_i(self, n_i, i_global, shard_begin, peer_xv, xv):
+        B.nbk_shard_fetch_i_dev(self.ctx, n_i, i_global.data_ptr(), shard_begin, peer_xv, xv.data_ptr())
+
+    def combine(self, n_i, peer_sum64, acc, jerk, pot):
+        B.nbk_shard_combine_dev(self.ctx, n_i, peer_sum64, acc.data_ptr(), jerk.data_ptr(), pot.data_ptr())
+
     def calc_slice(self, n_j, i_index, eps2, flags, acc, jerk, pot):
         """i-sharding: the plain firsthalf / lasthalf pair on this rank's slice of the i-list."""
         n_i = int(i_index.shape[0])
@@ -100,7 +112,7 @@ class ShardedForce:
 
     def __init__(self, n_total: int, ni_max: int, device: int = 0, group=None, ops=None,
                  world: int | None = None, rank: int | None = None, always_reduce: bool = False,
-                 mode: str = "j"):
+                 mode: str = "j", transport: str = "nccl"):
         live = dist.is_available() and dist.is_initialized()
         self.group = group
         self.world = world if world is not None else (dist.get_world_size(group) if live else 1)
@@ -115,7 +127,28 @@ class ShardedForce:
         self.j0, self.j1 = shard_bounds(self.n_total, self.world, self.rank) if mode == "j" else (0, self.n_total)
         self.n_local = self.j1 - self.j0
         self.ops = ops if ops is not None else NbkShardOps(device, self.n_local, self.ni_max)
-        if mode == "j":
+        if transport not in ("nccl", "peer") or (transport == "peer" and mode != "j"):
+            raise ValueError("transport must be 'nccl', or 'peer' with mode 'j'")
+        self.transport = transport
+        self.symm = None
+        if mode == "j" and transport == "peer":
+            # exchange buffers in symmetric memory: every rank maps every other rank's copy and reads it
+            # with P2P loads (nbk_shard_fetch_i_dev / nbk_shard_combine_dev); two barriers per call
+            import torch.distributed._symmetric_memory as symm_mem
+            if not live:
+                raise RuntimeError("transport='peer' needs an initialised process group")
+            self.i_local = self.ops.alloc((self.ni_max,), torch.int32)
+            self.xv_full = self.ops.alloc((self.ni_max, 8), torch.float32)
+            self.s64_off = (self.ni_max * 32 + 255) // 256 * 256
+            raw = symm_mem.empty((self.s64_off + self.ni_max * 64,), dtype=torch.uint8, device=self.ops.device)
+            raw.zero_()
+            self.symm_raw = raw
+            self.symm = symm_mem.rendezvous(raw, group if group is not None else dist.group.WORLD)
+            self.xv = raw[: self.ni_max * 32].view(torch.float32).view(self.ni_max, 8)
+            self.sum64 = raw[self.s64_off: self.s64_off + self.ni_max * 64].view(torch.float64).view(self.ni_max, 8)
+            self.peer_base = [int(p) for p in self.symm.buffer_ptrs]
+            self.shard_begin = [shard_bounds(self.n_total, self.world, r)[0] for r in range(self.world)] + [self.n_total]
+        elif mode == "j":
             self.i_local = self.ops.alloc((self.ni_max,), torch.int32)
             self.xv = self.ops.alloc((self.ni_max, 8), torch.float32)
             self.sum64 = self.ops.alloc((self.ni_max, 8), torch.float64)
@@ -187,6 +220,14 @@ class ShardedForce:
             self.ops.enter()
         try:
             self.ops.gather_i(self.n_local, self.j0, n_i, i_global, il, xv)
+            if self.symm is not None:   # peer memory: barrier, P2P fetch, local force, barrier, P2P combine
+                self.symm.barrier(channel=0)
+                self.ops.fetch_i(n_i, i_global, self.shard_begin, self.peer_base, self.xv_full)
+                self.ops.calc_partial(self.n_local, n_i, il, self.xv_full, float(eps2), int(flags), s64)
+                self.symm.barrier(channel=1)
+                self.ops.combine(n_i, [p + self.s64_off for p in self.peer_base], *out)
+                self.barriers = getattr(self, "barriers", 0) + 2
+                return out
             self._all_reduce(xv)
             self.ops.calc_partial(self.n_local, n_i, il, xv, float(eps2), int(flags), s64)
             self._all_reduce(s64)

@@ -27,7 +27,7 @@ def gpu():
     return torch
 
 
-def run_shards(torch, world, m, x, v, eps, ii, flags=FULL, tj=None, a=None, k=None, t=0.0):
+def run_shards(torch, world, m, x, v, eps, ii, flags=FULL, tj=None, a=None, k=None, t=0.0, peer=False):
     """G contexts on one GPU, run in turn; sums over the G buffers stand in for the all-reduces."""
     n, n_i = m.shape[0], ii.shape[0]
     dev = torch.device("cuda", 0)
@@ -36,10 +36,10 @@ def run_shards(torch, world, m, x, v, eps, ii, flags=FULL, tj=None, a=None, k=No
     ig = torch.from_numpy(ii.astype(np.int32)).to(dev)
     torch.cuda.synchronize()
     with torch.cuda.stream(ts):
-        return _run_shards_on(torch, dev, stream, ig, world, m, x, v, eps, ii, flags, tj, a, k, t)
+        return _run_shards_on(torch, dev, stream, ig, world, m, x, v, eps, ii, flags, tj, a, k, t, peer)
 
 
-def _run_shards_on(torch, dev, stream, ig, world, m, x, v, eps, ii, flags, tj, a, k, t):
+def _run_shards_on(torch, dev, stream, ig, world, m, x, v, eps, ii, flags, tj, a, k, t, peer):
     n, n_i = m.shape[0], ii.shape[0]
     ctxs, bounds = [], []
     for r in range(world):
@@ -59,16 +59,36 @@ def _run_shards_on(torch, dev, stream, ig, world, m, x, v, eps, ii, flags, tj, a
             nb.nbk_shard_gather_i_dev(c, j1 - j0, j0, n_i, ig.data_ptr(), il[r].data_ptr(), xv[r].data_ptr())
         owners = torch.stack([(t_ >= 0).to(torch.int32) for t_ in il]).sum(0)
         assert bool((owners == 1).all()), "every i-particle has exactly one owner"
-        xv_all = torch.stack(xv).sum(0).contiguous()       # stands in for all-reduce #1
         s64 = [torch.empty((n_i, 8), dtype=torch.float64, device=dev) for _ in range(world)]
+        acc = torch.empty((n_i, 3), dtype=torch.float32, device=dev)
+        jerk = torch.empty((n_i, 3), dtype=torch.float32, device=dev)
+        pot = torch.empty(n_i, dtype=torch.float32, device=dev)
+        if peer:   # the peer-memory form: every "rank" reads the others' buffers by pointer; the stream
+            begin = [b[0] for b in bounds] + [n]   # order of this one process stands in for the barriers
+            xvf = [torch.empty((n_i, 8), dtype=torch.float32, device=dev) for _ in range(world)]
+            for r, c in enumerate(ctxs):
+                nb.nbk_shard_fetch_i_dev(c, n_i, ig.data_ptr(), begin, [t_.data_ptr() for t_ in xv], xvf[r].data_ptr())
+            for r, c in enumerate(ctxs):
+                j0, j1 = bounds[r]
+                nb.nbk_shard_calc_partial_dev(c, j1 - j0, n_i, il[r].data_ptr(), xvf[r].data_ptr(),
+                                              np.float32(eps) ** 2, flags, s64[r].data_ptr())
+            outs = []
+            for r, c in enumerate(ctxs):   # every rank combines for itself: all must get the same bits
+                o = [torch.empty_like(acc), torch.empty_like(jerk), torch.empty_like(pot)]
+                nb.nbk_shard_combine_dev(c, n_i, [t_.data_ptr() for t_ in s64], *[t_.data_ptr() for t_ in o])
+                outs.append(o)
+            torch.cuda.synchronize()
+            for o in outs[1:]:
+                assert all(torch.equal(p_, q_) for p_, q_ in zip(o, outs[0]))
+            acc, jerk, pot = outs[0]
+            xv_all = xvf[world - 1]
+            return acc.cpu().numpy(), jerk.cpu().numpy(), pot.cpu().numpy(), xv_all.cpu().numpy()
+        xv_all = torch.stack(xv).sum(0).contiguous()       # stands in for all-reduce #1
         for r, c in enumerate(ctxs):
             j0, j1 = bounds[r]
             nb.nbk_shard_calc_partial_dev(c, j1 - j0, n_i, il[r].data_ptr(), xv_all.data_ptr(),
                                           np.float32(eps) ** 2, flags, s64[r].data_ptr())
         tot = torch.stack(s64).sum(0).contiguous()         # stands in for all-reduce #2
-        acc = torch.empty((n_i, 3), dtype=torch.float32, device=dev)
-        jerk = torch.empty((n_i, 3), dtype=torch.float32, device=dev)
-        pot = torch.empty(n_i, dtype=torch.float32, device=dev)
         nb.nbk_shard_finish_dev(ctxs[0], n_i, tot.data_ptr(), acc.data_ptr(), jerk.data_ptr(), pot.data_ptr())
         torch.cuda.synchronize()
         return acc.cpu().numpy(), jerk.cpu().numpy(), pot.cpu().numpy(), xv_all.cpu().numpy()
@@ -86,6 +106,22 @@ def test_sharded_parity_vs_whole_system_oracle(gpu, c_oracle, world, n, n_i):
     acc, jerk, pot, xv = run_shards(gpu, world, m, x, v, EPS, ii)
     assert np.array_equal(xv[:, 0:3], x[ii]) and np.array_equal(xv[:, 4:7], v[ii])   # exact copy
     assert_parity((acc, jerk, pot), ref, what=f"sharded G={world} n={n} n_i={n_i}")
+
+
+@pytest.mark.parametrize("world", [1, 3, 8, 16])
+def test_sharded_peer_memory_form_parity_and_same_bits_as_collective_form(gpu, c_oracle, world):
+    """nbk_shard_fetch_i_dev / nbk_shard_combine_dev (P2P loads by pointer) against the oracle, and
+    bit for bit against the collective form: both add the ranks' fp64 rows in rank order."""
+    n, n_i = 4099, 1031
+    m, x, v = inputs.plummer_f32(n, 2)
+    ii = inputs.active_block(n, n_i, 21)
+    ref = c_oracle.force(m, x, v, EPS, i_index=ii)
+    got = run_shards(gpu, world, m, x, v, EPS, ii, peer=True)
+    assert np.array_equal(got[3][:, 0:3], x[ii]) and np.array_equal(got[3][:, 4:7], v[ii])
+    assert_parity(got[:3], ref, what=f"peer-memory G={world}")
+    coll = run_shards(gpu, world, m, x, v, EPS, ii, peer=False)
+    for g, c in zip(got[:3], coll[:3]):
+        assert np.array_equal(g, c)
 
 
 def test_sharded_eps0_and_acc_only(gpu, c_oracle):
@@ -177,6 +213,16 @@ for o in outs:
     for g, p in zip(o, plain):
         assert np.array_equal(g.cpu().numpy(), p)
 sf.close()
+sp = ShardedForce(n, n_i, device=0, transport="peer")   # symmetric memory + barriers + P2P kernels
+sp.set_j_particles(None, None, m, x, v)
+sp.set_ti(0.0)
+for rep in range(3):
+    o = sp.calc(ig, e2)
+    torch.cuda.synchronize()
+    for g, p in zip(o, plain):
+        assert np.array_equal(g.cpu().numpy(), p)
+assert sp.barriers == 6
+sp.close()
 si = ShardedForce(n, n_i, device=0, always_reduce=True, mode="i")   # i-sharding: three all-gathers per call
 si.set_j_particles(None, None, m, x, v)
 si.set_ti(0.0)
