@@ -158,7 +158,8 @@ class ShardedForce:
             self.g_acc = self.ops.alloc((rows, 3), torch.float32)
             self.g_jerk = self.ops.alloc((rows, 3), torch.float32)
             self.g_pot = self.ops.alloc((rows,), torch.float32)
-        self.collectives = 0   # all-reduces issued so far (for tests and bench)
+        self.collectives = 0   # all-reduces / all-gathers issued so far (for tests and bench)
+        self.barriers = 0      # symmetric-memory barriers issued so far (transport 'peer')
         # issue the collectives at world size 1 too (needs a process group): lets a one-GPU box run
         # the NCCL calls, their dtypes and their stream ordering
         self.always_reduce = bool(always_reduce) and live
@@ -226,7 +227,7 @@ class ShardedForce:
                 self.ops.calc_partial(self.n_local, n_i, il, self.xv_full, float(eps2), int(flags), s64)
                 self.symm.barrier(channel=1)
                 self.ops.combine(n_i, [p + self.s64_off for p in self.peer_base], *out)
-                self.barriers = getattr(self, "barriers", 0) + 2
+                self.barriers += 2
                 return out
             self._all_reduce(xv)
             self.ops.calc_partial(self.n_local, n_i, il, xv, float(eps2), int(flags), s64)
