@@ -213,16 +213,6 @@ for o in outs:
     for g, p in zip(o, plain):
         assert np.array_equal(g.cpu().numpy(), p)
 sf.close()
-sp = ShardedForce(n, n_i, device=0, transport="peer")   # symmetric memory + barriers + P2P kernels
-sp.set_j_particles(None, None, m, x, v)
-sp.set_ti(0.0)
-for rep in range(3):
-    o = sp.calc(ig, e2)
-    torch.cuda.synchronize()
-    for g, p in zip(o, plain):
-        assert np.array_equal(g.cpu().numpy(), p)
-assert sp.barriers == 6
-sp.close()
 si = ShardedForce(n, n_i, device=0, always_reduce=True, mode="i")   # i-sharding: three all-gathers per call
 si.set_j_particles(None, None, m, x, v)
 si.set_ti(0.0)
@@ -278,6 +268,70 @@ def test_i_sharded_world1_class_equals_plain_path_bitwise(gpu, c_oracle):
     finally:
         sf.close()
     assert_parity(got, c_oracle.force(m, x, v, EPS, i_index=ii), what="i-sharded world 1")
+
+
+PEER_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+import numpy as np, torch
+import torch.distributed as dist
+from paper_0707_0438_b200 import binding as nb, inputs
+from paper_0707_0438_b200.sharded import ShardedForce
+torch.cuda.set_device(0)
+dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+n, n_i = 16384, 4096
+m, x, v = inputs.plummer_f32(n, 2)
+ii = inputs.active_block(n, n_i, 24)
+e2 = float(np.float32(inputs.EPS_PAPER) ** 2)
+try:   # platform capability: symmetric memory allocation and rendezvous
+    import torch.distributed._symmetric_memory as symm_mem
+    probe = symm_mem.empty((1024,), dtype=torch.uint8, device=torch.device("cuda", 0))
+    symm_mem.rendezvous(probe, dist.group.WORLD)
+except Exception as e:
+    print("SYMM_UNAVAILABLE", type(e).__name__, str(e)[:200])
+    dist.destroy_process_group()
+    sys.exit(0)
+sp = ShardedForce(n, n_i, device=0, transport="peer")   # symmetric memory + barriers + P2P kernels
+sp.set_j_particles(None, None, m, x, v)
+sp.set_ti(0.0)
+ig = torch.from_numpy(ii).to("cuda:0")
+outs = [tuple(t.clone() for t in sp.calc(ig, e2)) for _ in range(3)]
+torch.cuda.synchronize()
+assert sp.barriers == 6 and sp.collectives == 0
+c = nb.nbk_open(0, n, n_i)
+nb.nbk_set_j_particles(c, None, None, m, x, v)
+nb.nbk_set_ti(c, 0.0)
+nb.nbk_calc_firsthalf(c, n, n_i, ii, None, None, e2, nb.NBK_JERK | nb.NBK_POT)
+plain = nb.nbk_calc_lasthalf(c, n_i)
+nb.nbk_close(c)
+for o in outs:
+    for g, p in zip(o, plain):
+        assert np.array_equal(g.cpu().numpy(), p)
+sp.close()
+dist.destroy_process_group()
+print("PEER_OK")
+"""
+
+
+def test_sharded_peer_transport_with_symmetric_memory_at_world1(gpu, tmp_path):
+    """transport="peer" with real torch symmetric memory, its barriers and the P2P kernels at world size 1:
+    bit-equal to the plain path.  Skipped only if the platform cannot allocate / rendezvous symmetric memory."""
+    import os
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "peer_worker.py"
+    script.write_text(PEER_WORKER.format(root=root))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
+    p = subprocess.run([sys.executable, str(script)], env=env, capture_output=True, text=True, timeout=600)
+    assert p.returncode == 0, p.stdout + p.stderr
+    if "SYMM_UNAVAILABLE" in p.stdout:
+        pytest.skip("symmetric memory unavailable here: " + p.stdout.strip().splitlines()[-1])
+    assert "PEER_OK" in p.stdout, p.stdout + p.stderr
 
 
 def test_sharded_refused_calls(gpu):
