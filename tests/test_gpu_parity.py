@@ -110,3 +110,45 @@ def test_bad_calls_are_refused(gpu):
         with pytest.raises(nb.NbkError) as e:
             nb.nbk_set_j_particles(ctx, np.array([64], np.int32), None, m[:1], x[:1], v[:1])
         assert e.value.status == nb.NBK_ERANGE
+
+
+def test_seeded_random_sizes_flags_and_kernel_forms(gpu, c_oracle):
+    """300 seeded random cases over n, n_i (around the tile and warp boundaries), eps in {1/256, 0, 0.05},
+    with and without jerk / nearest neighbour, every kernel form the library can be pinned to, indexed and
+    external i-particles: every one inside the north_star tolerances."""
+    rng = np.random.default_rng(20071107)
+    sizes = [1, 2, 3, 5, 17, 63, 64, 65, 255, 256, 257, 1000, 1531, 2048, 4097]
+    for case in range(300):
+        n = int(rng.choice(sizes + [int(rng.integers(1, 6000))]))
+        n_i = min(n, int(rng.choice([1, 2, 31, 32, 33, n, max(1, n // 2), int(rng.integers(1, n + 1))])))
+        eps = float(rng.choice([EPS, 0.0, 0.05]))
+        jerk = bool(rng.integers(0, 2))
+        nn = jerk and rng.integers(0, 4) == 0
+        flags = (nb.NBK_JERK if jerk else 0) | nb.NBK_POT | (nb.NBK_NN if nn else 0) | (nb.NBK_EPS0 if eps == 0.0 else 0)
+        variant = int(rng.choice([0x00, 0x10, 0x20, 0x40, 0x100, 0x00 if nn else 0x01]))
+        m, x, v = inputs.plummer_f32(n, int(rng.integers(1, 1000)))
+        idx = np.sort(rng.choice(n, size=n_i, replace=False)).astype(np.int32)
+        xi = vi = None
+        ii = idx
+        if not nn and rng.integers(0, 5) == 0:   # external test particles beside the chosen ones
+            xi = (x[idx] + np.float32(0.013)).astype(np.float32)
+            vi = v[idx].copy()
+            ii = np.full(n_i, -1, np.int32)
+        what = f"case {case}: n={n} n_i={n_i} eps={eps} jerk={jerk} nn={nn} variant={variant:#x} external={xi is not None}"
+        with Ctx(n) as ctx:
+            nb.nbk_set_variant(ctx, variant)
+            got = gpu_force(ctx, m, x, v, eps, i_index=ii, flags=flags, xi=xi, vi=vi, n_i=n_i)
+            if nn:
+                gi, gr2 = nb.nbk_get_neighbours(ctx, n_i)
+        if n == 1 and xi is None:
+            assert not np.any(got[0]) and not np.any(got[2]), what
+            continue
+        ref = c_oracle.force(m, x, v, eps, i_index=ii, want_jerk=jerk, xi=xi, vi=vi)
+        e = errors(got, ref, jerk)
+        assert np.all(np.isfinite(got[0])) and np.all(np.isfinite(got[2])), what
+        assert e["acc_max"] <= 1e-4 and e["pot_max"] <= 1e-5, f"{what}: {e}"
+        if jerk:
+            assert e["jerk_p99"] <= 1e-3 and e["jerk_max"] <= 1e-2, f"{what}: {e}"
+        if nn:
+            ri, rr2 = c_oracle.nearest_neighbour(x, i_index=idx)
+            assert np.all(np.abs(gr2 - rr2) <= 4e-6 * rr2 + 1e-12), what
