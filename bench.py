@@ -236,11 +236,20 @@ def run_ours(args, wl):
             nb.nbk_calc_firsthalf_dev(ctx, n, n, 0, 0, 0, eps2, flags)
             nb.nbk_calc_lasthalf_dev(ctx, n, d_acc.data_ptr(), d_jrk.data_ptr(), d_pot.data_ptr())
 
+        # end-to-end arm: inputs and results in PINNED host memory (numpy views of pinned torch tensors);
+        # the library copies host <-> device directly from / into them
+        def pinned(a):
+            t = torch.from_numpy(a).pin_memory()
+            return t, t.numpy()
+        keep = [pinned(m), pinned(x), pinned(v), pinned(np.empty((n, 3), np.float32)),
+                pinned(np.empty((n, 3), np.float32)), pinned(np.empty(n, np.float32))]
+        hm, hx, hv, h_acc, h_jrk, h_pot = (k[1] for k in keep)
+
         def step_host():
-            nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+            nb.nbk_set_j_particles(ctx, None, None, hm, hx, hv)
             nb.nbk_set_ti(ctx, 0.0)
             nb.nbk_calc_firsthalf(ctx, n, n, None, None, None, eps2, flags)
-            return nb.nbk_calc_lasthalf(ctx, n)
+            return nb.nbk_calc_lasthalf(ctx, n, out=(h_acc, h_jrk, h_pot))
 
         def barrier():
             if world > 1:

@@ -26,7 +26,10 @@
  *     NaN/Inf in results is not an error.  After NBK_ECUDA, nbk_last_cuda_error() gives the
  *     cudaError_t value.
  *   - "host" pointers are ordinary host memory (pageable is fine; the library stages through
- *     its own pinned buffers).  "device" pointers (functions ending in _dev) are device
+ *     its own pinned buffers).  If every array of a call of >= 4096 particles lies in page-locked
+ *     memory (cudaHostAlloc / cudaHostRegister, a pinned torch tensor), set_j and lasthalf copy
+ *     straight from / into the caller's arrays instead; semantics are unchanged (the call returns
+ *     once the caller's arrays may be reused / hold the results).  "device" pointers (functions ending in _dev) are device
  *     memory on the context's device; the library only enqueues work on the context's
  *     stream and does not synchronise.
  *   - The caller owns every array it passes.  Host arrays may be reused as soon as the call

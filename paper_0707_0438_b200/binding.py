@@ -219,10 +219,19 @@ def nbk_calc_firsthalf_dev(ctx, n_j, n_i, i_index=0, xi=0, vi=0, eps2=0.0, flags
                                          float(eps2), flags), ctx)
 
 
-def nbk_calc_lasthalf(ctx, n_i):
-    acc = np.empty((n_i, 3), np.float32)
-    jerk = np.empty((n_i, 3), np.float32)
-    pot = np.empty(n_i, np.float32)
+def nbk_calc_lasthalf(ctx, n_i, out=None):
+    """out: optional (acc [n_i,3], jerk [n_i,3], pot [n_i]) float32 C-contiguous arrays to fill, e.g. views
+    of pinned memory (the library then copies device -> caller directly); default: fresh arrays."""
+    if out is None:
+        acc = np.empty((n_i, 3), np.float32)
+        jerk = np.empty((n_i, 3), np.float32)
+        pot = np.empty(n_i, np.float32)
+    else:
+        acc, jerk, pot = out
+        for arr, shape in ((acc, (n_i, 3)), (jerk, (n_i, 3)), (pot, (n_i,))):
+            if not (isinstance(arr, np.ndarray) and arr.dtype == np.float32 and arr.flags.c_contiguous
+                    and arr.shape == shape):
+                raise ValueError("lasthalf: out arrays must be C-contiguous float32 of shapes [n_i,3], [n_i,3], [n_i]")
     _check("nbk_calc_lasthalf",
            load().nbk_calc_lasthalf(ctx, n_i, acc.ctypes.data, jerk.ctypes.data, pot.ctypes.data), ctx)
     return acc, jerk, pot

@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <functional>
 #include <new>
 #include <vector>
 
@@ -25,6 +26,19 @@ bool pdl_enabled() {
     }();
     return on;
 }
+
+// Page-locked host memory (cudaHostAlloc / cudaHostRegister, e.g. a pinned torch tensor): the DMA engine
+// can read and write it directly, so large transfers skip the copy through the library's staging buffer.
+bool is_pinned_host(const void* p) {
+    if (!p) return true;   // absent arrays do not decide
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    return at.type == cudaMemoryTypeHost;
+}
+constexpr long long kDirectMin = 4096;   // particles from which a pinned caller array is copied directly
 
 int cuda_fail(nbk_ctx* c, cudaError_t e) {
     c->last_cuda = static_cast<int>(e);
@@ -291,12 +305,26 @@ int set_j_host(nbk_ctx* c, long long n, const int32_t* addr, const double* tj, c
     NBK_CUDA(c, cudaEventSynchronize(c->stage_free));
     // pack [tj | m | x | v | a | jerk | addr] into the pinned buffer: one H2D copy
     size_t off = 0;
-    auto put = [&](const void* src, size_t bytes) -> size_t {
+    std::function<size_t(const void*, size_t)> put = [&](const void* src, size_t bytes) -> size_t {
         const size_t at = off;
         if (src) std::memcpy(c->h_stage + at, src, bytes);
         off += (bytes + 15) & ~static_cast<size_t>(15);
         return at;
     };
+    // caller arrays in pinned memory: one asynchronous copy per array straight from them; the call
+    // waits for the copies before it returns (the caller may reuse its arrays at once, nbk.h)
+    const bool direct = n >= kDirectMin && is_pinned_host(tj) && is_pinned_host(m) && is_pinned_host(x) &&
+                        is_pinned_host(v) && is_pinned_host(a) && is_pinned_host(jerk) && is_pinned_host(addr);
+    cudaError_t derr = cudaSuccess;
+    if (direct) {
+        put = [&](const void* src, size_t bytes) -> size_t {
+            const size_t at = off;
+            if (src && derr == cudaSuccess)
+                derr = cudaMemcpyAsync(c->d_stage + at, src, bytes, cudaMemcpyHostToDevice, c->stream);
+            off += (bytes + 15) & ~static_cast<size_t>(15);
+            return at;
+        };
+    }
     const size_t o_t = put(tj, sizeof(double) * n);
     const size_t o_m = put(m, sizeof(T) * n);
     const size_t o_x = put(x, sizeof(T) * 3 * n);
@@ -305,8 +333,14 @@ int set_j_host(nbk_ctx* c, long long n, const int32_t* addr, const double* tj, c
     const size_t o_k = put(jerk, sizeof(T) * 3 * n);
     const size_t o_ad = put(addr, sizeof(int32_t) * n);
     if (off > c->stage_bytes) return NBK_ENOMEM;
-    NBK_CUDA(c, cudaMemcpyAsync(c->d_stage, c->h_stage, off, cudaMemcpyHostToDevice, c->stream));
-    NBK_CUDA(c, cudaEventRecord(c->stage_free, c->stream));
+    if (direct) {
+        NBK_CUDA(c, derr);
+        NBK_CUDA(c, cudaEventRecord(c->stage_free, c->stream));
+        NBK_CUDA(c, cudaEventSynchronize(c->stage_free));
+    } else {
+        NBK_CUDA(c, cudaMemcpyAsync(c->d_stage, c->h_stage, off, cudaMemcpyHostToDevice, c->stream));
+        NBK_CUDA(c, cudaEventRecord(c->stage_free, c->stream));
+    }
     ScatterArgs s;
     s.n = n;
     s.addr = addr ? reinterpret_cast<const int32_t*>(c->d_stage + o_ad) : nullptr;
@@ -639,6 +673,14 @@ int nbk_calc_lasthalf(nbk_ctx* c, int64_t n_i, float* acc, float* jerk, float* p
     DeviceGuard g(c->device);
     if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
     const size_t ni = static_cast<size_t>(n_i);
+    if (!c->host_has_result && n_i >= kDirectMin && (acc || jerk || pot) && is_pinned_host(acc) &&
+        is_pinned_host(jerk) && is_pinned_host(pot)) {   // pinned caller arrays: device -> caller directly
+        if (acc) NBK_CUDA(c, cudaMemcpyAsync(acc, c->d_result, sizeof(float) * 3 * ni, cudaMemcpyDeviceToHost, c->stream));
+        if (jerk) NBK_CUDA(c, cudaMemcpyAsync(jerk, c->d_result + 3 * ni, sizeof(float) * 3 * ni, cudaMemcpyDeviceToHost, c->stream));
+        if (pot) NBK_CUDA(c, cudaMemcpyAsync(pot, c->d_result + 6 * ni, sizeof(float) * ni, cudaMemcpyDeviceToHost, c->stream));
+        NBK_CUDA(c, cudaStreamSynchronize(c->stream));
+        return NBK_OK;
+    }
     if (!c->host_has_result)
         NBK_CUDA(c, cudaMemcpyAsync(c->h_result, c->d_result, sizeof(float) * 7 * ni,
                                     cudaMemcpyDeviceToHost, c->stream));

@@ -152,3 +152,48 @@ def test_seeded_random_sizes_flags_and_kernel_forms(gpu, c_oracle):
         if nn:
             ri, rr2 = c_oracle.nearest_neighbour(x, i_index=idx)
             assert np.all(np.abs(gr2 - rr2) <= 4e-6 * rr2 + 1e-12), what
+
+
+def test_pinned_caller_arrays_take_the_direct_copy_path_same_bits(gpu, c_oracle):
+    """Caller arrays in page-locked memory are copied by the DMA engine straight from / into them
+    (no staging copy): same bits as with pageable arrays, also with addresses, times, a and jerk given."""
+    n, t = 8192, 0.01
+    m, x, v = inputs.plummer_f32(n, 6)
+    a, k = inputs.gaussian_derivatives(n, 7)
+    tj = inputs.particle_times(n, t, 8)
+    addr = np.random.default_rng(9).permutation(n).astype(np.int32)
+    keep = []
+
+    def pin(arr):
+        tt = gpu.from_numpy(np.ascontiguousarray(arr)).pin_memory()
+        keep.append(tt)
+        return tt.numpy()
+
+    def run(pinned):
+        f = pin if pinned else (lambda z: z)
+        with Ctx(n) as ctx:
+            nb.nbk_set_j_particles(ctx, f(addr), f(tj), f(m), f(x), f(v), f(a), f(k))
+            nb.nbk_set_ti(ctx, t)
+            nb.nbk_calc_firsthalf(ctx, n, n, None, None, None, np.float32(EPS) ** 2, FULL)
+            if pinned:
+                out = (pin(np.empty((n, 3), np.float32)), pin(np.empty((n, 3), np.float32)), pin(np.empty(n, np.float32)))
+                got = nb.nbk_calc_lasthalf(ctx, n, out=out)
+                assert got[0] is out[0] and got[2] is out[2]
+            else:
+                got = nb.nbk_calc_lasthalf(ctx, n)
+            return tuple(np.array(g) for g in got)
+
+    plain, direct = run(False), run(True)
+    for p, d in zip(plain, direct):
+        assert np.array_equal(p, d)
+    # against the oracle: particle addr[q] holds input row q
+    xs, vs, ms = np.empty_like(x), np.empty_like(v), np.empty_like(m)
+    as_, ks, ts = np.empty_like(a), np.empty_like(k), np.empty_like(tj)
+    xs[addr], vs[addr], ms[addr], as_[addr], ks[addr], ts[addr] = x, v, m, a, k, tj
+    xp, vp = c_oracle.predict(t, ts, xs, vs, as_, ks)
+    ref = c_oracle.force(ms, xp.astype(np.float32), vp.astype(np.float32), EPS)
+    assert_parity(direct, ref, what="pinned direct path")
+    with pytest.raises(ValueError):
+        with Ctx(64) as ctx:
+            gpu_force(ctx, m[:64], x[:64], v[:64], EPS)
+            nb.nbk_calc_lasthalf(ctx, 64, out=(np.empty((64, 3)), np.empty((64, 3), np.float32), np.empty(64, np.float32)))
