@@ -474,6 +474,43 @@ def run_sharded(args, wl):
     return 0
 
 
+def run_hermite(args):
+    """--hermite host|dev: BASELINE.json config C5 (N = 65536 Plummer sphere, seed 5, eps = 1/256, eta = 0.01) integrated
+    to --t-end with the host-driven (a8) or the device-resident (8(f)-1) block-step loop.  Prints wall time, block-step
+    statistics and |dE/E| with the energies taken from the library's own fp32 potential (the fp64-oracle figure is in
+    tests/test_gpu_configs.py).  Not the bench line."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --hermite needs a CUDA device")
+    from paper_0707_0438_b200 import binding as nb
+    from paper_0707_0438_b200 import inputs
+    nb.load()
+    cfg = inputs.CONFIGS["C5"]
+    n, eps = cfg["N"], 1.0 / 256.0
+    m, x, v = inputs.plummer(n, cfg["seed"])
+    ctx = nb.nbk_open(0, n, n)
+
+    def energy():
+        nb.nbk_set_j_particles_f64(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, n, n, None, None, None, float(np.float32(eps) ** 2), nb.NBK_POT)
+        pot = nb.nbk_calc_lasthalf_f64(ctx, n)[2]
+        return float(0.5 * np.sum(m * np.sum(v * v, axis=1)) + 0.5 * np.sum(m * pot))
+    try:
+        e0 = energy()
+        fn = nb.nbk_hermite_evolve_dev if args.hermite == "dev" else nb.nbk_hermite_evolve
+        st = fn(ctx, m, x, v, eps, args.t_end, 0.01, args.dt_max)
+        e1 = energy()
+    finally:
+        nb.nbk_close(ctx)
+    print(json.dumps({"workload": f"C5: N={n} Plummer seed {cfg['seed']}, eps=1/256, eta=0.01, dt_max={args.dt_max}, to t={args.t_end}",
+                      "loop": "device-resident" if args.hermite == "dev" else "host-driven", "wall_s": st["wall_seconds"],
+                      "block_steps": st["block_steps"], "particle_steps": st["particle_steps"],
+                      "interactions": st["interactions"], "interactions_per_s": st["interactions"] / st["wall_seconds"],
+                      "dE_over_E_gpu_potential": (e0 - e1) / e0, "ni_histogram_log2": st["ni_histogram"][:18]}), flush=True)
+    return 0
+
+
 def run_sweep(args):
     """--sweep: the paper's Table 3 / Table 4 shape (kernel-only time against N)
     plus the block-step i-set sizes of config C2, as a markdown table on stdout.  Not the bench line."""
@@ -637,7 +674,13 @@ def main(argv=None):
                          "default: independent replicas (weak)")
     ap.add_argument("--transport", choices=["nccl", "peer"], default="nccl",
                     help="with --shard j: exchange by NCCL all-reduces, or by loads from peer (symmetric) memory")
+    ap.add_argument("--hermite", choices=["host", "dev"], default=None,
+                    help="integrate config C5 with the host-driven or the device-resident Hermite loop and print wall time")
+    ap.add_argument("--t-end", type=float, default=1.0)
+    ap.add_argument("--dt-max", type=float, default=1.0 / 16.0)
     args = ap.parse_args(argv)
+    if args.hermite:
+        return run_hermite(args)
     if args.sweep:
         return run_sweep(args)
     wl = WORKLOADS[args.workload]
