@@ -211,6 +211,8 @@ typedef struct nbk_hermite_stats {
  * fp64, forces from this context (which must have n_max >= n, ni_max >= n).
  * m[n], x[n][3], v[n][3] are HOST fp64 arrays, updated in place to the state at t_end
  * (t_end must be a multiple of dt_max so that all particles are synchronised there).
+ * dt_max is rounded down to a power of two and must lie in [2^-48, 2): step levels are 2^-k with
+ * k in [0, 48]; anything else (dt_max >= 2 included), t_end > 2047 or eta <= 0 is NBK_EINVAL.
  * stats may be NULL. */
 int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, double* x, double* v,
                        double eps, double t_end, double eta, double dt_max,
@@ -221,8 +223,8 @@ int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, double* x, doub
  * is four stream-ordered launches -- predictor + selection of the particles due, i x j force kernel
  * planned on the device, reduction, fp64 corrector + Aarseth step + block rule whose last block also
  * schedules the next step (next block time from per-level particle counts) -- replayed from a CUDA
- * graph in batches of 256 steps with no host synchronisation in between.  Same scheme, formulas and arguments as nbk_hermite_evolve (dt_max
- * <= 1); stats->gpu_call_seconds equals wall_seconds. */
+ * graph in batches of 256 steps with no host synchronisation in between.  Same scheme, formulas, arguments
+ * and argument limits as nbk_hermite_evolve; stats->gpu_call_seconds equals wall_seconds. */
 int nbk_hermite_evolve_dev(nbk_ctx* ctx, int64_t n, const double* m, double* x, double* v,
                            double eps, double t_end, double eta, double dt_max,
                            nbk_hermite_stats* stats);

@@ -162,6 +162,7 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
                   const float* d_xi, const float* d_vi, float eps2, uint32_t flags,
                   const int32_t* h_inline = nullptr, bool to_host = false,
                   double* sum64 = nullptr) {
+    eps2 = flushed_eps2(eps2);
     if (!c->pred_valid || c->pred_nj != n_j) {
         const int rc = do_predict(c, n_j);
         if (rc != NBK_OK) return rc;
@@ -189,6 +190,7 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     d.G = 0;
     plan_shape(n_i, n_j, c->num_sms, c->force_I, c->partial_bytes / sizeof(float), &v, &d);
     if (d.G < 1 || plan_partial_floats(d) * sizeof(float) > c->partial_bytes) return NBK_ENOMEM;
+    if ((d.P + d.G - 1) / d.G > INT_MAX) return NBK_ERANGE;   // the kernel counts a CTA's pairs in an int
 
     ForceArgs fa;
     fa.dyn = nullptr;
@@ -302,6 +304,13 @@ int set_j_host(nbk_ctx* c, long long n, const int32_t* addr, const double* tj, c
         c->pred_valid = false;
         return NBK_OK;
     }
+    {   // padded size of [tj | m | x | v | a | jerk | addr], checked before anything is copied
+        const size_t un = static_cast<size_t>(n);
+        auto pad = [](size_t b) { return (b + 15) & ~static_cast<size_t>(15); };
+        const size_t need = pad(sizeof(double) * un) + pad(sizeof(T) * un) + 4 * pad(sizeof(T) * 3 * un) +
+                            pad(sizeof(int32_t) * un);
+        if (need > c->stage_bytes) return NBK_ENOMEM;
+    }
     NBK_CUDA(c, cudaEventSynchronize(c->stage_free));
     // pack [tj | m | x | v | a | jerk | addr] into the pinned buffer: one H2D copy
     size_t off = 0;
@@ -332,7 +341,6 @@ int set_j_host(nbk_ctx* c, long long n, const int32_t* addr, const double* tj, c
     const size_t o_a = put(a, sizeof(T) * 3 * n);
     const size_t o_k = put(jerk, sizeof(T) * 3 * n);
     const size_t o_ad = put(addr, sizeof(int32_t) * n);
-    if (off > c->stage_bytes) return NBK_ENOMEM;
     if (direct) {
         NBK_CUDA(c, derr);
         NBK_CUDA(c, cudaEventRecord(c->stage_free, c->stream));

@@ -17,6 +17,7 @@ int batch_impl(nbk_ctx* c, int64_t n_groups, const int64_t* i_offset, const floa
                const int64_t* j_offset, const float* mj, const float* xj, float eps2, uint32_t flags,
                float* acc, float* pot, bool dev) {
     if (!c || n_groups < 0 || !(eps2 >= 0.f) || (flags & (NBK_JERK | NBK_NN))) return NBK_EINVAL;
+    eps2 = flushed_eps2(eps2);
     if (n_groups == 0) return NBK_OK;
     if (!i_offset || !j_offset || i_offset[0] != 0 || j_offset[0] != 0) return NBK_EINVAL;
     for (int64_t g = 0; g < n_groups; ++g)

@@ -13,6 +13,10 @@ namespace nbk {
 
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
 
+// The kernels' arithmetic flushes subnormals to zero (.ftz): a subnormal eps2 IS eps2 = 0 to them, so
+// it must select the zero-distance mask like an exact 0 does.
+inline float flushed_eps2(float eps2) { return eps2 < 1.17549435e-38f ? 0.f : eps2; }
+
 struct DeviceGuard {  // make the context's device current for the call, restore on exit
     int prev = -1;
     bool ok = true;

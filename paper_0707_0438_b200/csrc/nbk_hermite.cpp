@@ -23,11 +23,13 @@
 #include <vector>
 
 #include "../../include/nbk.h"
+#include "nbk_hermite_common.h"
 
 namespace {
 
-constexpr int kTickLog2 = 52;  // time unit 2^-52: exact integer block times up to t = 2048
-constexpr int kMaxLevel = 48;  // finest allowed step 2^-48
+using nbk::kMaxLevel;
+using nbk::kTickLog2;
+using nbk::level_for;
 
 struct Clock {
     std::chrono::steady_clock::time_point t0 = std::chrono::steady_clock::now();
@@ -36,18 +38,7 @@ struct Clock {
     }
 };
 
-inline double norm3(const double* a) { return std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]); }
-
-// largest level-step 2^-k <= want, clamped to [2^-kMaxLevel, 2^-kmin]
-inline int level_for(double want, int kmin) {
-    if (!(want > 0.0)) return kMaxLevel;
-    int e;
-    std::frexp(want, &e);           // want = f * 2^e, f in [0.5, 1)  =>  2^(e-1) <= want
-    int k = -(e - 1);
-    if (k < kmin) k = kmin;
-    if (k > kMaxLevel) k = kMaxLevel;
-    return k;
-}
+using nbk::norm3;
 
 struct Levels {
     std::vector<std::vector<int32_t>> list;
@@ -81,7 +72,8 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
     if (!ctx || n < 1 || !m || !x || !v || !(eps >= 0.0) || !(t_end >= 0.0) || !(eta > 0.0) ||
         !(dt_max > 0.0) || n > INT32_MAX)
         return NBK_EINVAL;
-    const int kmin = level_for(dt_max, -10);  // dt_max rounded down to a power of two
+    const int kmin = nbk::level_of_dt_max(dt_max);  // dt_max rounded down to a power of two
+    if (kmin < 0) return NBK_EINVAL;                // dt_max in [2^-48, 2): levels are indexed from 0
     const double dtm = std::ldexp(1.0, -kmin);
     if (t_end > 2047.0 || std::fmod(t_end, dtm) != 0.0) return NBK_EINVAL;
     const int64_t T_end = static_cast<int64_t>(std::ldexp(t_end, kTickLog2));
@@ -125,10 +117,8 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
     st.interactions += n * n;
     for (size_t i = 0; i < N; ++i) {
         for (int c = 0; c < 3; ++c) { a[3 * i + c] = fa[3 * i + c]; jk[3 * i + c] = fj[3 * i + c]; }
-        const double na = norm3(&a[3 * i]), nj = norm3(&jk[3 * i]);
-        double want = dtm;
-        if (nj > 0.0 && na > 0.0) want = std::fmin(0.25 * eta * na / nj, dtm);
-        L.insert(static_cast<int32_t>(i), level_for(want, kmin));
+        L.insert(static_cast<int32_t>(i),
+                 nbk::startup_level(norm3(&a[3 * i]), norm3(&jk[3 * i]), eta, kmin));
     }
     NBK_TIMED(nbk_set_j_particles_f64(ctx, n, nullptr, tl.data(), m, x, v, a.data(), jk.data()));
 
@@ -188,22 +178,7 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
             }
             tl[i] = t_new;
             // Aarseth criterion and block rule
-            const double na = norm3(a1), nj = norm3(j1), n2 = norm3(a2e), n3 = norm3(a3);
-            const double num = na * n2 + nj * nj, den = nj * n3 + n2 * n2;
-            double want = dtm;
-            if (den > 0.0) {
-                const double dta = std::sqrt(eta * num / den);
-                if (dta == dta && dta > 0.0) want = std::fmin(dta, dtm);
-            }
-            int k = L.lev[i];
-            const double dt_old = std::ldexp(1.0, -k);
-            if (want < dt_old) {
-                const int kn = level_for(want, kmin);
-                k = kn > k ? kn : k;
-            } else if (want >= 2.0 * dt_old && k > kmin &&
-                       T_new % (int64_t(1) << (kTickLog2 - (k - 1))) == 0) {
-                k -= 1;
-            }
+            const int k = nbk::next_level(a1, j1, a2e, a3, eta, L.lev[i], kmin, T_new);
             knew[q] = k;
             bt[q] = t_new;
             bm[q] = m[i];

@@ -1,0 +1,77 @@
+// nbk_hermite_common.h -- the pieces of reading R15 that both Hermite drivers share:
+// the power-of-two level of a wanted step and the start-up step.  One copy, used by the host driver
+// (nbk_hermite.cpp), the device-resident driver's set-up (nbk_hermite_dev.cu) and its kernels
+// (nbk_hermite_kernels.cu).  Plain C++ usable from host and device code; internal to the CUDA path.
+//
+// PAPER.md L68, L74 name the scheme (4th-order Hermite, block time steps) and print no formula; the
+// start-up rule is reading R15: dt_0 = largest 2^-k <= min((eta / 4) |a| / |jerk|, dt_max).
+#pragma once
+#include <math.h>
+
+#if defined(__CUDACC__)
+#define NBK_HD __host__ __device__
+#else
+#define NBK_HD
+#endif
+
+namespace nbk {
+
+constexpr int kTickLog2 = 52;   // time unit 2^-52: exact integer block times up to t = 2048
+constexpr int kMaxLevel = 48;   // finest step 2^-48
+
+// Level k of the largest step 2^-k <= want, clamped to [kmin, kMaxLevel] (kmin >= 0: dt_max <= 1).
+NBK_HD inline int level_for(double want, int kmin) {
+    if (!(want > 0.0)) return kMaxLevel;
+    int e;
+    frexp(want, &e);            // want = f 2^e, f in [0.5, 1)  =>  2^(e-1) <= want < 2^e
+    int k = -(e - 1);
+    if (k < kmin) k = kmin;
+    if (k > kMaxLevel) k = kMaxLevel;
+    return k;
+}
+
+// Level of dt_max rounded down to a power of two, or -1 if that is outside [2^-kMaxLevel, 1]
+// (dt_max >= 2 or < 2^-48: both drivers refuse it with NBK_EINVAL).
+NBK_HD inline int level_of_dt_max(double dt_max) {
+    if (!(dt_max > 0.0) || dt_max >= 2.0) return -1;
+    int e;
+    frexp(dt_max, &e);
+    const int k = -(e - 1);
+    return (k < 0 || k > kMaxLevel) ? -1 : k;
+}
+
+// Start-up level (reading R15): step (eta / 4) |a| / |jerk|, dt_max if either norm vanishes.
+NBK_HD inline int startup_level(double norm_a, double norm_jerk, double eta, int kmin) {
+    const double dtm = ldexp(1.0, -kmin);
+    double want = dtm;
+    if (norm_jerk > 0.0 && norm_a > 0.0) want = fmin(0.25 * eta * norm_a / norm_jerk, dtm);
+    return level_for(want, kmin);
+}
+
+// New level after a corrected step (reading R15): Aarseth criterion
+//   dt_A = sqrt(eta (|a1| |a2'| + |j1|^2) / (|j1| |a3| + |a2'|^2)),  a2' = a2 + a3 dt (end of the step),
+// then the block rule: the step may halve as often as needed, may double once and only if dt_A >= 2 dt,
+// 2 dt <= dt_max and the new block time T_new (in ticks of 2^-kTickLog2) is a multiple of 2 dt.
+NBK_HD inline double norm3(const double* a) { return sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]); }
+NBK_HD inline int next_level(const double* a1, const double* j1, const double* a2e, const double* a3,
+                             double eta, int k_old, int kmin, long long T_new) {
+    const double dtm = ldexp(1.0, -kmin), dt_old = ldexp(1.0, -k_old);
+    const double na = norm3(a1), nj = norm3(j1), n2 = norm3(a2e), n3 = norm3(a3);
+    const double num = na * n2 + nj * nj, den = nj * n3 + n2 * n2;
+    double want = dtm;
+    if (den > 0.0) {
+        const double dta = sqrt(eta * num / den);
+        if (dta == dta && dta > 0.0) want = fmin(dta, dtm);
+    }
+    int k = k_old;
+    if (want < dt_old) {
+        const int kn = level_for(want, kmin);
+        k = kn > k ? kn : k;
+    } else if (want >= 2.0 * dt_old && k > kmin &&
+               (T_new & ((1LL << (kTickLog2 - (k - 1))) - 1)) == 0) {
+        k -= 1;
+    }
+    return k;
+}
+
+}  // namespace nbk

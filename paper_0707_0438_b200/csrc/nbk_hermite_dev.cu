@@ -23,18 +23,15 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
         !(dt_max > 0.0) || n > INT32_MAX)
         return NBK_EINVAL;
     if (n > c->n_max || n > c->ni_max) return NBK_ERANGE;
-    int e0;
-    std::frexp(dt_max, &e0);
-    int kmin = -(e0 - 1);            // dt_max rounded down to a power of two
-    if (kmin < -10) kmin = -10;
-    if (kmin < 0 || kmin > kMaxLevel) return NBK_EINVAL;   // dt_max in (2^-48, 1]... 2^0
+    const int kmin = level_of_dt_max(dt_max);   // dt_max rounded down to a power of two
+    if (kmin < 0) return NBK_EINVAL;            // dt_max in [2^-48, 2)
     const double dtm = std::ldexp(1.0, -kmin);
     if (t_end > 2047.0 || std::fmod(t_end, dtm) != 0.0) return NBK_EINVAL;
     DeviceGuard g(c->device);
     if (!g.ok) return cuda_fail(c, cudaErrorInvalidDevice);
     const auto wall0 = std::chrono::steady_clock::now();
     const size_t N = static_cast<size_t>(n);
-    const float eps2 = static_cast<float>(eps * eps);
+    const float eps2 = flushed_eps2(static_cast<float>(eps * eps));
     const uint32_t flags = NBK_JERK | NBK_POT;
     int rc;
 
@@ -73,17 +70,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
             na += a[3 * i + q] * a[3 * i + q];
             nj += jk[3 * i + q] * jk[3 * i + q];
         }
-        na = std::sqrt(na); nj = std::sqrt(nj);
-        double want = dtm;
-        if (nj > 0.0 && na > 0.0) want = std::fmin(0.25 * eta * na / nj, dtm);
-        int k = kMaxLevel;
-        if (want > 0.0) {
-            int e;
-            std::frexp(want, &e);
-            k = -(e - 1);
-            if (k < kmin) k = kmin;
-            if (k > kMaxLevel) k = kMaxLevel;
-        }
+        const int k = startup_level(std::sqrt(na), std::sqrt(nj), eta, kmin);
         lev[i] = k;
         H.level_count[k] += 1;
     }

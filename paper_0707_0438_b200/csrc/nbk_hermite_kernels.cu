@@ -129,18 +129,6 @@ __global__ void __launch_bounds__(256) hd_predict_kernel(const RawJ raw, DynHead
     }
 }
 
-__device__ __forceinline__ double norm3d(const double* a) {
-    return sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
-}
-__device__ __forceinline__ int level_for_dev(double want, int kmin) {
-    if (!(want > 0.0)) return kMaxLevel;
-    int e;
-    frexp(want, &e);
-    int k = -(e - 1);
-    if (k < kmin) k = kmin;
-    if (k > kMaxLevel) k = kMaxLevel;
-    return k;
-}
 
 // a8 on the device: Hermite corrector, Aarseth step, block rule (fp64), one thread per due particle;
 // writes the fp64 state, the level lists' counts and the raw j-state the predictor reads.
@@ -179,20 +167,7 @@ __global__ void hd_correct_kernel(const RawJ raw, DynHeader* h, const HermiteSta
         raw.k[c * raw.cap + i] = static_cast<float>(j1[c]);
     }
     raw.t[i] = h->t_next;
-    const double na = norm3d(a1), nj = norm3d(j1), n2 = norm3d(a2e), n3 = norm3d(a3);
-    const double num = na * n2 + nj * nj, den = nj * n3 + n2 * n2;
-    double want = dtm;
-    if (den > 0.0) {
-        const double dta = sqrt(h->eta * num / den);
-        if (dta == dta && dta > 0.0) want = fmin(dta, dtm);
-    }
-    int k = k0;
-    if (want < dt) {
-        const int kn = level_for_dev(want, h->kmin);
-        k = kn > k ? kn : k;
-    } else if (want >= 2.0 * dt && k > h->kmin && (T_next & ((1LL << (kTickLog2 - (k - 1))) - 1)) == 0) {
-        k -= 1;
-    }
+    const int k = next_level(a1, j1, a2e, a3, h->eta, k0, h->kmin, T_next);
     if (k != k0) {
         hs.level[i] = k;
         atomicAdd(reinterpret_cast<unsigned long long*>(&h->level_count[k0]), ~0ULL);   // -1

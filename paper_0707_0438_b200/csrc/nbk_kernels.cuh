@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "nbk_hermite_common.h"
+
 namespace nbk {
 
 constexpr int kTileJMax = 256;  // largest j-tile (particles); ring slots are sized for it
@@ -138,8 +140,7 @@ size_t plan_partial_floats(const Decomp& d);
 size_t plan_partial_floats_bound(long long ni_max, int num_sms);
 
 // ---- device-resident Hermite integrator: all block-step state lives here ------
-constexpr int kTickLog2 = 52;   // time unit 2^-52: exact integer block times
-constexpr int kMaxLevel = 48;   // finest step 2^-48
+// kTickLog2 (time unit 2^-52) and kMaxLevel (finest step 2^-48): nbk_hermite_common.h
 struct DynHeader {
     long long T_now, T_end, T_next;     // block times in ticks
     double t_next;                      // T_next in time units

@@ -648,3 +648,102 @@ def test_caller_owned_workspace_and_double_readback(gpu, c_oracle):
         assert b.dtype == np.float64 and np.array_equal(a.astype(np.float64), b)
     ref_nn, ref_r2 = c_oracle.nearest_neighbour(x)
     _check_nn(nn, r2, ref_nn, ref_r2, x, np.arange(n), what="workspace ctx nn")
+
+
+# ----------------------------------------------------------------------------- round-2 additions
+def test_set_j_dev_with_addresses_times_and_derivatives(gpu, c_oracle):
+    """a1 for a device-resident caller (PAPER.md L427 GPU_set_j_particle: address, time, mass, x, v,
+    a, jerk): nbk_set_j_particles_dev with DEVICE addr, tj, a, jerk in two shuffled batches, then the
+    device predictor (a3) and a force block: predicted state and forces against the oracle."""
+    torch = gpu
+    n = 5000
+    m, x, v = inputs.plummer_f32(n, seed=91)
+    t = 0.01
+    tj = inputs.particle_times(n, t, seed=9)
+    a, jk = inputs.gaussian_derivatives(n, seed=9)
+    a, jk = a.astype(np.float32), jk.astype(np.float32)
+    perm = np.random.default_rng(12).permutation(n).astype(np.int32)
+    xp, vp = c_oracle.predict(t, tj, x, v, a, jk)
+    idx = inputs.active_block(n, 777, seed=4)
+    keep = []
+    with Ctx(n) as ctx:
+        for part in (perm[:1803], perm[1803:]):
+            dev = [torch.from_numpy(np.ascontiguousarray(arr[part])).cuda() for arr in (tj, m, x, v, a, jk)]
+            dad = torch.from_numpy(part.copy()).cuda()
+            keep += dev + [dad]
+            torch.cuda.synchronize()
+            nb.nbk_set_j_particles_dev(ctx, part.shape[0], dad.data_ptr(), *[d.data_ptr() for d in dev])
+        nb.nbk_set_ti(ctx, t)
+        nb.nbk_calc_firsthalf(ctx, n, 777, idx, None, None, np.float32(EPS) ** 2, FULL)
+        got = nb.nbk_calc_lasthalf(ctx, 777)
+        gm, gx, gv = nb.nbk_get_predicted(ctx, n)
+    assert np.array_equal(gm, m)
+    for g, ref in ((gx, xp), (gv, vp)):
+        ulp = np.spacing(np.abs(ref).astype(np.float32)).astype(np.float64)
+        assert np.all(np.abs(g.astype(np.float64) - ref) <= ulp)
+        assert np.mean(g == ref.astype(np.float32)) > 0.99
+    assert_parity(got, c_oracle.force(m, xp, vp, EPS, i_index=idx), what="set_j_dev addr/tj/a/jerk")
+
+
+@pytest.mark.parametrize("driver", ["host", "dev"])
+def test_hermite_start_up_step_closed_form(gpu, driver):
+    """Reading R15's start-up step dt_0 = largest 2^-k <= (eta/4)|a|/|j| through the C ABI, on a case
+    with a closed form (same as tests/test_hermite_oracle.py): equal masses 1/2 on a circular orbit of
+    separation 1, eps = 0: |a| = |j| = 1/2, (0.01/4) -> 2^-9.  The Aarseth step of a circle (0.1) exceeds
+    dt_max = 1/16, so the step doubles whenever the block rule allows: 2^-9, 2^-9, 2^-8, 2^-7, 2^-6,
+    2^-5 reach t = 1/16 in exactly 6 block steps of 2 particles (5 if dt_0 were 2^-8, 4 if 2^-7)."""
+    m = np.array([0.5, 0.5])
+    x0 = np.array([[-0.5, 0, 0], [0.5, 0, 0]])
+    v0 = np.array([[0, -0.5, 0], [0, 0.5, 0]])
+    fn = nb.nbk_hermite_evolve if driver == "host" else nb.nbk_hermite_evolve_dev
+    with Ctx(64) as ctx:
+        x, v = x0.copy(), v0.copy()
+        st = fn(ctx, m, x, v, 0.0, 1.0 / 16.0, eta=0.01, dt_max=1.0 / 16.0)
+        assert st["t_reached"] == 1.0 / 16.0
+        assert st["block_steps"] == 6 and st["particle_steps"] == 12
+        assert sum(st["ni_histogram"]) == 6
+        # one step of dt_max = 2^-9 lands exactly on t_end = 2^-9
+        x, v = x0.copy(), v0.copy()
+        st = fn(ctx, m, x, v, 0.0, 2.0 ** -9, eta=0.01, dt_max=2.0 ** -9)
+        assert st["block_steps"] == 1 and st["particle_steps"] == 2
+    # the orbit: after t the pair has turned by the angle t (omega = 1)
+    ang = 2.0 ** -9
+    np.testing.assert_allclose(x[1], [0.5 * np.cos(ang), 0.5 * np.sin(ang), 0.0], atol=1e-9)
+
+
+@pytest.mark.parametrize("driver", ["host", "dev"])
+def test_hermite_drivers_refuse_dt_max_of_two_or_more(gpu, driver):
+    """dt_max in [2^-48, 2): the level lists are indexed from 2^0 (include/nbk.h); 2 and above, and
+    non-positive or NaN values, are NBK_EINVAL in both drivers (no out-of-range level)."""
+    m, x, v = inputs.plummer(64, seed=5)
+    fn = nb.nbk_hermite_evolve if driver == "host" else nb.nbk_hermite_evolve_dev
+    with Ctx(64) as ctx:
+        for bad in (2.0, 4.0, 1024.0, 0.0, -1.0, float("nan"), 2.0 ** -60):
+            with pytest.raises(nb.NbkError) as e:
+                fn(ctx, m, x.copy(), v.copy(), EPS, 1024.0 if bad > 2 else 2.0, eta=0.01, dt_max=bad)
+            assert e.value.status == nb.NBK_EINVAL, bad
+        st = fn(ctx, m, x.copy(), v.copy(), EPS, 1.0, eta=0.01, dt_max=1.9)   # rounds down to 2^0
+        assert st["t_reached"] == 1.0 and st["block_steps"] > 16
+
+
+@pytest.mark.parametrize("n,n_i", [(1024, 1024), (300, 7)])
+def test_subnormal_softening_is_zero_softening(gpu, c_oracle, n, n_i):
+    """The kernels flush subnormals (.ftz): eps = 1e-20 (eps^2 = 1e-40, a subnormal fp32) must act as
+    eps = 0 -- own entry and zero-distance pairs skipped -- not produce NaN."""
+    m, x, v = inputs.plummer_f32(n, seed=33)
+    x[5] = x[9]                                    # a coincident pair besides the own entries
+    idx = inputs.active_block(n, n_i, seed=1) if n_i < n else None
+    if idx is not None:
+        idx[0] = 5
+        idx = np.unique(idx).astype(np.int32)
+        n_i = idx.shape[0]
+    eps2 = np.float32(1e-40)
+    assert 0 < eps2 < np.finfo(np.float32).tiny
+    ref = c_oracle.force(m, x, v, 0.0, i_index=idx)
+    with Ctx(n) as ctx:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, n, n_i, idx, None, None, eps2, FULL)
+        got = nb.nbk_calc_lasthalf(ctx, n_i)
+    assert all(np.isfinite(g).all() for g in got)
+    assert_parity(got, ref, what="subnormal eps2")

@@ -108,3 +108,53 @@ def test_block_steps_commensurate_and_energy_small_plummer():
     assert out["particle_steps"] > out["block_steps"] > 2
     e1 = no.energy(m, out["x"], out["v"], eps)
     assert abs(no.relative_energy_error(e0, e1)) < 1e-7
+
+
+def test_initial_dt_hand_values():
+    """Start-up step, reading R15 (PAPER.md L68, L74 print no formula): dt_0 = largest 2^-k <=
+    min((eta / 4) |a| / |j|, dt_max).  Expected values worked by hand, not by the formula's code:
+      |a| = 1, |j| = 8,  eta = 0.01: (0.01/4)/8 = 3.125e-4;  2^-12 = 2.44e-4 <= 3.125e-4 < 2^-11 = 4.88e-4
+      |a| = 3, |j| = 0.5 (3-4-5 vectors): 0.0025 * 6 = 0.015;  2^-7 = 0.0078 <= 0.015 < 2^-6 = 0.0156
+      |a| = 2, |j| = 0.01: 0.0025 * 200 = 0.5 > dt_max = 1/16  -> dt_max
+      |j| = 0 -> dt_max;   |a| = 0 -> dt_max (a zero step is no step)
+      exact power of two: |a| = 1, |j| = 0.64, eta = 0.01: 0.0025/0.64 = 2^-8 exactly -> 2^-8
+    With eta/2 the first row gives 2^-11, with eta 2^-10: the pin tells the readings apart."""
+    a = np.array([[1.0, 0, 0], [0, 1.8, 2.4], [0, 0, -2.0], [0.3, 0.1, 0.2], [0, 0, 0], [0, -1.0, 0]])
+    j = np.array([[0, 8.0, 0], [0.3, 0, -0.4], [0.01, 0, 0], [0, 0, 0], [1.0, 2.0, 3.0], [0.64, 0, 0]])
+    dt = ho.initial_dt(a, j, 0.01, 1 / 16)
+    np.testing.assert_array_equal(dt, [2.0 ** -12, 2.0 ** -7, 1 / 16, 1 / 16, 1 / 16, 2.0 ** -8])
+    # eta scales the step linearly: 4 eta -> two levels coarser, capped by dt_max
+    dt4 = ho.initial_dt(a, j, 0.04, 1 / 16)
+    np.testing.assert_array_equal(dt4, [2.0 ** -10, 2.0 ** -5, 1 / 16, 1 / 16, 1 / 16, 2.0 ** -6])
+    # dt_max itself is not rounded by this function's caller contract: a power of two comes back as is
+    np.testing.assert_array_equal(ho.initial_dt(a[:1], j[:1], 0.01, 2.0 ** -14), [2.0 ** -14])
+
+
+def test_evolve_takes_the_start_up_step_first():
+    """The integrator's first block time is the smallest start-up step (R15): circular two-body orbit
+    with |a| / |j| known in closed form.  Bodies m1 = m2 = 1/2 at separation d = 1, eps = 0: each feels
+    |a| = m / d^2 = 1/2; relative speed of a circular orbit v = sqrt(M/d) = 1, so |j| = m v / d^3 = 1/2
+    (r.w = 0 on a circle).  (eta/4) |a|/|j| = 0.0025 -> 2^-9 = 0.00195 (2^-8 = 0.0039 is too large)."""
+    m = np.array([0.5, 0.5])
+    x = np.array([[-0.5, 0, 0], [0.5, 0, 0]])
+    v = np.array([[0, -0.5, 0], [0, 0.5, 0]])
+    seen = []
+
+    def spy(m_, x_, v_, eps_, i_index=None):
+        seen.append(None if i_index is None else len(i_index))
+        return no.force(m_, x_, v_, eps_, i_index=i_index)
+
+    out = ho.evolve(m, x, v, 0.0, 2.0 ** -9, eta=0.01, dt_max=2.0 ** -9, force_fn=spy)
+    assert out["block_steps"] == 1 and np.all(out["t"] == 2.0 ** -9)
+    a, jk, _ = no.force(m, x, v, 0.0)
+    np.testing.assert_allclose(np.linalg.norm(a, axis=1), 0.5, rtol=1e-14)
+    np.testing.assert_allclose(np.linalg.norm(jk, axis=1), 0.5, rtol=1e-14)
+    np.testing.assert_array_equal(ho.initial_dt(a, jk, 0.01, 1 / 16), [2.0 ** -9, 2.0 ** -9])
+    # to t = 1/16 with dt_max = 1/16: 32 steps of 2^-9 if the step never changed; the Aarseth step of a
+    # circular orbit is sqrt(eta) / omega = 0.1 > dt_max, so the step doubles whenever the block rule allows
+    # and may double only at times that are multiples of the doubled step.  By hand: 2^-9 to t = 2^-9 (odd:
+    # no doubling), 2^-9 to 2^-8 (doubles), 2^-8 to 2^-7, 2^-7 to 2^-6, 2^-6 to 2^-5, 2^-5 to 2^-4: 6 steps.
+    # (A start-up step of 2^-8 would give 5, of 2^-7 4.)
+    out = ho.evolve(m, x, v, 0.0, 1 / 16, eta=0.01, dt_max=1 / 16)
+    assert out["block_steps"] == 6 and out["particle_steps"] == 12
+    np.testing.assert_array_equal(out["dt"], [2.0 ** -4, 2.0 ** -4])   # t = 2^-4 allows one more doubling

@@ -322,3 +322,37 @@ def test_nearest_neighbour_brute_force_subset_external_and_degenerate(oracle):
     assert np.array_equal(nn, nn2)
     nn1, r1 = oracle.nearest_neighbour(x[:1])
     assert nn1[0] == -1 and np.isinf(r1[0])
+
+
+# --- the numpy form's i-chunk loop (more than _CHUNK_ELEMS pair temporaries): several chunks ---
+def test_numpy_form_across_i_chunks():
+    """n_i * N > 4 M pairs makes nbody_oracle.force walk several i-chunks.  Pins that a chunk's rows
+    land in the right slots: momentum sums over ALL i vanish (a shifted or dropped chunk breaks the
+    pairwise cancellation), and the rows on both sides of every chunk boundary equal a scalar loop
+    written from the definition (Eq. 1)."""
+    n = 3000
+    m, x, v = _rand(n, 77)
+    eps = 1.0 / 256.0
+    chunk = py_oracle._CHUNK_ELEMS // n
+    assert n > 2 * chunk                      # three chunks
+    acc, jrk, pot = py_oracle.force(m, x, v, eps)
+    assert np.abs((m[:, None] * acc).sum(0)).max() < 1e-13 * np.sum(m[:, None] * np.abs(acc))
+    assert np.abs((m[:, None] * jrk).sum(0)).max() < 1e-12 * np.sum(m[:, None] * np.abs(jrk))
+    for i in (0, chunk - 1, chunk, 2 * chunk - 1, 2 * chunk, n - 1):
+        a, jk, p = np.zeros(3), np.zeros(3), 0.0
+        for j in range(n):
+            if j == i:
+                continue
+            r, w = x[j] - x[i], v[j] - v[i]
+            s = r @ r + eps * eps
+            a += m[j] * r * s ** -1.5
+            jk += m[j] * (w * s ** -1.5 - 3.0 * (r @ w) * r * s ** -2.5)
+            p -= m[j] * s ** -0.5
+        np.testing.assert_allclose(acc[i], a, rtol=1e-11)
+        np.testing.assert_allclose(jrk[i], jk, rtol=1e-10, atol=1e-12 * np.abs(jk).max())
+        np.testing.assert_allclose(pot[i], p, rtol=1e-12)
+    # an i-subset that straddles a chunk boundary of its own (n_i = 1500 > chunk) with a permutation
+    idx = np.random.default_rng(3).permutation(n)[:1500]
+    acc_s, jrk_s, pot_s = py_oracle.force(m, x, v, eps, i_index=idx)
+    np.testing.assert_array_equal(acc_s, acc[idx])
+    np.testing.assert_array_equal(pot_s, pot[idx])
