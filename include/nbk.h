@@ -306,11 +306,11 @@ int nbk_last_launch(const nbk_ctx* ctx, int64_t out[8]);
  * CTA k works on pairs [k*P/G, (k+1)*P/G) of the i-major (i-tile, j-tile) list. */
 int nbk_plan(int64_t n_i, int64_t n_j, int num_sms, int force_i, int64_t out[12]);
 
-/* Measurement knobs.  bit 0: inner-loop form, 0 = packed f32x2 (FFMA2, two j per instruction;
- * default), 1 = scalar fp32.  bits 4-7: pin the i-particles per thread (1, 2, 4; 0 = planner's
- * choice).  bit 8: switch off the one-launch path for blocks of <= 32 i-particles (reduction by
- * the last CTA, indices in the launch parameters, results written to mapped host memory).  All
- * forms compute the same sums. */
+/* Test and measurement knob, not needed by callers: pins a launch shape the planner would not
+ * pick so that the test matrix reaches every kernel form.  bits 4-7: pin the i-particles per
+ * thread (1, 2, 4; 0 = planner's choice).  bit 8: switch off the one-launch path for blocks of
+ * <= 32 i-particles (reduction by the last CTA, indices in the launch parameters, results
+ * written to mapped host memory).  Any other bit: NBK_EINVAL.  All forms compute the same sums. */
 int nbk_set_variant(nbk_ctx* ctx, int variant);
 
 int nbk_last_cuda_error(const nbk_ctx* ctx);

@@ -185,7 +185,6 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     v.jerk = (flags & NBK_JERK) != 0;
     v.eps0 = (flags & NBK_EPS0) != 0 || eps2 == 0.f;
     v.nn = (flags & NBK_NN) != 0;
-    v.packed = c->variant_scalar == 0 || v.nn;   // the neighbour search exists in the packed form
     c->last_nn = v.nn;
     d.G = 0;
     plan_shape(n_i, n_j, c->num_sms, c->force_I, c->partial_bytes / sizeof(float), &v, &d);
@@ -442,11 +441,10 @@ int open_impl(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cu
         c->raw.cap = c->n_cap;
         for (int I : {1, 2, 4})
             for (int jk = 0; jk < 2 && e == cudaSuccess; ++jk)
-                for (int e0 = 0; e0 < 2 && e == cudaSuccess; ++e0)
-                    for (int pk = 0; pk < 2 && e == cudaSuccess; ++pk) {
-                        Variant v{I, jk != 0, e0 != 0, pk != 0};
-                        e = force_prepare(v);
-                    }
+                for (int e0 = 0; e0 < 2 && e == cudaSuccess; ++e0) {
+                    Variant v{I, jk != 0, e0 != 0, false};
+                    e = force_prepare(v);
+                }
         if (e != cudaSuccess) break;
         const size_t cap = static_cast<size_t>(c->n_cap);
         if ((e = dalloc(reinterpret_cast<void**>(&c->raw.x), sizeof(double) * 3 * cap)) != cudaSuccess) break;
@@ -875,7 +873,7 @@ int nbk_plan(int64_t n_i, int64_t n_j, int num_sms, int force_i, int64_t out[12]
     if (n_i < 1 || n_j < 1 || num_sms < 1 || !out || n_i > (1LL << 30) || n_j > (1LL << 30) ||
         !(force_i == 0 || force_i == 1 || force_i == 2 || force_i == 4))
         return NBK_EINVAL;
-    Variant v{0, true, false, true};
+    Variant v{0, true, false, false};
     Decomp d;
     d.G = 0;
     plan_shape(n_i, n_j, num_sms, force_i, plan_partial_floats_bound(n_i, num_sms), &v, &d);
@@ -888,10 +886,9 @@ int nbk_plan(int64_t n_i, int64_t n_j, int num_sms, int force_i, int64_t out[12]
 }
 
 int nbk_set_variant(nbk_ctx* c, int variant) {
-    if (!c || variant < 0) return NBK_EINVAL;
+    if (!c || variant < 0 || (variant & ~0x1f0)) return NBK_EINVAL;
     const int I = (variant >> 4) & 15;
     if (!(I == 0 || I == 1 || I == 2 || I == 4)) return NBK_EINVAL;
-    c->variant_scalar = variant & 1;
     c->force_I = I;
     c->fused_ok = (variant & 0x100) == 0;
     return NBK_OK;

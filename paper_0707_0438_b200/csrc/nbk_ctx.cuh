@@ -81,7 +81,6 @@ struct nbk_ctx {
 
     long long last_ni = -1;
     bool in_flight = false;
-    int variant_scalar = 0;
     int force_I = 0;
     bool fused_ok = true;  // nbk_set_variant bit 8 switches the one-launch small-block path off
     int last_cuda = 0;

@@ -5,14 +5,8 @@
 #pragma once
 #include "nbk_kernels.cuh"
 
-#ifndef NBK_USE_RCP
-#define NBK_USE_RCP 0
-#endif
 #ifndef NBK_FOLD
 #define NBK_FOLD 2     // j-tiles between folds of the fp32 accumulators into fp64 (power of two)
-#endif
-#ifndef NBK_UNROLL
-#define NBK_UNROLL 1   // trips of the 4-j step of the packed tile loop unrolled together
 #endif
 
 namespace nbk {
@@ -46,11 +40,6 @@ __device__ __forceinline__ void unpack(u64 d, float& lo, float& hi) {
 __device__ __forceinline__ float rsq(float x) {
     float y;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-__device__ __forceinline__ float rcp(float x) {
-    float y;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 
@@ -147,8 +136,7 @@ __device__ __forceinline__ void tile_packed(const float* __restrict__ sx, int jb
                                             u64 (&acc)[I][Shape<JERK>::nacc], float eps2,
                                             float (&tmin)[I]) {
     const u64 e2p = pack(eps2, eps2);
-    constexpr int kUnroll = NBK_UNROLL;
-#pragma unroll kUnroll
+#pragma unroll 1
     for (int jj = jbeg; jj < jend; jj += 4) {
         const ulonglong2 X = *reinterpret_cast<const ulonglong2*>(sx + jj);
         const ulonglong2 Y = *reinterpret_cast<const ulonglong2*>(sx + kTileJMax + jj);
@@ -197,9 +185,6 @@ __device__ __forceinline__ void tile_packed(const float* __restrict__ sx, int jb
                     rb = r2b > 0.f ? rb : 0.f;
                     rinv = pack(ra, rb);
                     rinv2 = mul2(rinv, rinv);
-                } else if (NBK_USE_RCP) {
-                    rinv = pack(ra, rb);
-                    rinv2 = pack(rcp(r2a), rcp(r2b));
                 } else {
                     rinv = pack(ra, rb);
                     rinv2 = mul2(rinv, rinv);
@@ -226,47 +211,6 @@ __device__ __forceinline__ void tile_packed(const float* __restrict__ sx, int jb
                     acc[q][8] = fma2(beta, dy, acc[q][8]);
                     acc[q][9] = fma2(beta, dz, acc[q][9]);
                 }
-            }
-        }
-    }
-}
-
-template <int I, bool JERK, bool EPS0, bool MASK>
-__device__ __forceinline__ void tile_scalar(const float* __restrict__ sx, int jbeg, int jend,
-                                            const float (&ni)[I][6], const int (&sl)[I],
-                                            float (&acc)[I][Shape<JERK>::nacc], float eps2) {
-#pragma unroll 2
-    for (int jj = jbeg; jj < jend; ++jj) {
-        const float xj = sx[jj], yj = sx[kTileJMax + jj], zj = sx[2 * kTileJMax + jj];
-        const float mj0 = sx[3 * kTileJMax + jj];
-        float vxj = 0.f, vyj = 0.f, vzj = 0.f;
-        if (JERK) {
-            vxj = sx[4 * kTileJMax + jj]; vyj = sx[5 * kTileJMax + jj]; vzj = sx[6 * kTileJMax + jj];
-        }
-#pragma unroll
-        for (int q = 0; q < I; ++q) {
-            const float mj = (MASK && jj == sl[q]) ? 0.f : mj0;
-            const float dx = xj + ni[q][0], dy = yj + ni[q][1], dz = zj + ni[q][2];
-            const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
-            float rinv = rsq(r2);
-            if (EPS0) rinv = r2 > 0.f ? rinv : 0.f;
-            const float rinv2 = (!EPS0 && NBK_USE_RCP) ? rcp(r2) : rinv * rinv;
-            const float mrinv = mj * rinv;
-            acc[q][3] += mrinv;
-            const float mrinv3 = mrinv * rinv2;
-            acc[q][0] = fmaf(mrinv3, dx, acc[q][0]);
-            acc[q][1] = fmaf(mrinv3, dy, acc[q][1]);
-            acc[q][2] = fmaf(mrinv3, dz, acc[q][2]);
-            if (JERK) {
-                const float dvx = vxj + ni[q][3], dvy = vyj + ni[q][4], dvz = vzj + ni[q][5];
-                const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
-                acc[q][4] = fmaf(mrinv3, dvx, acc[q][4]);
-                acc[q][5] = fmaf(mrinv3, dvy, acc[q][5]);
-                acc[q][6] = fmaf(mrinv3, dvz, acc[q][6]);
-                const float beta = (rv * rinv2) * mrinv3;
-                acc[q][7] = fmaf(beta, dx, acc[q][7]);
-                acc[q][8] = fmaf(beta, dy, acc[q][8]);
-                acc[q][9] = fmaf(beta, dz, acc[q][9]);
             }
         }
     }
@@ -317,19 +261,11 @@ __device__ __forceinline__ void nn_scan(const JPred& j, int n_j, int tile, int t
     }
 }
 
-template <bool PACKED> struct AccT { typedef float type; };
-template <> struct AccT<true> { typedef u64 type; };
-
 __device__ __forceinline__ float acc_take(u64& a) {
     float lo, hi;
     unpack(a, lo, hi);
     a = 0ull;
     return lo + hi;
-}
-__device__ __forceinline__ float acc_take(float& a) {
-    const float s = a;
-    a = 0.f;
-    return s;
 }
 
 

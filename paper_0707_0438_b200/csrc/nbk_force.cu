@@ -38,19 +38,18 @@
 
 namespace nbk {
 
-#ifdef NBK_TRACE
-__device__ long long nbk_trace_buf[3 * 4096];
-#endif
-
 
 // ------------------------------------------------------------------------------ force kernel
-template <int I, bool JERK, bool EPS0, bool PACKED, bool NN>
+template <int I, bool JERK, bool EPS0, bool NN>
 __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceArgs a) {
     using S = Shape<JERK>;
     constexpr int NACC = S::nacc;
     constexpr int W = warps_of(I);
     constexpr int T = W * 32;
-    typedef typename AccT<PACKED>::type acc_t;
+    // eps = 0 keeps the ring slots of a fold group until the group's sums are known to be finite
+    // (see below), so the producer runs fewer tiles ahead; a tile lasts tens of microseconds
+    constexpr int PF = EPS0 ? kPrefetch - NBK_FOLD : kPrefetch;
+    typedef u64 acc_t;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const uint32_t full0 = smem_u32(smem_raw);
     const uint32_t empty0 = full0 + 8 * kStages;
@@ -70,10 +69,6 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     const int warp = tid >> 5;
-#ifdef NBK_TRACE
-    long long trace_t0 = 0;
-    if (tid == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(trace_t0));
-#endif
     // launch plan: from the host (kernel parameters) or, for the device-resident integrator, from
     // the step header (made by hd_begin_kernel with the same function the host planner runs)
     Decomp dplan = a.d;
@@ -110,7 +105,7 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
     __syncthreads();
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < kPrefetch; ++s)
+        for (int s = 0; s < PF; ++s)
             if (s < n_local)
                 issue_tile<JERK>(a.j, (jt_first + s) % d.njt, d.tj, stages + s * S::stage_floats,
                                  full0 + 8 * s);
@@ -125,12 +120,13 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
     int it = it_first;
     int jt = jt_first;
     bool fresh = true;
+    int held_slot[NBK_FOLD], held_jt[NBK_FOLD], nheld = 0;   // EPS0: tiles of the open fold group
 
     for (int n = 0; n < n_local; ++n) {
         // producer: keep the ring kPrefetch tiles ahead; a slot is refilled once every warp has
         // arrived on its "empty" barrier (tile m - kStages was the slot's previous tenant)
         if (tid == 0) {
-            const int m = n + kPrefetch;
+            const int m = n + PF;
             if (m < n_local) {
                 const int slot = m % kStages;
                 if (m >= kStages) mbar_wait(empty0 + 8 * slot, ((m / kStages) - 1) & 1);
@@ -183,12 +179,16 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
             sl[q] = self[q] - jbase;
             mine |= static_cast<unsigned>(sl[q]) < static_cast<unsigned>(d.tj);
         }
+        // eps = 0 (zero-distance pairs contribute nothing).  Zero distance can
+        // only occur at the own entry (guarded copy of the loop, as for eps > 0 where its mass is
+        // zeroed) or between coincident distinct particles.  Every other tile runs the plain loop:
+        // there a zero distance makes rsqrt = inf and the potential sum non-finite, which the
+        // fold below tests once per group of NBK_FOLD tiles; only then the group is redone with
+        // the guarded loop.  Common case: no per-pair compare-and-select at all.
         if (__any_sync(0xffffffffu, mine)) {
-            if constexpr (PACKED) tile_packed<I, JERK, EPS0, true, NN>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2, tmin);
-            else tile_scalar<I, JERK, EPS0, true>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2);
+            tile_packed<I, JERK, EPS0, true, NN>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2, tmin);
         } else {
-            if constexpr (PACKED) tile_packed<I, JERK, EPS0, false, NN>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2, tmin);
-            else tile_scalar<I, JERK, EPS0, false>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2);
+            tile_packed<I, JERK, false, false, NN>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2, tmin);
         }
 
         if (NN) {
@@ -198,14 +198,56 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
                 tmin[q] = __int_as_float(0x7f800000);
             }
         }
-        // this warp is done with the ring slot
-        __syncwarp();
-        if (lane == 0) mbar_arrive(empty0 + 8 * slot);
+        if constexpr (EPS0) {   // released after the fold group's check
+#pragma unroll
+            for (int h = 0; h < NBK_FOLD; ++h)
+                if (h == nheld) { held_slot[h] = slot; held_jt[h] = jt; }
+            ++nheld;
+        } else {   // this warp is done with the ring slot
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty0 + 8 * slot);
+        }
 
         // second level: fold the fp32 sums into the thread's private fp64 slots, every NBK_FOLD tiles
         // (fp32 stays within <= NBK_FOLD * 128 terms per packed half) and at the end of a segment
         const bool last_of_tile = (jt == d.njt - 1) || (n == n_local - 1);
         if (last_of_tile || (jt & (NBK_FOLD - 1)) == NBK_FOLD - 1) {
+            if constexpr (EPS0) {
+                bool bad = false;
+#pragma unroll
+                for (int q = 0; q < I; ++q) {
+                    float lo, hi;
+                    unpack(acc[q][3], lo, hi);
+                    bad |= !(fabsf(lo + hi) < __int_as_float(0x7f800000));
+                }
+                if (__any_sync(0xffffffffu, bad)) {   // a coincident pair: redo the group, guarded
+#pragma unroll
+                    for (int q = 0; q < I; ++q) {
+#pragma unroll
+                        for (int v = 0; v < NACC; ++v) acc[q][v] = acc_t(0);
+                    }
+#pragma unroll
+                    for (int h = 0; h < NBK_FOLD; ++h) {
+                        if (h >= nheld) break;
+                        const float* hx = stages + held_slot[h] * S::stage_floats;
+                        int hl[I];   // the guarded loop with the own-entry mask serves every tile
+#pragma unroll
+                        for (int q = 0; q < I; ++q) hl[q] = self[q] - held_jt[h] * d.tj;
+                        tile_packed<I, JERK, true, true, NN>(hx, jbeg, jbeg + jlen, ni, hl, acc, a.eps2, tmin);
+                        if (NN) {   // the same minima as the first pass found
+#pragma unroll
+                            for (int q = 0; q < I; ++q) tmin[q] = __int_as_float(0x7f800000);
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) {
+#pragma unroll
+                    for (int h = 0; h < NBK_FOLD; ++h)
+                        if (h < nheld) mbar_arrive(empty0 + 8 * held_slot[h]);
+                }
+                nheld = 0;
+            }
 #pragma unroll
             for (int q = 0; q < I; ++q) {
 #pragma unroll
@@ -382,17 +424,6 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
             }
         }
     }
-#ifdef NBK_TRACE
-    if (tid == 0 && blockIdx.x < 4096) {
-        long long t1;
-        unsigned smid;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
-        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        nbk_trace_buf[3 * blockIdx.x] = trace_t0;
-        nbk_trace_buf[3 * blockIdx.x + 1] = t1;
-        nbk_trace_buf[3 * blockIdx.x + 2] = smid;
-    }
-#endif
 }
 
 // ----------------------------------------------------------------------------- reduce kernel
@@ -528,9 +559,9 @@ __global__ void __launch_bounds__(256) nn_scan_kernel(const NnScanArgs a) {
 
 
 // --------------------------------------------------------------------------------- launchers
-template <int I, bool JERK, bool EPS0, bool PACKED, bool NN>
+template <int I, bool JERK, bool EPS0, bool NN>
 static cudaError_t prepare_nn() {
-    auto fn = force_kernel<I, JERK, EPS0, PACKED, NN>;
+    auto fn = force_kernel<I, JERK, EPS0, NN>;
     const size_t smem = smem_bytes_of<I, JERK>();
     cudaError_t err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            static_cast<int>(smem));
@@ -541,62 +572,50 @@ static cudaError_t prepare_nn() {
     return nb >= 1 ? cudaSuccess : cudaErrorLaunchOutOfResources;
 }
 
-// the nearest-neighbour form exists for the packed acc + jerk + pot kernels only
-template <int I, bool JERK, bool EPS0, bool PACKED>
+// the nearest-neighbour form exists for the acc + jerk + pot kernels only
+template <int I, bool JERK, bool EPS0>
 static cudaError_t prepare_of() {
-    cudaError_t err = prepare_nn<I, JERK, EPS0, PACKED, false>();
+    cudaError_t err = prepare_nn<I, JERK, EPS0, false>();
     if (err != cudaSuccess) return err;
-    if constexpr (JERK && PACKED) err = prepare_nn<I, JERK, EPS0, PACKED, true>();
+    if constexpr (JERK) err = prepare_nn<I, JERK, EPS0, true>();
     return err;
 }
 
-template <int I, bool JERK, bool EPS0, bool PACKED>
+template <int I, bool JERK, bool EPS0>
 static cudaError_t launch_of(const ForceArgs& a, bool nn, cudaStream_t s) {
     const size_t smem = smem_bytes_of<I, JERK>();
-    if constexpr (JERK && PACKED) {
+    if constexpr (JERK) {
         if (nn) {
             if constexpr (I == 1)
-                return launch_pdl(force_kernel<I, JERK, EPS0, PACKED, true>, a.d.G, warps_of(I) * 32, smem, s, a);
-            force_kernel<I, JERK, EPS0, PACKED, true><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
+                return launch_pdl(force_kernel<I, JERK, EPS0, true>, a.d.G, warps_of(I) * 32, smem, s, a);
+            force_kernel<I, JERK, EPS0, true><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
             return cudaGetLastError();
         }
     }
     if (nn) return cudaErrorInvalidValue;
     if constexpr (I == 1)
-        return launch_pdl(force_kernel<I, JERK, EPS0, PACKED, false>, a.d.G, warps_of(I) * 32, smem, s, a);
-    force_kernel<I, JERK, EPS0, PACKED, false><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
+        return launch_pdl(force_kernel<I, JERK, EPS0, false>, a.d.G, warps_of(I) * 32, smem, s, a);
+    force_kernel<I, JERK, EPS0, false><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
     return cudaGetLastError();
 }
 
 #define NBK_DISPATCH(CALL, ...)                                                         \
     do {                                                                                \
-        const int key = (v.I == 1 ? 0 : v.I == 2 ? 1 : 2) * 8 + (v.jerk ? 4 : 0) +      \
-                        (v.eps0 ? 2 : 0) + (v.packed ? 1 : 0);                          \
+        const int key = (v.I == 1 ? 0 : v.I == 2 ? 1 : 2) * 4 + (v.jerk ? 2 : 0) +      \
+                        (v.eps0 ? 1 : 0);                                               \
         switch (key) {                                                                  \
-            case 0: return CALL<1, false, false, false>(__VA_ARGS__);                   \
-            case 1: return CALL<1, false, false, true>(__VA_ARGS__);                    \
-            case 2: return CALL<1, false, true, false>(__VA_ARGS__);                    \
-            case 3: return CALL<1, false, true, true>(__VA_ARGS__);                     \
-            case 4: return CALL<1, true, false, false>(__VA_ARGS__);                    \
-            case 5: return CALL<1, true, false, true>(__VA_ARGS__);                     \
-            case 6: return CALL<1, true, true, false>(__VA_ARGS__);                     \
-            case 7: return CALL<1, true, true, true>(__VA_ARGS__);                      \
-            case 8: return CALL<2, false, false, false>(__VA_ARGS__);                   \
-            case 9: return CALL<2, false, false, true>(__VA_ARGS__);                    \
-            case 10: return CALL<2, false, true, false>(__VA_ARGS__);                   \
-            case 11: return CALL<2, false, true, true>(__VA_ARGS__);                    \
-            case 12: return CALL<2, true, false, false>(__VA_ARGS__);                   \
-            case 13: return CALL<2, true, false, true>(__VA_ARGS__);                    \
-            case 14: return CALL<2, true, true, false>(__VA_ARGS__);                    \
-            case 15: return CALL<2, true, true, true>(__VA_ARGS__);                     \
-            case 16: return CALL<4, false, false, false>(__VA_ARGS__);                  \
-            case 17: return CALL<4, false, false, true>(__VA_ARGS__);                   \
-            case 18: return CALL<4, false, true, false>(__VA_ARGS__);                   \
-            case 19: return CALL<4, false, true, true>(__VA_ARGS__);                    \
-            case 20: return CALL<4, true, false, false>(__VA_ARGS__);                   \
-            case 21: return CALL<4, true, false, true>(__VA_ARGS__);                    \
-            case 22: return CALL<4, true, true, false>(__VA_ARGS__);                    \
-            default: return CALL<4, true, true, true>(__VA_ARGS__);                     \
+            case 0: return CALL<1, false, false>(__VA_ARGS__);                          \
+            case 1: return CALL<1, false, true>(__VA_ARGS__);                           \
+            case 2: return CALL<1, true, false>(__VA_ARGS__);                           \
+            case 3: return CALL<1, true, true>(__VA_ARGS__);                            \
+            case 4: return CALL<2, false, false>(__VA_ARGS__);                          \
+            case 5: return CALL<2, false, true>(__VA_ARGS__);                           \
+            case 6: return CALL<2, true, false>(__VA_ARGS__);                           \
+            case 7: return CALL<2, true, true>(__VA_ARGS__);                            \
+            case 8: return CALL<4, false, false>(__VA_ARGS__);                          \
+            case 9: return CALL<4, false, true>(__VA_ARGS__);                           \
+            case 10: return CALL<4, true, false>(__VA_ARGS__);                          \
+            default: return CALL<4, true, true>(__VA_ARGS__);                           \
         }                                                                               \
     } while (0)
 
@@ -637,9 +656,3 @@ cudaError_t launch_nn_scan(const NnScanArgs& a, cudaStream_t s) {
 
 
 }  // namespace nbk
-
-#ifdef NBK_TRACE
-extern "C" int nbk_debug_trace(long long* out, int n) {
-    return static_cast<int>(cudaMemcpyFromSymbol(out, nbk::nbk_trace_buf, sizeof(long long) * 3 * n));
-}
-#endif

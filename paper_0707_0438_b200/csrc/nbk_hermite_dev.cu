@@ -100,7 +100,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
 
     // one block step = predict + select, force (+ reduce), correct + next step's header; enqueued in batches with
     // no host synchronisation inside a batch; steps past t_end return at once (done flag)
-    Variant vv{1, true, eps2 == 0.f, true, false};
+    Variant vv{1, true, eps2 == 0.f, false};
     const long long n_pad = round_up_ll(n, kTileJMax);
     const size_t ni_max = static_cast<size_t>(c->ni_max);
     ForceArgs f;

@@ -79,8 +79,7 @@ struct Variant {
     int I;        // 1, 2 or 4
     bool jerk;
     bool eps0;
-    bool packed;  // f32x2 inner loop
-    bool nn;      // nearest neighbour too (instantiated for jerk && packed only)
+    bool nn;      // nearest neighbour too (instantiated for the jerk forms only)
 };
 
 // Planner for one i-per-thread count I: choose wj and tj and cut the pair list.  Runs on the host

@@ -48,10 +48,10 @@ def gpu_force(ctx, m, x, v, eps, i_index=None, flags=FULL, xi=None, vi=None, n_i
 
 
 # ----------------------------------------------------------------------------- config 1
-@pytest.mark.parametrize("variant", [0x00, 0x01, 0x10, 0x11, 0x20, 0x21, 0x40, 0x41])
+@pytest.mark.parametrize("variant", [0x00, 0x10, 0x20, 0x40, 0x100])
 def test_c1_full_parity_all_kernel_forms(gpu, c_oracle, variant):
-    """BASELINE config 1: N=1024, seed 1, eps=1/256, all i active; every inner-loop form
-    (packed f32x2 / scalar) and every i-per-thread count the library can launch."""
+    """BASELINE config 1: N=1024, seed 1, eps=1/256, all i active; every i-per-thread count the
+    library can launch, and the two-launch form of small blocks."""
     m, x, v = inputs.config_inputs("C1")
     ref = c_oracle.force(m, x, v, EPS)
     with Ctx(1024) as ctx:
@@ -59,8 +59,8 @@ def test_c1_full_parity_all_kernel_forms(gpu, c_oracle, variant):
         got = gpu_force(ctx, m, x, v, EPS)
         shape = nb.nbk_last_launch(ctx)
     assert shape["launches"] >= 1 and shape["grid"] >= 1
-    if variant >> 4:
-        assert shape["i_per_thread"] == variant >> 4
+    if (variant >> 4) & 15:
+        assert shape["i_per_thread"] == (variant >> 4) & 15
     assert_parity(got, ref, what=f"C1 variant {variant:#x}")
 
 
@@ -125,7 +125,7 @@ def test_seeded_random_sizes_flags_and_kernel_forms(gpu, c_oracle):
         jerk = bool(rng.integers(0, 2))
         nn = jerk and rng.integers(0, 4) == 0
         flags = (nb.NBK_JERK if jerk else 0) | nb.NBK_POT | (nb.NBK_NN if nn else 0) | (nb.NBK_EPS0 if eps == 0.0 else 0)
-        variant = int(rng.choice([0x00, 0x10, 0x20, 0x40, 0x100, 0x00 if nn else 0x01]))
+        variant = int(rng.choice([0x00, 0x10, 0x20, 0x40, 0x100, 0x110]))
         m, x, v = inputs.plummer_f32(n, int(rng.integers(1, 1000)))
         idx = np.sort(rng.choice(n, size=n_i, replace=False)).astype(np.int32)
         xi = vi = None
