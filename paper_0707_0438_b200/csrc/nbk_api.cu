@@ -78,7 +78,7 @@ void free_all(nbk_ctx* c) {
     }
     cudaFree(c->d_batch);
     cudaFree(c->hs.x); cudaFree(c->hs.v); cudaFree(c->hs.a); cudaFree(c->hs.j);
-    cudaFree(c->hs.level); cudaFree(c->hs.act); cudaFree(c->hs.bc_ge); cudaFree(c->d_hdr);
+    cudaFree(c->hs.level); cudaFree(c->hs.act); cudaFree(c->hs.bc_ge); cudaFree(c->hs.flag); cudaFree(c->hs.rows); cudaFree(c->d_hdr);
     if (c->h_hdr) cudaFreeHost(c->h_hdr);
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_stage) cudaFreeHost(c->h_stage);

@@ -67,6 +67,8 @@ struct nbk_ctx {
     bool batch_ready = false;
     nbk::HermiteState hs{};              // device-resident integrator state (allocated on first use)
     long long hs_cap = 0;
+    unsigned hs_seq = 0;                 // steps the stepping kernel has taken in this context (tags of its rows and flags)
+    size_t hs_rows_bytes = 0;
     nbk::DynHeader* d_hdr = nullptr;
     nbk::DynHeader* h_hdr = nullptr;     // pinned
     bool host_has_result = false;   // the last firsthalf wrote h_result itself (no D2H needed)

@@ -261,6 +261,109 @@ __device__ __forceinline__ void nn_scan(const JPred& j, int n_j, int tile, int t
     }
 }
 
+// ------------------------------------------------------- Hermite predictor / corrector, one particle
+// Predictor (reading R8), fp64, rounded once to fp32:
+//   x_p = x + v dt + a dt^2/2 + jerk dt^3/6 ;  v_p = v + a dt + jerk dt^2/2 ;  dt = t - t_j
+// o = x y z m vx vy vz.  One copy for predict_kernel, hd_predict_kernel and hd_steps_kernel, so that an
+// i-particle predicted on its own has the bits of its j entry.
+// CG: load through L2 (ld.global.cg) -- for the persistent stepping kernel, where other CTAs rewrite
+// the state between two reads by this one and a line kept in L1 would be stale.
+template <bool CG, typename T>
+__device__ __forceinline__ T ld_state(const T* p) { return CG ? __ldcg(p) : *p; }
+
+// one component: x_p (o_x) and v_p (o_v) from the raw state of a particle
+__device__ __forceinline__ void predict_component(double x, double v, double ac, double jk, double dt,
+                                                  double dt2, double dt3, float& o_x, float& o_v) {
+    o_x = static_cast<float>(x + v * dt + ac * dt2 + jk * dt3);
+    o_v = static_cast<float>(v + ac * dt + jk * dt2);
+}
+
+template <bool CG = false>
+__device__ __forceinline__ void predict_one(const RawJ& raw, long long j, double t, float (&o)[7]) {
+    const double dt = t - ld_state<CG>(raw.t + j);
+    const double dt2 = dt * dt * 0.5, dt3 = dt * dt * dt * (1.0 / 6.0);
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        predict_component(ld_state<CG>(raw.x + c * raw.cap + j), ld_state<CG>(raw.v + c * raw.cap + j),
+                          ld_state<CG>(raw.a + c * raw.cap + j), ld_state<CG>(raw.k + c * raw.cap + j), dt,
+                          dt2, dt3, o[c], o[4 + c]);
+    o[3] = ld_state<CG>(raw.m + j);
+}
+
+// Corrector of one component (reading R15; fp64).  dt = 2^-k is a power of two, so the divisions by
+// dt^2 and dt^3 are exact multiplications by 2^2k and 2^3k (same bits as the quotient).
+__device__ __forceinline__ void correct_component(double x, double v, double a0, double j0, double a1,
+                                                  double j1, int k, double& x1, double& v1,
+                                                  double& a2e, double& a3) {
+    // exact powers of two, written as bit patterns (k <= kMaxLevel = 48: exponents stay normal)
+    const double dt = __longlong_as_double((1023LL - k) << 52);
+    const double inv_dt2 = __longlong_as_double((1023LL + 2 * k) << 52);
+    const double inv_dt3 = __longlong_as_double((1023LL + 3 * k) << 52);
+    const double xp = x + v * dt + a0 * (dt * dt / 2.0) + j0 * (dt * dt * dt / 6.0);
+    const double vp = v + a0 * dt + j0 * (dt * dt / 2.0);
+    const double da = a0 - a1;
+    const double a2 = (-6.0 * da - dt * (4.0 * j0 + 2.0 * j1)) * inv_dt2;
+    a3 = (12.0 * da + 6.0 * dt * (j0 + j1)) * inv_dt3;
+    const double dt3 = dt * dt * dt, dt4 = dt3 * dt;
+    x1 = xp + a2 * (dt4 / 24.0) + a3 * (dt4 * dt / 120.0);
+    v1 = vp + a2 * (dt3 / 6.0) + a3 * (dt4 / 24.0);
+    a2e = a2 + a3 * dt;
+}
+
+// What a corrected particle writes: the fp64 state and the raw j-state the predictor reads.
+__device__ __forceinline__ void store_corrected(const RawJ& raw, const HermiteState& hs, int i, int c,
+                                                double x1, double v1, double a1, double j1) {
+    const size_t e = 3 * static_cast<size_t>(i) + c;
+    hs.x[e] = x1; hs.v[e] = v1; hs.a[e] = a1; hs.j[e] = j1;
+    raw.x[c * raw.cap + i] = x1;
+    raw.v[c * raw.cap + i] = static_cast<float>(v1);
+    raw.a[c * raw.cap + i] = static_cast<float>(a1);
+    raw.k[c * raw.cap + i] = static_cast<float>(j1);
+}
+
+// Level change of particle i: its level, the level counts and the per-index-block counts (integer
+// atomics: order-independent).
+__device__ __forceinline__ void store_level(const HermiteState& hs, DynHeader* h, int i, int k0, int k) {
+    if (k == k0) return;
+    hs.level[i] = k;
+    atomicAdd(reinterpret_cast<unsigned long long*>(&h->level_count[k0]), ~0ULL);   // -1
+    atomicAdd(reinterpret_cast<unsigned long long*>(&h->level_count[k]), 1ULL);
+    const int b = i >> 8;
+    for (int l = k0 + 1; l <= k; ++l) atomicAdd(&hs.bc_ge[l * hs.nblk + b], 1);
+    for (int l = k + 1; l <= k0; ++l) atomicAdd(&hs.bc_ge[l * hs.nblk + b], -1);
+}
+
+// Corrector, Aarseth step and block rule for one due particle i (reading R15; fp64): a1f, j1f are the
+// new force and jerk (fp32 results of the force path).
+__device__ __forceinline__ void correct_one(const RawJ& raw, const HermiteState& hs, DynHeader* h, int i,
+                                            const float* a1f, const float* j1f, long long T_next,
+                                            double t_next, double eta, int kmin) {
+    const int k0 = hs.level[i];
+    double a1[3], j1[3], a2e[3], a3[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const size_t e = 3 * static_cast<size_t>(i) + c;
+        double x1, v1;
+        a1[c] = a1f[c];
+        j1[c] = j1f[c];
+        correct_component(hs.x[e], hs.v[e], hs.a[e], hs.j[e], a1[c], j1[c], k0, x1, v1, a2e[c], a3[c]);
+        store_corrected(raw, hs, i, c, x1, v1, a1[c], j1[c]);
+    }
+    raw.t[i] = t_next;
+    store_level(hs, h, i, k0, next_level(a1, j1, a2e, a3, eta, k0, kmin, T_next));
+}
+
+// Bookkeeping of one finished block step (one thread).
+__device__ __forceinline__ void step_bookkeeping(DynHeader* h, long long T_next, int n_act) {
+    h->T_now = T_next;
+    h->block_steps += 1;
+    h->particle_steps += n_act;
+    h->interactions += static_cast<long long>(n_act) * h->n;
+    int b = 0;
+    while ((2LL << b) <= n_act && b < 31) ++b;
+    h->hist[b] += 1;
+}
+
 __device__ __forceinline__ float acc_take(u64& a) {
     float lo, hi;
     unpack(a, lo, hi);

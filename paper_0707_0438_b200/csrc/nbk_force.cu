@@ -40,7 +40,7 @@ namespace nbk {
 
 
 // ------------------------------------------------------------------------------ force kernel
-template <int I, bool JERK, bool EPS0, bool NN>
+template <int I, bool JERK, bool EPS0, bool NN, bool DYN>
 __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceArgs a) {
     using S = Shape<JERK>;
     constexpr int NACC = S::nacc;
@@ -59,10 +59,10 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
     float* snn_best = reinterpret_cast<float*>(sacc + NACC * I * T);   // [I][T]
     int* snn_tile = reinterpret_cast<int*>(snn_best + I * T);          // [I][T]
 
-    // Small-block form only (I == 1: block steps, the device-resident integrator): the I = 2 and 4
-    // forms run for milliseconds, are launched without the attribute, and their code is left as it
-    // was (two more instructions ahead of the tile loop cost 1 % at C3 -- code placement).
-    if constexpr (I == 1) {
+    // Block-step forms only (I == 1, and the device-planned DYN forms): the I = 2 and 4 forms of the
+    // host entry points run for milliseconds, are launched without the attribute, and their code is
+    // left as it was (two more instructions ahead of the tile loop cost 1 % at C3 -- code placement).
+    if constexpr (I == 1 || DYN) {
         pdl_trigger();
         pdl_wait();   // before anything the predictor (or the step header) wrote is read
     }
@@ -73,15 +73,13 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
     // the step header (made by hd_begin_kernel with the same function the host planner runs)
     Decomp dplan = a.d;
     bool tail_on = a.tail.enabled != 0;
-    if constexpr (I == 1) {
-        if (a.dyn) {
-            if (a.dyn->done || a.dyn->n_act <= 0) return;
-            dplan = a.dyn->plan;
-            if (static_cast<int>(blockIdx.x) >= dplan.G) return;
-            tail_on = a.dyn->fused != 0;
-        }
+    if constexpr (DYN) {
+        if (a.dyn->done || a.dyn->skip || a.dyn->n_act <= 0 || a.dyn->plan_I != I) return;
+        dplan = a.dyn->plan;
+        if (static_cast<int>(blockIdx.x) >= dplan.G) return;
+        tail_on = a.dyn->fused != 0;
     }
-    const Decomp& d = (I == 1) ? dplan : a.d;
+    const Decomp& d = DYN ? dplan : a.d;
     const int wjn = d.wj;
     const int wj = warp % wjn;           // which slice of each j-tile this warp takes
     const int wi = warp / wjn;           // which 32*I-wide group of the i-tile
@@ -443,7 +441,7 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
     pdl_wait();   // every thread, also those of a launch that returns at once (the successor waits on us)
     Decomp dplan = a.d;
     if (a.dyn) {   // device-resident integrator: same plan as the force kernel made
-        if (a.dyn->done || a.dyn->n_act <= 0 || a.dyn->fused) return;   // fused: already reduced
+        if (a.dyn->done || a.dyn->skip || a.dyn->n_act <= 0 || a.dyn->fused) return;   // fused: already reduced
         dplan = a.dyn->plan;
         ix_log2 = 5;
     }
@@ -559,9 +557,9 @@ __global__ void __launch_bounds__(256) nn_scan_kernel(const NnScanArgs a) {
 
 
 // --------------------------------------------------------------------------------- launchers
-template <int I, bool JERK, bool EPS0, bool NN>
-static cudaError_t prepare_nn() {
-    auto fn = force_kernel<I, JERK, EPS0, NN>;
+template <int I, bool JERK, bool EPS0, bool NN, bool DYN>
+static cudaError_t prepare_one() {
+    auto fn = force_kernel<I, JERK, EPS0, NN, DYN>;
     const size_t smem = smem_bytes_of<I, JERK>();
     cudaError_t err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            static_cast<int>(smem));
@@ -572,12 +570,15 @@ static cudaError_t prepare_nn() {
     return nb >= 1 ? cudaSuccess : cudaErrorLaunchOutOfResources;
 }
 
-// the nearest-neighbour form exists for the acc + jerk + pot kernels only
+// the nearest-neighbour form exists for the acc + jerk + pot kernels only; the device-planned (DYN)
+// form for acc + jerk + pot with I = 1 and I = 4 (the device-resident integrator)
 template <int I, bool JERK, bool EPS0>
 static cudaError_t prepare_of() {
-    cudaError_t err = prepare_nn<I, JERK, EPS0, false>();
+    cudaError_t err = prepare_one<I, JERK, EPS0, false, false>();
     if (err != cudaSuccess) return err;
-    if constexpr (JERK) err = prepare_nn<I, JERK, EPS0, true>();
+    if constexpr (JERK) err = prepare_one<I, JERK, EPS0, true, false>();
+    if (err != cudaSuccess) return err;
+    if constexpr (JERK && (I == 1 || I == 4)) err = prepare_one<I, JERK, EPS0, false, true>();
     return err;
 }
 
@@ -587,16 +588,22 @@ static cudaError_t launch_of(const ForceArgs& a, bool nn, cudaStream_t s) {
     if constexpr (JERK) {
         if (nn) {
             if constexpr (I == 1)
-                return launch_pdl(force_kernel<I, JERK, EPS0, true>, a.d.G, warps_of(I) * 32, smem, s, a);
-            force_kernel<I, JERK, EPS0, true><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
+                return launch_pdl(force_kernel<I, JERK, EPS0, true, false>, a.d.G, warps_of(I) * 32, smem, s, a);
+            force_kernel<I, JERK, EPS0, true, false><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
             return cudaGetLastError();
         }
     }
     if (nn) return cudaErrorInvalidValue;
     if constexpr (I == 1)
-        return launch_pdl(force_kernel<I, JERK, EPS0, false>, a.d.G, warps_of(I) * 32, smem, s, a);
-    force_kernel<I, JERK, EPS0, false><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
+        return launch_pdl(force_kernel<I, JERK, EPS0, false, false>, a.d.G, warps_of(I) * 32, smem, s, a);
+    force_kernel<I, JERK, EPS0, false, false><<<a.d.G, warps_of(I) * 32, smem, s>>>(a);
     return cudaGetLastError();
+}
+
+template <int I, bool EPS0>
+static cudaError_t launch_dyn_of(const ForceArgs& a, cudaStream_t s) {
+    return launch_pdl(force_kernel<I, true, EPS0, false, true>, a.d.G, warps_of(I) * 32,
+                      smem_bytes_of<I, true>(), s, a);
 }
 
 #define NBK_DISPATCH(CALL, ...)                                                         \
@@ -629,6 +636,13 @@ cudaError_t force_prepare(const Variant& v) { NBK_DISPATCH(prepare_of); }
 
 cudaError_t launch_force(const Variant& v, const ForceArgs& a, cudaStream_t s) {
     NBK_DISPATCH(launch_of, a, v.nn, s);
+}
+
+cudaError_t launch_force_dyn(const Variant& v, const ForceArgs& a, cudaStream_t s) {
+    if (!v.jerk || v.nn || !a.dyn) return cudaErrorInvalidValue;
+    if (v.I == 1) return v.eps0 ? launch_dyn_of<1, true>(a, s) : launch_dyn_of<1, false>(a, s);
+    if (v.I == 4) return v.eps0 ? launch_dyn_of<4, true>(a, s) : launch_dyn_of<4, false>(a, s);
+    return cudaErrorInvalidValue;
 }
 
 cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s) {

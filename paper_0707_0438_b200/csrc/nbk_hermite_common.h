@@ -53,10 +53,9 @@ NBK_HD inline int startup_level(double norm_a, double norm_jerk, double eta, int
 // then the block rule: the step may halve as often as needed, may double once and only if dt_A >= 2 dt,
 // 2 dt <= dt_max and the new block time T_new (in ticks of 2^-kTickLog2) is a multiple of 2 dt.
 NBK_HD inline double norm3(const double* a) { return sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]); }
-NBK_HD inline int next_level(const double* a1, const double* j1, const double* a2e, const double* a3,
-                             double eta, int k_old, int kmin, long long T_new) {
+NBK_HD inline int next_level_norms(double na, double nj, double n2, double n3, double eta, int k_old,
+                                   int kmin, long long T_new) {
     const double dtm = ldexp(1.0, -kmin), dt_old = ldexp(1.0, -k_old);
-    const double na = norm3(a1), nj = norm3(j1), n2 = norm3(a2e), n3 = norm3(a3);
     const double num = na * n2 + nj * nj, den = nj * n3 + n2 * n2;
     double want = dtm;
     if (den > 0.0) {
@@ -72,6 +71,10 @@ NBK_HD inline int next_level(const double* a1, const double* j1, const double* a
         k -= 1;
     }
     return k;
+}
+NBK_HD inline int next_level(const double* a1, const double* j1, const double* a2e, const double* a3,
+                             double eta, int k_old, int kmin, long long T_new) {
+    return next_level_norms(norm3(a1), norm3(j1), norm3(a2e), norm3(a3), eta, k_old, kmin, T_new);
 }
 
 }  // namespace nbk

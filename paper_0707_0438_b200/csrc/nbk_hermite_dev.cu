@@ -1,9 +1,12 @@
 // nbk_hermite_dev.cu -- nbk_hermite_evolve_dev: the Hermite block-step loop resident on the device
-// (SURVEY.md 8(f)-1).  Host side only: state upload, CUDA-graph replay of the five launches of a step,
-// termination check; the kernels (hd_*) are in nbk_hermite_kernels.cu.
+// (SURVEY.md 8(f)-1).  Host side only: state upload, CUDA-graph replay of the rounds (persistent stepping
+// kernel + the chain of launches for the large steps), termination check; the kernels are in
+// nbk_hermite_steps.cu and nbk_hermite_kernels.cu.
 #include <chrono>
 #include <climits>
 #include <cmath>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -37,8 +40,9 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
 
     if (c->hs_cap < n) {
         cudaFree(c->hs.x); cudaFree(c->hs.v); cudaFree(c->hs.a); cudaFree(c->hs.j);
-        cudaFree(c->hs.level); cudaFree(c->hs.act); cudaFree(c->hs.bc_ge);
+        cudaFree(c->hs.level); cudaFree(c->hs.act); cudaFree(c->hs.bc_ge); cudaFree(c->hs.flag); cudaFree(c->hs.rows);
         c->hs = HermiteState{};
+        c->hs_rows_bytes = 0;
         c->hs_cap = 0;
         NBK_CUDA(c, cudaMalloc(&c->hs.x, sizeof(double) * 3 * N));
         NBK_CUDA(c, cudaMalloc(&c->hs.v, sizeof(double) * 3 * N));
@@ -47,6 +51,8 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
         NBK_CUDA(c, cudaMalloc(&c->hs.level, sizeof(int) * N));
         NBK_CUDA(c, cudaMalloc(&c->hs.act, sizeof(int32_t) * N));
         NBK_CUDA(c, cudaMalloc(&c->hs.bc_ge, sizeof(int) * (kMaxLevel + 1) * ((N + 255) / 256)));
+        NBK_CUDA(c, cudaMalloc(&c->hs.flag, sizeof(unsigned long long) * kStepsMaxAct));
+        NBK_CUDA(c, cudaMemset(c->hs.flag, 0, sizeof(unsigned long long) * kStepsMaxAct));
         c->hs_cap = n;
     }
     if (!c->d_hdr) NBK_CUDA(c, cudaMalloc(&c->d_hdr, sizeof(DynHeader)));
@@ -95,12 +101,42 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     NBK_CUDA(c, cudaMemcpyAsync(c->hs.j, jk.data(), sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
     NBK_CUDA(c, cudaMemcpyAsync(c->hs.level, lev.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream));
     NBK_CUDA(c, cudaMemcpyAsync(c->hs.bc_ge, bc.data(), sizeof(int) * bc.size(), cudaMemcpyHostToDevice, c->stream));
+
+    // Block steps of up to max_act due particles run inside the persistent stepping kernel
+    // (nbk_hermite_steps.cu); it returns at the first larger step, which the chain of launches
+    // hd_begin -> hd_predict -> force (I = 1 or 4, the device planner's choice) -> reduce -> hd_correct
+    // takes; then the stepping kernel again.  One graph holds kIterPerGraph such rounds; they are enqueued
+    // in batches with no host synchronisation inside a batch, and rounds past t_end return at once.
+    const int G = H.num_sms;
+    int max_act = kStepsMaxAct;
+    if (const char* e = std::getenv("NBK_STEPS_MAX_ACT")) max_act = std::atoi(e);
+    if (max_act > kStepsMaxAct) max_act = kStepsMaxAct;
+    if (max_act > G * (kStepsThreads / 32)) max_act = G * (kStepsThreads / 32);   // one due particle per warp
+    const int chunk = static_cast<int>(round_up_ll((n + G - 1) / G, 4));
+    const int n_lev = static_cast<int>(round_up_ll(n, 16 * kStepsThreads));
+    if (steps_smem_bytes(chunk, n_lev) > 220 * 1024 || n_lev / (16 * kStepsThreads) > kStepsMaxVec) max_act = 0;   // does not fit one SM: chain of launches only
+    if (max_act > 0) {
+        int per_sm = 0;
+        NBK_CUDA(c, steps_prepare(chunk, n_lev, &per_sm));
+        if (per_sm < 1) max_act = 0;
+    }
+    if (max_act > 0) {   // the stepping kernel's rows: its own buffer, zeroed once (tags only grow, hs_seq)
+        const size_t need = static_cast<size_t>(G) * max_act * 8 * sizeof(unsigned long long);
+        if (c->hs_rows_bytes < need) {
+            cudaFree(c->hs.rows);
+            c->hs.rows = nullptr;
+            c->hs_rows_bytes = 0;
+            NBK_CUDA(c, cudaMalloc(&c->hs.rows, need));
+            NBK_CUDA(c, cudaMemsetAsync(c->hs.rows, 0, need, c->stream));
+            c->hs_rows_bytes = need;
+        }
+    }
+    H.steps_max_act = max_act;
+    H.seq = c->hs_seq;
     NBK_CUDA(c, cudaMemcpyAsync(c->d_hdr, &H, sizeof(H), cudaMemcpyHostToDevice, c->stream));
     NBK_CUDA(c, cudaStreamSynchronize(c->stream));   // the host vectors above may go away
 
-    // one block step = predict + select, force (+ reduce), correct + next step's header; enqueued in batches with
-    // no host synchronisation inside a batch; steps past t_end return at once (done flag)
-    Variant vv{1, true, eps2 == 0.f, false};
+    Variant v1{1, true, eps2 == 0.f, false}, v4{4, true, eps2 == 0.f, false};
     const long long n_pad = round_up_ll(n, kTileJMax);
     const size_t ni_max = static_cast<size_t>(c->ni_max);
     ForceArgs f;
@@ -123,49 +159,73 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     r.dyn = c->d_hdr;
     r.sum64 = nullptr;
     r.n_j = static_cast<int>(n);
-    // the four launches of a block step are captured into a CUDA graph and replayed
-    const int kBatch = 256;
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t gexec = nullptr;
-    NBK_CUDA(c, launch_hd_begin(c->d_hdr, c->stream));   // first step; later ones: hd_correct's tail
-    auto enqueue_step = [&]() -> cudaError_t {
+    StepsArgs sa;
+    sa.raw = c->raw;
+    sa.h = c->d_hdr;
+    sa.hs = c->hs;
+    sa.eps2 = eps2;
+    sa.chunk = chunk;
+    sa.n_lev = n_lev;
+    sa.max_act = max_act;
+    sa.max_steps = 1 << 20;
+    auto enqueue_round = [&](bool cooperative) -> cudaError_t {
         cudaError_t e;
+        if (max_act > 0 && (e = launch_hd_steps(sa, eps2 == 0.f, G, cooperative, c->stream)) != cudaSuccess) return e;
+        if ((e = launch_hd_begin(c->d_hdr, c->stream)) != cudaSuccess) return e;
         if ((e = launch_hd_predict(c->raw, c->d_hdr, c->hs, n_pad, pred_arr(c, 0), pred_arr(c, 1),
                                    pred_arr(c, 2), pred_arr(c, 3), pred_arr(c, 4), pred_arr(c, 5),
                                    pred_arr(c, 6), c->stream)) != cudaSuccess) return e;
-        if ((e = launch_force(vv, f, c->stream)) != cudaSuccess) return e;
-        if ((e = launch_reduce_dyn(vv, r, static_cast<int>(n), c->stream)) != cudaSuccess) return e;
+        if ((e = launch_force_dyn(v1, f, c->stream)) != cudaSuccess) return e;   // one of the two returns at once
+        if ((e = launch_force_dyn(v4, f, c->stream)) != cudaSuccess) return e;
+        if ((e = launch_reduce_dyn(v1, r, static_cast<int>(n), c->stream)) != cudaSuccess) return e;
         return launch_hd_correct(c->raw, c->d_hdr, c->hs, f.tail.acc, f.tail.jerk,
                                  static_cast<int>(n), c->stream);
     };
-    // kStepsPerGraph steps per graph: inside a graph consecutive kernels are joined by programmatic
-    // dependent-launch edges (nbk_kernels.cuh), between graph launches the stream serialises fully
-    const int kStepsPerGraph = 8;
-    NBK_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
+    // inside a graph consecutive kernels are joined by programmatic dependent-launch edges
+    // (nbk_kernels.cuh), between graph launches the stream serialises fully
+    const int kIterPerGraph = 8, kGraphsPerBatch = 32;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t gexec = nullptr;
     cudaError_t ce = cudaSuccess;
-    for (int s = 0; s < kStepsPerGraph && ce == cudaSuccess; ++s) ce = enqueue_step();
-    cudaError_t ce2 = cudaStreamEndCapture(c->stream, &graph);
-    if (ce != cudaSuccess || ce2 != cudaSuccess) {
+    for (int attempt = 0; attempt < 2; ++attempt) {   // cooperative launch of the stepping kernel, else plain
+        const bool cooperative = attempt == 0;
+        NBK_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
+        ce = cudaSuccess;
+        for (int s = 0; s < kIterPerGraph && ce == cudaSuccess; ++s) ce = enqueue_round(cooperative);
+        cudaError_t ce2 = cudaStreamEndCapture(c->stream, &graph);
+        if (ce == cudaSuccess) ce = ce2;
+        if (ce == cudaSuccess) ce = cudaGraphInstantiate(&gexec, graph, 0);
+        if (ce == cudaSuccess) break;
         if (graph) cudaGraphDestroy(graph);
-        return cuda_fail(c, ce != cudaSuccess ? ce : ce2);
+        graph = nullptr;
+        gexec = nullptr;
+        (void)cudaGetLastError();
+        if (max_act == 0) break;
     }
-    ce = cudaGraphInstantiate(&gexec, graph, 0);
-    if (ce != cudaSuccess) { cudaGraphDestroy(graph); return cuda_fail(c, ce); }
+    if (ce != cudaSuccess) return cuda_fail(c, ce);
     for (;;) {
-        for (int s = 0; s < kBatch / kStepsPerGraph && ce == cudaSuccess; ++s) ce = cudaGraphLaunch(gexec, c->stream);
+        for (int s = 0; s < kGraphsPerBatch && ce == cudaSuccess; ++s) ce = cudaGraphLaunch(gexec, c->stream);
         if (ce == cudaSuccess)
             ce = cudaMemcpyAsync(c->h_hdr, c->d_hdr, sizeof(DynHeader), cudaMemcpyDeviceToHost, c->stream);
         if (ce == cudaSuccess) ce = cudaStreamSynchronize(c->stream);
-        if (ce != cudaSuccess || c->h_hdr->done) break;
+        if (ce != cudaSuccess || c->h_hdr->done || c->h_hdr->error) break;
     }
+    c->hs_seq = c->h_hdr->seq;   // tags of the stepping kernel's rows and flags never repeat in this context
     cudaGraphExecDestroy(gexec);
     cudaGraphDestroy(graph);
     if (ce != cudaSuccess) return cuda_fail(c, ce);
+    if (c->h_hdr->error) {   // a wait inside the stepping kernel gave up: its tags are not to be trusted again
+        c->hs_seq = c->h_hdr->seq + (1u << 24);
+        return cuda_fail(c, cudaErrorLaunchTimeout);
+    }
     NBK_CUDA(c, cudaMemcpyAsync(x, c->hs.x, sizeof(double) * 3 * N, cudaMemcpyDeviceToHost, c->stream));
     NBK_CUDA(c, cudaMemcpyAsync(v, c->hs.v, sizeof(double) * 3 * N, cudaMemcpyDeviceToHost, c->stream));
     NBK_CUDA(c, cudaStreamSynchronize(c->stream));
     c->pred_valid = false;
     c->in_flight = false;
+#ifdef NBK_STEPS_PROF
+    if (std::getenv("NBK_PROF")) { for (int k = 0; k < 20; ++k) std::fprintf(stderr, "prof[%d]=%lld (%.0f per step)\n", k, c->h_hdr->prof[k], double(c->h_hdr->prof[k]) / double(c->h_hdr->prof[18])); }
+#endif
     if (stats) {
         std::memset(stats, 0, sizeof(*stats));
         stats->block_steps = c->h_hdr->block_steps;

@@ -155,8 +155,15 @@ struct DynHeader {
     long long level_count[kMaxLevel + 1];
     long long hist[32];
     Decomp plan;                        // launch plan of the current step (made once, hd_begin_kernel)
+    int plan_I;                         // i-particles per thread of that plan: which force kernel runs
     int fused;                          // the force kernel's last CTA reduces (small block)
-    unsigned ticket;                    // arrival counter of hd_correct_kernel's blocks
+    int skip;                           // this step is left to hd_steps_kernel: the launched chain returns
+    int steps_max_act;                  // hd_steps_kernel takes steps of up to this many due particles (0: off)
+    int error;                          // a grid barrier of hd_steps_kernel gave up waiting
+    unsigned seq;                       // hd_steps_kernel: steps it has taken so far
+#ifdef NBK_STEPS_PROF
+    long long prof[20];
+#endif
 };
 struct HermiteState {        // fp64 integrator state, [n][3] row-major; level[n]
     double* x;
@@ -168,6 +175,8 @@ struct HermiteState {        // fp64 integrator state, [n][3] row-major; level[n
     int* bc_ge;              // [kMaxLevel + 1][nblk]: particles of index block b (256 indices) with
                              // level >= k; gives each block its offset into act without a scan
     int nblk;
+    unsigned long long* flag;  // [kStepsMaxAct] stepping kernel: (step number << 32 | new level) of each particle of the last step
+    unsigned long long* rows;  // [ctas][max_act][8] stepping kernel: partial rows, (step number << 32 | value bits)
 };
 
 constexpr int kFusedMaxI = 32;  // largest i-block served by the one-launch small-block path
@@ -198,7 +207,7 @@ struct ForceArgs {
     float eps2;
     Decomp d;
     FusedTail tail;
-    const DynHeader* dyn;    // non-null (I = 1 only): n_i and the launch plan come from the device
+    const DynHeader* dyn;    // DYN instantiations: n_i and the launch plan come from the device
 };
 
 struct ReduceArgs {
@@ -231,6 +240,8 @@ size_t force_smem_bytes(const Variant& v);
 // Raises the dynamic shared-memory limit of the instantiation and checks that one CTA fits an SM.
 cudaError_t force_prepare(const Variant& v);
 cudaError_t launch_force(const Variant& v, const ForceArgs& a, cudaStream_t s);
+// DYN instantiation (I = 1 or 4, acc + jerk + pot): the plan and n_i come from a.dyn on the device
+cudaError_t launch_force_dyn(const Variant& v, const ForceArgs& a, cudaStream_t s);
 cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s);
 // Nearest neighbour, second step for the two-kernel path: one warp per i re-scans the winning tile.
 struct NnScanArgs {
@@ -349,6 +360,24 @@ cudaError_t launch_batch(const BatchArgs& a, bool eps0, cudaStream_t s);
 cudaError_t launch_batch_reduce(const BatchArgs& a, cudaStream_t s);
 
 // device-resident integrator kernels (one block step = begin, predict+select, force, reduce, correct)
+// hd_steps_kernel (nbk_hermite_steps.cu): whole block steps of up to max_act due particles inside one
+// persistent kernel, one CTA per SM, grid barriers between the phases of a step.
+constexpr int kStepsThreads = 512;     // 16 warps per CTA
+constexpr int kStepsMaxAct = 1024;     // largest step the stepping kernel can hold (due list in shared memory)
+constexpr int kStepsMaxVec = 16;       // 16-byte loads of level bytes per thread at most: n <= 131072
+struct StepsArgs {
+    RawJ raw;
+    DynHeader* h;
+    HermiteState hs;
+    float eps2;
+    int chunk;             // j-particles per CTA (multiple of 4); G * chunk >= n
+    int n_lev;             // n rounded up to a multiple of 16 * kStepsThreads (level bytes every CTA keeps)
+    int max_act;           // steps with more due particles end the launch (the chain of launches takes them)
+    int max_steps;         // block steps per launch at most
+};
+size_t steps_smem_bytes(int chunk, int n_lev);
+cudaError_t steps_prepare(int chunk, int n_lev, int* ctas_per_sm);
+cudaError_t launch_hd_steps(const StepsArgs& a, bool eps0, int grid, bool cooperative, cudaStream_t st);
 cudaError_t launch_hd_begin(DynHeader* h, cudaStream_t st);
 cudaError_t launch_hd_predict(const RawJ& raw, DynHeader* h, const HermiteState& hs, long long n_pad,
                               float* px, float* py, float* pz, float* pm, float* pvx, float* pvy,

@@ -28,8 +28,7 @@ __global__ void scatter_kernel(const ScatterArgs s, const RawJ raw) {
     }
 }
 
-// Hermite predictor (reading R8), fp64, rounded once to fp32:
-//   x_p = x + v dt + a dt^2/2 + jerk dt^3/6 ;  v_p = v + a dt + jerk dt^2/2 ;  dt = t - t_j
+// Hermite predictor (reading R8): predict_one, nbk_device.cuh
 __global__ void predict_kernel(const RawJ raw, double t, long long n_j, long long n_pad, float* px,
                                float* py, float* pz, float* pm, float* pvx, float* pvy,
                                float* pvz) {
@@ -39,20 +38,7 @@ __global__ void predict_kernel(const RawJ raw, double t, long long n_j, long lon
     if (j >= n_pad) return;
     // padding (n_j <= j < n_pad): massless and far away, so that it is nobody's neighbour
     float o[7] = {1e18f, 1e18f, 1e18f, 0.f, 0.f, 0.f, 0.f};
-    if (j < n_j) {
-        const double dt = t - raw.t[j];
-        const double dt2 = dt * dt * 0.5, dt3 = dt * dt * dt * (1.0 / 6.0);
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const double x = raw.x[c * raw.cap + j];
-            const double v = raw.v[c * raw.cap + j];
-            const double ac = raw.a[c * raw.cap + j];
-            const double jk = raw.k[c * raw.cap + j];
-            o[c] = static_cast<float>(x + v * dt + ac * dt2 + jk * dt3);
-            o[4 + c] = static_cast<float>(v + ac * dt + jk * dt2);
-        }
-        o[3] = raw.m[j];
-    }
+    if (j < n_j) predict_one(raw, j, t, o);
     px[j] = o[0]; py[j] = o[1]; pz[j] = o[2]; pm[j] = o[3];
     pvx[j] = o[4]; pvy[j] = o[5]; pvz[j] = o[6];
 }
