@@ -5,7 +5,6 @@
 #include <chrono>
 #include <climits>
 #include <cmath>
-#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <vector>
@@ -223,9 +222,6 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     NBK_CUDA(c, cudaStreamSynchronize(c->stream));
     c->pred_valid = false;
     c->in_flight = false;
-#ifdef NBK_STEPS_PROF
-    if (std::getenv("NBK_PROF")) { for (int k = 0; k < 20; ++k) std::fprintf(stderr, "prof[%d]=%lld (%.0f per step)\n", k, c->h_hdr->prof[k], double(c->h_hdr->prof[k]) / double(c->h_hdr->prof[18])); }
-#endif
     if (stats) {
         std::memset(stats, 0, sizeof(*stats));
         stats->block_steps = c->h_hdr->block_steps;

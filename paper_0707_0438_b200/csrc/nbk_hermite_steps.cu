@@ -38,11 +38,6 @@ constexpr int kSW = kStepsThreads / 32;   // warps per CTA
 constexpr int kLaneJMax = 4;              // steps of up to this many particles: lanes run over j
 constexpr long long kSpinLimit = 1LL << 26;
 
-#ifdef NBK_STEPS_PROF
-#define PROF(k) do { if (tid == 0) { const long long tn = clock64(); prof[k] += tn - tmark; tmark = tn; } } while (0)
-#else
-#define PROF(k) do { } while (0)
-#endif
 
 // one value of a partial row and the number of the step it belongs to, in one 8-byte word
 __device__ __forceinline__ unsigned long long row_word(float v, unsigned seq) {
@@ -184,10 +179,6 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
     int n_prev = 0;
     long long steps_done = 0, psteps = 0;
     __syncthreads();
-#ifdef NBK_STEPS_PROF
-    long long prof[20] = {0};
-    long long tmark = clock64();
-#endif
 
     for (int step = 0;; ++step) {
         // --------------------------------------------- A: last step's changes, header, due list
@@ -208,7 +199,6 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
             if (i >= j0 && i < j0 + chunk) fetch_raw(raw, L, chunk, i, i - j0);
         }
         __syncthreads();
-        PROF(0);
         if (warp == 0) {   // header: finest occupied level -> next block time -> threshold level -> number due
             const int c0 = S.cnt[lane], c1 = lane + 32 <= kMaxLevel ? S.cnt[lane + 32] : 0;
             const unsigned m0 = __ballot_sync(0xffffffffu, c0 > 0), m1 = __ballot_sync(0xffffffffu, c1 > 0);
@@ -242,7 +232,6 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
         }
         __syncthreads();
         if (S.stop) break;
-        PROF(1);
         const int kstar = S.kstar, n_act = S.n_act;
         const long long T_next = S.T_next;
         const double t_next = S.t_next;
@@ -299,7 +288,6 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
             }
         }
         __syncthreads();
-        PROF(2);
         // ------------------------------------------- B: predict the due particles and the own chunk
         for (int q = tid; q < n_act; q += kStepsThreads) {
             float o[7];
@@ -324,7 +312,6 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
             for (int c = 0; c < 7; ++c) dst[c * kTileJMax] = o[c];
         }
         __syncthreads();
-        PROF(3);
         // ---------------------------------------------------------------------- B: the pair sums
         if (n_act <= kLaneJMax) {
             // a few due particles: every thread takes j-particles of the chunk (one each for chunks of up
@@ -433,7 +420,6 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
                 if (wj > 1) __syncthreads();   // scratch is reused by the next round
             }
         }
-        PROF(4);
         // ------------------------------------------------------ C: reduce + correct, by the owning CTA
         // Due particle q belongs to CTA q mod G.  All its threads fetch the G rows at once (thread =
         // (row, half): one round trip), wait until every word carries this step's number, and add the
@@ -531,11 +517,6 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
             h->interactions += psteps * n;
             if (S.stop == 2) { h->done = 1; h->n_act = 0; }
             if (S.stop == 3) h->error = 1;
-#ifdef NBK_STEPS_PROF
-            for (int k = 0; k < 18; ++k) h->prof[k] += prof[k];
-            h->prof[18] += steps_done;
-            h->prof[19] += 1;
-#endif
         }
         if (tid < 32) h->hist[tid] += S.hist[tid];
     }

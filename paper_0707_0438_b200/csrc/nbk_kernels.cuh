@@ -161,9 +161,6 @@ struct DynHeader {
     int steps_max_act;                  // hd_steps_kernel takes steps of up to this many due particles (0: off)
     int error;                          // a grid barrier of hd_steps_kernel gave up waiting
     unsigned seq;                       // hd_steps_kernel: steps it has taken so far
-#ifdef NBK_STEPS_PROF
-    long long prof[20];
-#endif
 };
 struct HermiteState {        // fp64 integrator state, [n][3] row-major; level[n]
     double* x;
