@@ -657,6 +657,68 @@ def run_sweep(args):
     return 0
 
 
+def run_batch(args):
+    """--batch: batched acceleration + potential calls (the treecode use of PAPER.md L229-L231,
+    Table 7): about one million i-particles per call in groups of ~8, ~64, ~256 and ~1024 particles, each with
+    its own interaction list, all groups in one launch.  Markdown table on stdout: kernel time (the library's CUDA events
+    around batch_kernel), interactions/s in the kernel, and the whole call (packing, descriptors, reduction) with device
+    pointers.  Seeded synthetic groups (clump of i-particles, list of cells around it).  Not the bench line."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --batch needs a CUDA device")
+    from paper_0707_0438_b200 import binding as nb
+    nb.load()
+    eps2 = float(np.float32(1.0 / 256.0) ** 2)
+    shapes = [("~8", (4, 12), (300, 700)), ("~64", (32, 96), (900, 1500)), ("~256", (128, 384), (1800, 2700)),
+              ("~1024", (512, 1536), (3600, 5400))]
+    print("| group size | groups | i-particles | list entries | interactions | launch (i per lane, j-slices) | "
+          "batch_kernel ms | interactions/s (kernel) | whole call ms | interactions/s (call) |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    ctx = nb.nbk_open(0, 64, 64)
+    try:
+        for name, (i_lo, i_hi), (j_lo, j_hi) in shapes:
+            rng = np.random.default_rng(1234)
+            n_groups = int(round(1048576 / (0.5 * (i_lo + i_hi))))
+            ni = rng.integers(i_lo, i_hi + 1, n_groups)
+            nj = rng.integers(j_lo, j_hi + 1, n_groups)
+            io = np.concatenate([[0], np.cumsum(ni)]).astype(np.int64)
+            jo = np.concatenate([[0], np.cumsum(nj)]).astype(np.int64)
+            centre = rng.standard_normal((n_groups, 3)).astype(np.float32)
+            xi = np.repeat(centre, ni, axis=0) + np.float32(0.05) * rng.standard_normal((io[-1], 3)).astype(np.float32)
+            xj = np.repeat(centre, nj, axis=0) + rng.standard_normal((jo[-1], 3)).astype(np.float32)
+            mj = (rng.uniform(0.5, 2.0, jo[-1]) / 1000.0).astype(np.float32)
+            inter = float(np.sum(ni.astype(np.float64) * nj))
+            dxi, dmj, dxj = (torch.from_numpy(t).cuda() for t in (xi, mj, xj))
+            acc = torch.empty((int(io[-1]), 3), dtype=torch.float32, device="cuda")
+            pot = torch.empty(int(io[-1]), dtype=torch.float32, device="cuda")
+            torch.cuda.synchronize()
+
+            def call():
+                nb.nbk_calc_batch_dev(ctx, io, dxi.data_ptr(), jo, dmj.data_ptr(), dxj.data_ptr(), eps2, nb.NBK_POT,
+                                      acc.data_ptr(), pot.data_ptr())
+            for _ in range(2):
+                call()
+            nb.nbk_set_timing(ctx, True)
+            ks = []
+            for _ in range(5):
+                call()
+                ks.append(nb.nbk_get_timing(ctx)["force"])
+            nb.nbk_set_timing(ctx, False)
+            t0 = time.perf_counter()
+            for _ in range(5):
+                call()
+            w = (time.perf_counter() - t0) / 5
+            k = float(np.median(ks))
+            shape = nb.nbk_last_launch(ctx)
+            print(f"| {name} | {n_groups} | {int(io[-1])} | {int(jo[-1])} | {inter:.3e} | {shape['i_per_thread']}, "
+                  f"{shape['j_split_warps']} | {k:.3f} | {inter / (k * 1e-3):.3e} | {w * 1e3:.3f} | {inter / w:.3e} |",
+                  flush=True)
+            del dxi, dmj, dxj, acc, pot
+    finally:
+        nb.nbk_close(ctx)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -676,6 +738,8 @@ def main(argv=None):
                     help="with --shard j: exchange by NCCL all-reduces, or by loads from peer (symmetric) memory")
     ap.add_argument("--hermite", choices=["host", "dev"], default=None,
                     help="integrate config C5 with the host-driven or the device-resident Hermite loop and print wall time")
+    ap.add_argument("--batch", action="store_true",
+                    help="time the batched acceleration + potential calls (groups of ~8 to ~1024 particles) as a markdown table")
     ap.add_argument("--t-end", type=float, default=1.0)
     ap.add_argument("--dt-max", type=float, default=1.0 / 16.0)
     args = ap.parse_args(argv)
@@ -683,6 +747,8 @@ def main(argv=None):
         return run_hermite(args)
     if args.sweep:
         return run_sweep(args)
+    if args.batch:
+        return run_batch(args)
     wl = WORKLOADS[args.workload]
     if args.impl == "reference":
         return run_reference(args, wl)

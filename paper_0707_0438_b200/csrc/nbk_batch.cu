@@ -32,8 +32,8 @@ int batch_impl(nbk_ctx* c, int64_t n_groups, const int64_t* i_offset, const floa
         NBK_CUDA(c, batch_prepare());
         c->batch_ready = true;
     }
-    // launch form from the mean group size: the i-tile is the power of two >= mean n_i in [32, 512];
-    // the 16 warps that do not fit the i-tile split the j-tiles (wj)
+    // launch form from the mean group size: a chunk (what one warp works on) is 64 i-particles (two per
+    // lane), 32, or -- small groups -- 16 or 8 with the lanes splitting each j-tile 2 or 4 ways
     std::vector<int> keep;
     int64_t sum_ni = 0;
     for (int64_t q = 0; q < n_groups; ++q)
@@ -45,9 +45,10 @@ int batch_impl(nbk_ctx* c, int64_t n_groups, const int64_t* i_offset, const floa
     float* d_acc = acc;
     float* d_pot = pot;
     const int ng = static_cast<int>(keep.size());
-    int ti = 32;
-    if (ng > 0) while (ti < 512 && ti < sum_ni / ng) ti *= 2;
-    const int wj = 512 / ti, tj = 128;
+    const long long mean = ng > 0 ? sum_ni / ng : 0;
+    const int ipl = mean >= 96 ? 2 : 1;
+    const int slices = mean >= 24 ? 1 : (mean >= 12 ? 2 : 4);
+    const int ti = 32 * ipl / slices, tj = 128;   // ti: i-particles per chunk
     std::vector<long long> pair_prefix(ng + 1, 0), seg_prefix(ng + 1, 0), joff(ng + 1, 0), src_off(ng + 1, 0);
     std::vector<int> ioff(ng + 1, 0), njt(ng > 0 ? ng : 1, 0);
     for (int q = 0; q < ng; ++q) {
@@ -60,8 +61,9 @@ int batch_impl(nbk_ctx* c, int64_t n_groups, const int64_t* i_offset, const floa
         joff[q + 1] = joff[q] + nt * tj;
     }
     const long long P = pair_prefix[ng], n_seg = seg_prefix[ng], n_padded = joff[ng];
-    const int gmax = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
-    const int G = static_cast<int>(P < gmax ? P : gmax);
+    const long long gmax = 16LL * (c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas);   // workers: all warps of the grid
+    const long long G = P < gmax ? P : gmax;
+    if ((P + G - 1) / (G > 0 ? G : 1) > INT_MAX) return NBK_ERANGE;
     // arena: [x y z m | descriptors | partial | (host entry: xi, mj, xj, acc, pot)]
     size_t off = 0;
     auto take = [&](size_t bytes) { const size_t at = off; off += (bytes + 255) & ~static_cast<size_t>(255); return at; };
@@ -142,7 +144,7 @@ int batch_impl(nbk_ctx* c, int64_t n_groups, const int64_t* i_offset, const floa
         ba.i_end = reinterpret_cast<const int*>(B + o_ie);
         ba.partial = reinterpret_cast<float*>(B + o_part);
         ba.acc = d_acc; ba.pot = d_pot;
-        ba.n_groups = ng; ba.ti = ti; ba.tj = tj; ba.wj = wj;
+        ba.n_groups = ng; ba.ci = ti; ba.ipl = ipl; ba.slices = slices;
         ba.P = P; ba.n_seg = n_seg; ba.G = G; ba.eps2 = eps2;
         {
             TimeScope ts(c, 2);
@@ -152,7 +154,7 @@ int batch_impl(nbk_ctx* c, int64_t n_groups, const int64_t* i_offset, const floa
             TimeScope ts(c, 3);
             NBK_CUDA(c, launch_batch_reduce(ba, c->stream));
         }
-        c->last_launch[0] = G; c->last_launch[1] = 512; c->last_launch[2] = 1; c->last_launch[3] = wj;
+        c->last_launch[0] = (G + 15) / 16; c->last_launch[1] = 512; c->last_launch[2] = ipl; c->last_launch[3] = slices;
         c->last_launch[4] = tj; c->last_launch[5] = c->num_sms;
         c->last_launch[6] = static_cast<long long>(batch_smem_bytes()); c->last_launch[7] = 3;
     }

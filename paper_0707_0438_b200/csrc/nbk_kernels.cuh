@@ -319,25 +319,27 @@ cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n
 
 // ---- batched acc + pot calls: many (i-group, j-list) problems in one launch ----
 struct BatchArgs {
-    const float* x;            // packed j-lists, SoA, each list padded to a multiple of tj (m = 0 far away)
+    const float* x;            // packed j-lists, SoA, each list padded to a multiple of 128 (m = 0 far away)
     const float* y;
     const float* z;
     const float* m;
     const float* xi;           // [n_i_total][3] i-positions, groups back to back (caller's order)
-    const long long* pair_prefix;  // [n_groups + 1] pairs (i-tiles x j-tiles) before group g
-    const long long* seg_prefix;   // [n_groups + 1] i-tiles before group g
+    const long long* pair_prefix;  // [n_groups + 1] pairs (chunks x j-tiles) before group g
+    const long long* seg_prefix;   // [n_groups + 1] chunks before group g
     const long long* j_off;        // [n_groups] start of the group's padded list in x, y, z, m
     const int* i_off;              // [n_groups] start / end of the group's i-particles in xi and the
     const int* i_end;              //            outputs (the caller's offsets)
     const int* njt;                // [n_groups] j-tiles of the group's list
-    float* partial;                // [seg + cta][ti][4]
+    float* partial;                // [chunk + worker][ci][4]
     float* acc;                    // [n_i_total][3]  (reduce)
     float* pot;                    // [n_i_total]     (reduce)
     int n_groups;                  // non-empty groups only
-    int ti, tj, wj;
-    long long P;
-    long long n_seg;
-    int G;
+    int ci;                        // i-particles per chunk = 32 * ipl / slices
+    int ipl;                       // i-particles per lane (1 or 2)
+    int slices;                    // lanes of a warp split this many ways over a tile's j-particles (1, 2, 4)
+    long long P;                   // pairs in all
+    long long n_seg;               // chunks in all
+    long long G;                   // workers (warps) that take a range of the pair list
     float eps2;
 };
 struct BatchPackArgs {
