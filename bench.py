@@ -12,11 +12,16 @@ A "step" is one pass of the whole hot path through t
   a6 reduce kernel  a7 nbk_calc_lasthalf[_dev]
 `value`   : inputs resident in HBM, _dev entry points, each step timed with CUDA events on the
             stream the library launches on; L2 is flushed between steps (outside the events).
-`e2e`     : the same step through the HOST entry points (pageable numpy arrays in, numpy arrays
-            out; the library stages through its pinned buffers), host clock around K steps.
+`e2e`     : the same step through the HOST entry points with inputs and results in PINNED host
+            arrays (the library copies host <-> device directly from / into them), host clock
+            around K steps, copies inside the timed region.
 `roofline`: the i x j force kernel alone (the library's own CUDA events around that launch),
             bound "alu": executed fp32 flops / (SMs x 128 lanes x 2 x max SM clock).
-`cpu_baseline`: oracle/nbody_oracle.c (fp64, OpenMP) on a bounded i-slice of the same workload.
+`cpu_baseline`: oracle/nbody_oracle.c (fp64, OpenMP) on a bounded i-slice of the same workload, on all
+            host cores; `cpu_baseline_1core`: the same with OMP_NUM_THREADS=1 (a child process).
+--extras  : adds `block_sweep` (config C2: i-blocks of 1..16384 at N=16384: kernel, call and launch-floor
+            microseconds) and `hermite` (config C5 on the device-resident loop: wall time, steps, dE/E)
+            to the JSON line.
 
 N > 1 (torchrun): the path does not shard under BASELINE.json's north_star ("Everything runs on
 one GPU, with no sharding or collectives"), so every rank runs an independent replica of the
@@ -37,7 +42,27 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "pairwise interactions/sec (acc+jerk+pot) and % of B200 FP32 peak at N=131072"
+METRIC = "pairwise interactions/sec (acc+jerk+pot) and % of B200 FP32 peak at N=131072"   # BASELINE.json (config C3)
+
+
+def metric_of(wl, n):
+    """BASELINE.json's metric string for its own workload (C3); the same wording with the workload's
+    quantities and N for the others, so that a line never claims a workload it did not run."""
+    _, eps, jerk, _ = wl
+    what = "acc+jerk+pot" if jerk else "acc+pot"
+    if eps == 0.0:
+        what += ", eps=0"
+    return f"pairwise interactions/sec ({what}) and % of B200 FP32 peak at N={n}"
+
+
+def sm_max_mhz_measured(fallback=1965.0):
+    """Max SM clock from the driver-written MEASURED_PEAKS.json (the roofline denominator's clock)."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["sm_max_mhz"]), "MEASURED_PEAKS.json sm_max_mhz"
+    except Exception:
+        return float(fallback), "nvml max SM clock"
+
 UNIT = "interactions/s"
 FLOPS_EXECUTED = {True: 42.0, False: 20.0}   # per interaction, FFMA = 2 (DESIGN.md "Flop conventions")
 FLOPS_PAPER = {True: 60.0, False: 38.0}      # PAPER.md Eq. 3, L178-L180
@@ -153,6 +178,31 @@ def oracle_sample(m, x, v, eps, jerk, target_s=15.0, seed=11):
     return n_i * n / dt, cores, n_i, dt
 
 
+def oracle_sample_1core(workload, target_s=6.0):
+    """The same oracle sample with OMP_NUM_THREADS=1, in a child process (the thread count of an OpenMP
+    runtime is fixed once it has started); None if the child fails."""
+    import subprocess
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        out = subprocess.run([sys.executable, os.path.abspath(__file__), "--oracle-sample", str(target_s),
+                              "--workload", workload], env=env, capture_output=True, text=True, timeout=300)
+        return json.loads(out.stdout.strip().splitlines()[-1])
+    except Exception:
+        return None
+
+
+def run_oracle_sample(args, wl):
+    """--oracle-sample SECONDS: time the oracle on a bounded i-slice of the workload, print one JSON object."""
+    from paper_0707_0438_b200 import inputs
+    cfg, eps, jerk, _ = wl
+    m, x, v = inputs.config_inputs(cfg)
+    ov, cores, ni_s, secs = oracle_sample(m, x, v, eps, jerk, target_s=args.oracle_sample)
+    n = m.shape[0]
+    print(json.dumps({"value": ov, "unit": UNIT, "cores": cores, "kind": "oracle",
+                      "sample": f"{ni_s} of {n} i-particles (seeded choice) x all {n} j, {secs:.1f} s"}), flush=True)
+    return 0
+
+
 def run_reference(args, wl):
     """--impl reference: the oracle as it stands, on the host cores, same metric and config."""
     rank, _, world = dist_env()
@@ -184,7 +234,7 @@ def run_reference(args, wl):
     value = args.steps * n_i * n / dt
     sample = f"{n_i} of {n} i-particles (seeded choice) x all {n} j per step"
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "impl": "reference", "metric": metric_of(wl, n), "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": {"workload": desc, "sample": sample},
@@ -311,31 +361,25 @@ def run_ours(args, wl):
 
     # ---- roofline of the dominant kernel (i x j force tile), rank 0
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    sm_max_mhz = clocks.get("sm_max_mhz") or 1965.0
-    peak_src = "nvml max SM clock"
-    if os.path.exists(peaks_path):
-        try:
-            with open(peaks_path) as f:
-                sm_max_mhz = float(json.load(f)["sm_max_mhz"])
-            peak_src = "MEASURED_PEAKS.json sm_max_mhz"
-        except Exception:
-            pass
+    sm_max_mhz, peak_src = sm_max_mhz_measured(clocks.get("sm_max_mhz") or 1965.0)
     peak_tflops = sm_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12
     force_ms = float(np.mean(kern_ms["force"]))
     kint = n * n / (force_ms * 1e-3)
     achieved = FLOPS_EXECUTED[jerk] * kint / 1e12
     # DRAM bytes of one launch of the kernel from the committed ncu --set full capture (bench.py cannot
     # run under ncu itself); null for workloads that were not captured
-    traffic = None
+    traffic, traffic_src = None, None
     try:
         with open(os.path.join(ROOT, "profiles", "force_kernel_traffic.json")) as f:
-            traffic = json.load(f).get(args.workload)
+            tj = json.load(f)
+        traffic = tj.get(args.workload)
+        if traffic is not None:
+            traffic_src = tj.get("source", "committed ncu --set full capture, not measured in this run")
     except Exception:
         pass
     roofline = {
         "bound": "alu", "kernel": "nbk::force_kernel", "achieved": achieved, "peak": peak_tflops,
-        "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": traffic,
+        "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": traffic, "traffic_source": traffic_src,
         "peak_source": f"{sm_count} SMs x 128 fp32 lanes x 2 x {sm_max_mhz:.0f} MHz ({peak_src}); "
                        "DESIGN.md 'Roofline'",
         "flops_per_interaction": FLOPS_EXECUTED[jerk],
@@ -357,8 +401,13 @@ def run_ours(args, wl):
         cpu_baseline = {"value": ov, "unit": UNIT, "cores": cores, "kind": "oracle",
                         "sample": f"{ni_s} of {n} i-particles (seeded choice) x all {n} j, {secs:.1f} s"}
 
+    cpu_1core = None
+    if not args.skip_cpu_baseline:
+        cpu_1core = oracle_sample_1core(args.workload)
+    extras = extras_objects(args) if args.extras else {}
+
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": metric_of(wl, n), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": desc, "n_i": n, "n_j": n, "l2": f"flushed between steps ({L2_FLUSH_BYTES >> 20} MiB write)",
@@ -370,10 +419,94 @@ def run_ours(args, wl):
         "gpu_launches": int(args.steps * 4),
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
+        "cpu_baseline_1core": cpu_1core,
         "tflops_paper_convention": FLOPS_PAPER[jerk] * value / 1e12,
     }
+    line.update(extras)
     print(json.dumps(line), flush=True)
     return 0
+
+
+def launch_floor_us(nb):
+    """Launch + synchronise floor of this box: one 1-particle predictor launch and a stream sync."""
+    ctx = nb.nbk_open(0, 256, 256)
+    try:
+        nb.nbk_set_j_particles(ctx, None, None, np.ones(1, np.float32), np.zeros((1, 3), np.float32))
+        for q in range(20):
+            nb.nbk_predict(ctx, 1)
+            nb.nbk_sync(ctx)
+        t0 = time.perf_counter()
+        for q in range(500):
+            nb.nbk_predict(ctx, 1)
+            nb.nbk_sync(ctx)
+        return (time.perf_counter() - t0) / 500 * 1e6
+    finally:
+        nb.nbk_close(ctx)
+
+
+def extras_objects(args):
+    """--extras: the block-step sweep of config C2 and the C5 Hermite run, as objects for the JSON line
+    (the numbers of DESIGN.md section 9 from one committed command)."""
+    from paper_0707_0438_b200 import binding as nb
+    from paper_0707_0438_b200 import inputs
+    eps = 1.0 / 256.0
+    eps2 = float(np.float32(eps) ** 2)
+    flags = nb.NBK_JERK | nb.NBK_POT
+    # ---- C2: N = 16384, i-blocks drawn without replacement, prediction to a new time before every call
+    m, x, v = inputs.config_inputs("C2")
+    n = m.shape[0]
+    floor = launch_floor_us(nb)
+    sweep = []
+    ctx = nb.nbk_open(0, n, n)
+    try:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        for n_i in (1, 32, 256, 2048, 16384):
+            idx = inputs.active_block(n, n_i, seed=2)
+            nb.nbk_set_ti(ctx, 0.0)
+            nb.nbk_set_timing(ctx, True)
+            ks = []
+            for _ in range(11):
+                nb.nbk_calc_firsthalf(ctx, n, n_i, idx, None, None, eps2, flags)
+                t = nb.nbk_get_timing(ctx)
+                ks.append(t["force"] + t["reduce"])
+            nb.nbk_set_timing(ctx, False)
+            reps = 100 if n_i <= 2048 else 20
+            for q in range(-5, reps):
+                if q == 0:
+                    t0 = time.perf_counter()
+                nb.nbk_set_ti(ctx, 1e-4 * (q + 6))     # forces a new prediction, as a block step does
+                nb.nbk_calc_firsthalf(ctx, n, n_i, idx, None, None, eps2, flags)
+                nb.nbk_calc_lasthalf(ctx, n_i)
+            w = (time.perf_counter() - t0) / reps
+            k = float(np.median(ks[2:]))
+            sweep.append({"n_i": n_i, "n_j": n, "kernel_us": 1e3 * k, "kernel_interactions_per_s": n * n_i / (k * 1e-3),
+                          "api_us": 1e6 * w, "launch_sync_floor_us": floor})
+    finally:
+        nb.nbk_close(ctx)
+    # ---- C5: N = 65536 to t = 1 on the device-resident loop; energies from the library's own potential
+    cfg = inputs.CONFIGS["C5"]
+    n5 = cfg["N"]
+    m5, x5, v5 = inputs.plummer(n5, cfg["seed"])
+    ctx = nb.nbk_open(0, n5, n5)
+
+    def energy():
+        nb.nbk_set_j_particles_f64(ctx, None, None, m5, x5, v5)
+        nb.nbk_set_ti(ctx, 0.0)
+        nb.nbk_calc_firsthalf(ctx, n5, n5, None, None, None, eps2, nb.NBK_POT)
+        pot = nb.nbk_calc_lasthalf_f64(ctx, n5)[2]
+        return float(0.5 * np.sum(m5 * np.sum(v5 * v5, axis=1)) + 0.5 * np.sum(m5 * pot))
+    try:
+        e0 = energy()
+        st = nb.nbk_hermite_evolve_dev(ctx, m5, x5, v5, eps, 1.0, 0.01, 1.0 / 16.0)
+        e1 = energy()
+    finally:
+        nb.nbk_close(ctx)
+    hermite = {"workload": f"C5: N={n5} Plummer seed {cfg['seed']}, eps=1/256, eta=0.01, dt_max=1/16, to t=1",
+               "loop": "device-resident", "wall_s": st["wall_seconds"], "block_steps": st["block_steps"],
+               "particle_steps": st["particle_steps"], "interactions": st["interactions"],
+               "interactions_per_s": st["interactions"] / st["wall_seconds"],
+               "dE_over_E_gpu_potential": (e0 - e1) / e0}
+    return {"block_sweep": sweep, "hermite": hermite}
 
 
 def run_sharded(args, wl):
@@ -452,11 +585,11 @@ def run_sharded(args, wl):
     if rank != 0:
         return 0
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
-    peak_tflops = sm_count * 128 * 2 * 1.965e9 / 1e12
+    peak_tflops = sm_count * 128 * 2 * sm_max_mhz_measured()[0] * 1e6 / 1e12
     kint = n_i_rank * sf.n_local / (float(np.mean(force_ms)) * 1e-3)
     achieved = FLOPS_EXECUTED[jerk] * kint / 1e12
     line = {
-        "metric": METRIC, "value": units_sum / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": metric_of(wl, n), "value": units_sum / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": desc, "n_i": n, "n_j": n, "parallelism": f"{args.shard}-sharded x{world}",
@@ -521,7 +654,7 @@ def run_sweep(args):
     from paper_0707_0438_b200 import inputs
     nb.load()
     sm = torch.cuda.get_device_properties(0).multi_processor_count
-    peak = sm * 128 * 2 * 1.965e9
+    peak = sm * 128 * 2 * sm_max_mhz_measured()[0] * 1e6
     eps2 = float(np.float32(1.0 / 256.0) ** 2)
 
     def kernel_ms(ctx, n_j, n_i, idx, flags, e2, reps):
@@ -614,20 +747,7 @@ def run_sweep(args):
             nb.nbk_close(ctx)
         gbs = 100.0 * n / (us * 1e-6) / 1e9
         print(f"| {n} | {us:.1f} | {gbs:.0f} | {gbs / hbm_peak:.2f} |", flush=True)
-    # launch + synchronise floor of this box: one 1-particle predictor launch and a stream sync
-    ctx = nb.nbk_open(0, 256, 256)
-    try:
-        nb.nbk_set_j_particles(ctx, None, None, np.ones(1, np.float32), np.zeros((1, 3), np.float32))
-        for q in range(20):
-            nb.nbk_predict(ctx, 1)
-            nb.nbk_sync(ctx)
-        t0 = time.perf_counter()
-        for q in range(500):
-            nb.nbk_predict(ctx, 1)
-            nb.nbk_sync(ctx)
-        floor_us = (time.perf_counter() - t0) / 500 * 1e6
-    finally:
-        nb.nbk_close(ctx)
+    floor_us = launch_floor_us(nb)
     print()
     print(f"Launch + synchronise floor (one 1-thread-block kernel, stream sync, through the binding): {floor_us:.1f} us")
     print()
@@ -654,6 +774,68 @@ def run_sweep(args):
                 print(f"| {n} | {n_i} | {k * 1e3:.1f} | {n * n_i / (k * 1e-3):.3e} | {w * 1e6:.1f} |", flush=True)
         finally:
             nb.nbk_close(ctx)
+    return 0
+
+
+def run_profile_pass(args):
+    """--profile-pass: one call of each launch shape outside the headline kernel, few launches in all, meant to be run
+    under ncu (profiles/): config C2 blocks of 32, 256, 2048 and 16384 i-particles (predict, force, reduce), the predictor
+    at N = 1048576, one batched call (groups of ~256), and config C5 on the device-resident loop for one dt_max."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --profile-pass needs a CUDA device")
+    from paper_0707_0438_b200 import binding as nb
+    from paper_0707_0438_b200 import inputs
+    nb.load()
+    eps = 1.0 / 256.0
+    eps2 = float(np.float32(eps) ** 2)
+    flags = nb.NBK_JERK | nb.NBK_POT
+    m, x, v = inputs.config_inputs("C2")
+    n = m.shape[0]
+    ctx = nb.nbk_open(0, n, n)
+    try:
+        nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+        for rep in range(2):   # second round: warm
+            for n_i in (32, 256, 2048, 16384):
+                nb.nbk_set_ti(ctx, 1e-3 * (rep + 1) + 1e-5 * n_i)
+                nb.nbk_calc_firsthalf(ctx, n, n_i, inputs.active_block(n, n_i, seed=2), None, None, eps2, flags)
+                nb.nbk_calc_lasthalf(ctx, n_i)
+    finally:
+        nb.nbk_close(ctx)
+    n4 = 1 << 20
+    m4, x4, v4 = inputs.plummer_f32(n4, 4)
+    ctx = nb.nbk_open(0, n4, 1024)
+    try:
+        nb.nbk_set_j_particles(ctx, None, None, m4, x4, v4)
+        for rep in range(3):
+            nb.nbk_set_ti(ctx, 1e-3 * (rep + 1))
+            nb.nbk_predict(ctx, n4)
+        nb.nbk_sync(ctx)
+    finally:
+        nb.nbk_close(ctx)
+    rng = np.random.default_rng(1234)
+    ng = 1024
+    ni, nj = rng.integers(128, 385, ng), rng.integers(1800, 2701, ng)
+    io = np.concatenate([[0], np.cumsum(ni)]).astype(np.int64)
+    jo = np.concatenate([[0], np.cumsum(nj)]).astype(np.int64)
+    centre = rng.standard_normal((ng, 3)).astype(np.float32)
+    xi = np.repeat(centre, ni, axis=0) + np.float32(0.05) * rng.standard_normal((io[-1], 3)).astype(np.float32)
+    xj = np.repeat(centre, nj, axis=0) + rng.standard_normal((jo[-1], 3)).astype(np.float32)
+    mj = (rng.uniform(0.5, 2.0, jo[-1]) / 1000.0).astype(np.float32)
+    ctx = nb.nbk_open(0, 64, 64)
+    try:
+        for rep in range(2):
+            nb.nbk_calc_batch(ctx, io, xi, jo, mj, xj, eps2, nb.NBK_POT)
+    finally:
+        nb.nbk_close(ctx)
+    cfg = inputs.CONFIGS["C5"]
+    m5, x5, v5 = inputs.plummer(cfg["N"], cfg["seed"])
+    ctx = nb.nbk_open(0, cfg["N"], cfg["N"])
+    try:
+        st = nb.nbk_hermite_evolve_dev(ctx, m5, x5, v5, eps, args.dt_max, 0.01, args.dt_max)
+    finally:
+        nb.nbk_close(ctx)
+    print(json.dumps({"profile_pass": "ok", "hermite_block_steps": st["block_steps"]}), flush=True)
     return 0
 
 
@@ -738,6 +920,11 @@ def main(argv=None):
                     help="with --shard j: exchange by NCCL all-reduces, or by loads from peer (symmetric) memory")
     ap.add_argument("--hermite", choices=["host", "dev"], default=None,
                     help="integrate config C5 with the host-driven or the device-resident Hermite loop and print wall time")
+    ap.add_argument("--extras", action="store_true",
+                    help="add block_sweep (config C2) and hermite (config C5, device-resident loop) objects to the JSON line")
+    ap.add_argument("--oracle-sample", type=float, default=None, help=argparse.SUPPRESS)
+    ap.add_argument("--profile-pass", action="store_true",
+                    help="one call of each launch shape outside the headline kernel (for ncu)")
     ap.add_argument("--batch", action="store_true",
                     help="time the batched acceleration + potential calls (groups of ~8 to ~1024 particles) as a markdown table")
     ap.add_argument("--t-end", type=float, default=1.0)
@@ -749,7 +936,11 @@ def main(argv=None):
         return run_sweep(args)
     if args.batch:
         return run_batch(args)
+    if args.profile_pass:
+        return run_profile_pass(args)
     wl = WORKLOADS[args.workload]
+    if args.oracle_sample is not None:
+        return run_oracle_sample(args, wl)
     if args.impl == "reference":
         return run_reference(args, wl)
     if args.shard in ("j", "i"):
