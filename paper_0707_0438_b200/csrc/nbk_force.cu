@@ -646,8 +646,13 @@ cudaError_t launch_force_dyn(const Variant& v, const ForceArgs& a, cudaStream_t 
 }
 
 cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s) {
+    // ix i-particles x 256 / ix row lanes per CTA.  Small blocks have many rows per i-particle (every CTA
+    // of the force launch worked on the one i-tile) and few i-particles: fewer i per CTA then gives more
+    // CTAs and more row lanes (n_i = 256 at N = 16384: 8 CTAs x 16 rows per lane -> 128 CTAs x 1 row).
     int ix_log2 = 5;
     while (ix_log2 > 0 && (1 << (ix_log2 - 1)) >= a.d.n_i) --ix_log2;
+    const long long rows_per_i = (static_cast<long long>(a.d.njt) * a.d.G + a.d.P - 1) / a.d.P + 1;   // at most
+    while (ix_log2 > 0 && (a.d.n_i >> ix_log2) < 128 && (256 >> ix_log2) < rows_per_i) --ix_log2;
     const int ix = 1 << ix_log2;
     const unsigned grid = static_cast<unsigned>((a.d.n_i + ix - 1) / ix);
     if (v.jerk && v.nn) return launch_pdl(reduce_kernel<true, true>, grid, 256, 0, s, a, ix_log2);
