@@ -219,12 +219,18 @@ int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, double* x, doub
                        nbk_hermite_stats* stats);
 
 /* The same integration with the whole block-step loop on the device (PAPER.md
- * L346, L368 name it as what fp64 GPUs make possible): after the forces at t = 0, every block step
- * is four stream-ordered launches -- predictor + selection of the particles due, i x j force kernel
- * planned on the device, reduction, fp64 corrector + Aarseth step + block rule whose last block also
- * schedules the next step (next block time from per-level particle counts) -- replayed from a CUDA
- * graph in batches of 256 steps with no host synchronisation in between.  Same scheme, formulas, arguments
- * and argument limits as nbk_hermite_evolve; stats->gpu_call_seconds equals wall_seconds. */
+ * L346, L368 name it as what fp64 GPUs make possible).  After the forces at t = 0, block steps of up to
+ * 1024 due particles run inside one persistent kernel (one CTA per SM, every CTA keeps its share of the
+ * j-particles' state and every particle's step level in shared memory: scheduler, predictor, pair sums,
+ * reduction and fp64 corrector of a step without leaving the kernel); larger steps are five stream-ordered
+ * launches -- step header + launch plan made on the device, predictor + selection of the particles due,
+ * i x j force kernel (1 or 4 i-particles per thread, the device planner's choice), reduction, fp64
+ * corrector + Aarseth step + block rule.  Everything is replayed from a CUDA graph in batches with no
+ * host synchronisation in between.  For n > 131072 (or when the state does not fit shared memory) every
+ * step takes the launches.  Same scheme, formulas, arguments and argument limits as nbk_hermite_evolve;
+ * results are bitwise repeatable; stats->gpu_call_seconds equals wall_seconds.  NBK_ECUDA with
+ * nbk_last_cuda_error() == cudaErrorLaunchTimeout means a wait inside the persistent kernel gave up
+ * (another process holding SMs for seconds): the state is then undefined. */
 int nbk_hermite_evolve_dev(nbk_ctx* ctx, int64_t n, const double* m, double* x, double* v,
                            double eps, double t_end, double eta, double dt_max,
                            nbk_hermite_stats* stats);
@@ -294,7 +300,8 @@ int nbk_get_timing(nbk_ctx* ctx, float ms[4]);
  * per CTA, out[2] i-particles per thread, out[3] warps splitting each j-tile, out[4] j-tile
  * size, out[5] SM count, out[6] dynamic shared memory bytes, out[7] number of kernels launched
  * by the last firsthalf (2: force + reduce; 1: small block, reduced by the force kernel's last
- * CTA; 3: force + reduce + neighbour re-scan). */
+ * CTA; 3: force + reduce + neighbour re-scan).  After nbk_calc_batch: out[0] CTAs of 16 warps, out[2]
+ * i-particles per lane (1, 2), out[3] ways the lanes of a warp split a j-tile (1, 2, 4), out[4] 128. */
 int nbk_last_launch(const nbk_ctx* ctx, int64_t out[8]);
 
 /* Host-only (no GPU needed): the launch plan firsthalf would use for (n_i, n_j) on a device with
