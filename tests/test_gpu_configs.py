@@ -747,3 +747,45 @@ def test_subnormal_softening_is_zero_softening(gpu, c_oracle, n, n_i):
         got = nb.nbk_calc_lasthalf(ctx, n_i)
     assert all(np.isfinite(g).all() for g in got)
     assert_parity(got, ref, what="subnormal eps2")
+
+
+@pytest.mark.parametrize("eps", [EPS, 0.0])
+def test_device_resident_paths_agree(gpu, monkeypatch, eps):
+    """nbk_hermite_evolve_dev by its three routes -- every step through the chain of launches
+    (NBK_STEPS_MAX_ACT=0: what runs for n > 131072), steps of <= 4 particles in the persistent stepping
+    kernel (lanes over j), steps of <= 1024 (lanes over i too) -- against the host driver: same scheme,
+    so the same step counts to a few per cent, nearby end states, the same energy; each route bitwise
+    repeatable.  eps = 0 takes the guarded pair loops (hd_steps_kernel<true>, EPS0 force kernels)."""
+    from oracle import nbody_oracle
+    m, x, v = inputs.plummer(1500, seed=23)
+    e0 = nbody_oracle.energy(m, x, v, eps)
+    with Ctx(1500) as ctx:
+        hx, hv = x.copy(), v.copy()
+        sh = nb.nbk_hermite_evolve(ctx, m, hx, hv, eps, 0.125)
+        for max_act in ("0", "4", "1024"):
+            monkeypatch.setenv("NBK_STEPS_MAX_ACT", max_act)
+            runs = []
+            for _ in range(2):
+                gx, gv = x.copy(), v.copy()
+                st = nb.nbk_hermite_evolve_dev(ctx, m, gx, gv, eps, 0.125)
+                runs.append((gx, gv, st))
+            assert np.array_equal(runs[0][0], runs[1][0]) and np.array_equal(runs[0][1], runs[1][1]), max_act
+            gx, gv, st = runs[0]
+            assert st["t_reached"] == 0.125
+            assert sum(st["ni_histogram"]) == st["block_steps"]
+            assert abs(st["particle_steps"] - sh["particle_steps"]) <= 0.03 * sh["particle_steps"], max_act
+            assert abs((nbody_oracle.energy(m, gx, gv, eps) - e0) / e0) < 1e-6, max_act
+            assert np.median(np.linalg.norm(gx - hx, axis=1)) < 1e-4, max_act
+
+
+def test_batched_calls_small_groups_split_lanes(gpu, c_oracle):
+    """Batched calls with the lanes of a warp split 2 and 4 ways over each j-tile (mean group size
+    12-23 and below 12): every group against the oracle, bitwise repeatable."""
+    for ni_range, slices in (((6, 30), 2), ((2, 12), 4)):
+        io, jo, xi, mj, xj = _batch_problem(31 + slices, 500, ni_range, (40, 900))
+        racc, rpot = _batch_oracle(c_oracle, io, jo, xi, mj, xj, EPS)
+        with Ctx(64) as ctx:
+            outs = [nb.nbk_calc_batch(ctx, io, xi, jo, mj, xj, np.float32(EPS) ** 2, nb.NBK_POT) for _ in range(2)]
+            assert nb.nbk_last_launch(ctx)["j_split_warps"] == slices
+        assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+        assert_parity((outs[0][0], None, outs[0][1]), (racc, None, rpot), jerk=False, what=f"batch slices={slices}")
