@@ -654,7 +654,7 @@ cudaError_t launch_reduce(const Variant& v, const ReduceArgs& a, cudaStream_t s)
     const long long rows_per_i = (static_cast<long long>(a.d.njt) * a.d.G + a.d.P - 1) / a.d.P + 1;   // at most
     while (ix_log2 > 0 && (a.d.n_i >> ix_log2) < 128 && (256 >> ix_log2) < rows_per_i) --ix_log2;
     // large blocks have two or three rows per i-particle: one thread per i-particle, no row lanes
-    if (rows_per_i <= 4 && a.d.ti % 256 == 0 && a.d.n_i >= 256 * 128) ix_log2 = 8;
+    if (rows_per_i <= 4 && a.d.ti % 256 == 0 && a.d.n_i >= 256 * 32) ix_log2 = 8;
     const int ix = 1 << ix_log2;
     const unsigned grid = static_cast<unsigned>((a.d.n_i + ix - 1) / ix);
     if (v.jerk && v.nn) return launch_pdl(reduce_kernel<true, true>, grid, 256, 0, s, a, ix_log2);
