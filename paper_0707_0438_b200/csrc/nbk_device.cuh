@@ -325,7 +325,7 @@ __device__ __forceinline__ void store_corrected(const RawJ& raw, const HermiteSt
 // atomics: order-independent).
 __device__ __forceinline__ void store_level(const HermiteState& hs, DynHeader* h, int i, int k0, int k) {
     if (k == k0) return;
-    hs.level[i] = k;
+    hs.level[i] = static_cast<unsigned char>(k + 1);
     atomicAdd(reinterpret_cast<unsigned long long*>(&h->level_count[k0]), ~0ULL);   // -1
     atomicAdd(reinterpret_cast<unsigned long long*>(&h->level_count[k]), 1ULL);
     const int b = i >> 8;
@@ -338,7 +338,7 @@ __device__ __forceinline__ void store_level(const HermiteState& hs, DynHeader* h
 __device__ __forceinline__ void correct_one(const RawJ& raw, const HermiteState& hs, DynHeader* h, int i,
                                             const float* a1f, const float* j1f, long long T_next,
                                             double t_next, double eta, int kmin) {
-    const int k0 = hs.level[i];
+    const int k0 = hs.level[i] - 1;
     double a1[3], j1[3], a2e[3], a3[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {

@@ -443,7 +443,9 @@ __global__ void __launch_bounds__(256) reduce_kernel(const ReduceArgs a, int ix_
     if (a.dyn) {   // device-resident integrator: same plan as the force kernel made
         if (a.dyn->done || a.dyn->skip || a.dyn->n_act <= 0 || a.dyn->fused) return;   // fused: already reduced
         dplan = a.dyn->plan;
-        ix_log2 = 5;
+        // large steps have two or three rows per i-particle: one thread per particle (as launch_reduce chooses)
+        const long long rows_per_i = (static_cast<long long>(dplan.njt) * dplan.G + dplan.P - 1) / dplan.P + 1;
+        ix_log2 = (rows_per_i <= 4 && dplan.ti % 256 == 0) ? 8 : 5;
     }
     const Decomp& d = dplan;
     const int ix = 1 << ix_log2, ry = 256 >> ix_log2;

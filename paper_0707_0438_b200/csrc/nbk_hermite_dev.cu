@@ -47,7 +47,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
         NBK_CUDA(c, cudaMalloc(&c->hs.v, sizeof(double) * 3 * N));
         NBK_CUDA(c, cudaMalloc(&c->hs.a, sizeof(double) * 3 * N));
         NBK_CUDA(c, cudaMalloc(&c->hs.j, sizeof(double) * 3 * N));
-        NBK_CUDA(c, cudaMalloc(&c->hs.level, sizeof(int) * N));
+        NBK_CUDA(c, cudaMalloc(&c->hs.level, (N + 15) / 16 * 16));
         NBK_CUDA(c, cudaMalloc(&c->hs.act, sizeof(int32_t) * N));
         NBK_CUDA(c, cudaMalloc(&c->hs.bc_ge, sizeof(int) * (kMaxLevel + 1) * ((N + 255) / 256)));
         NBK_CUDA(c, cudaMalloc(&c->hs.flag, sizeof(unsigned long long) * kStepsMaxAct));
@@ -60,7 +60,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     // t = 0 through the ordinary entry points: forces on everybody, first steps (reading R15)
     std::vector<float> fa(3 * N), fj(3 * N);
     std::vector<double> a(3 * N), jk(3 * N), tl(N, 0.0);
-    std::vector<int> lev(N);
+    std::vector<unsigned char> lev((N + 15) / 16 * 16, 0);   // k + 1
     if ((rc = nbk_set_j_particles_f64(c, n, nullptr, nullptr, m, x, v, nullptr, nullptr)) != NBK_OK) return rc;
     if ((rc = nbk_set_ti(c, 0.0)) != NBK_OK) return rc;
     if ((rc = nbk_calc_firsthalf(c, n, n, nullptr, nullptr, nullptr, eps2, flags)) != NBK_OK) return rc;
@@ -76,14 +76,14 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
             nj += jk[3 * i + q] * jk[3 * i + q];
         }
         const int k = startup_level(std::sqrt(na), std::sqrt(nj), eta, kmin);
-        lev[i] = k;
+        lev[i] = static_cast<unsigned char>(k + 1);
         H.level_count[k] += 1;
     }
     const int nblk = static_cast<int>((N + 255) / 256);
     c->hs.nblk = nblk;
     std::vector<int> bc(static_cast<size_t>(kMaxLevel + 1) * nblk, 0);
     for (size_t i = 0; i < N; ++i)
-        for (int l = 0; l <= lev[i]; ++l) bc[static_cast<size_t>(l) * nblk + (i >> 8)] += 1;
+        for (int l = 0; l < lev[i]; ++l) bc[static_cast<size_t>(l) * nblk + (i >> 8)] += 1;
     if ((rc = nbk_set_j_particles_f64(c, n, nullptr, tl.data(), m, x, v, a.data(), jk.data())) != NBK_OK) return rc;
     if ((rc = flush_pending(c)) != NBK_OK) return rc;
     H.T_now = 0;
@@ -98,7 +98,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     NBK_CUDA(c, cudaMemcpyAsync(c->hs.v, v, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
     NBK_CUDA(c, cudaMemcpyAsync(c->hs.a, a.data(), sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
     NBK_CUDA(c, cudaMemcpyAsync(c->hs.j, jk.data(), sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
-    NBK_CUDA(c, cudaMemcpyAsync(c->hs.level, lev.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream));
+    NBK_CUDA(c, cudaMemcpyAsync(c->hs.level, lev.data(), lev.size(), cudaMemcpyHostToDevice, c->stream));
     NBK_CUDA(c, cudaMemcpyAsync(c->hs.bc_ge, bc.data(), sizeof(int) * bc.size(), cudaMemcpyHostToDevice, c->stream));
 
     // Block steps of up to max_act due particles run inside the persistent stepping kernel
@@ -174,7 +174,8 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
         if ((e = launch_hd_predict(c->raw, c->d_hdr, c->hs, n_pad, pred_arr(c, 0), pred_arr(c, 1),
                                    pred_arr(c, 2), pred_arr(c, 3), pred_arr(c, 4), pred_arr(c, 5),
                                    pred_arr(c, 6), c->stream)) != cudaSuccess) return e;
-        if ((e = launch_force_dyn(v1, f, c->stream)) != cudaSuccess) return e;   // one of the two returns at once
+        // without the stepping kernel the planner may pick I = 1: both forms are launched, one returns at once
+        if (max_act == 0 && (e = launch_force_dyn(v1, f, c->stream)) != cudaSuccess) return e;
         if ((e = launch_force_dyn(v4, f, c->stream)) != cudaSuccess) return e;
         if ((e = launch_reduce_dyn(v1, r, static_cast<int>(n), c->stream)) != cudaSuccess) return e;
         return launch_hd_correct(c->raw, c->d_hdr, c->hs, f.tail.acc, f.tail.jerk,

@@ -69,8 +69,8 @@ __global__ void hd_begin_kernel(DynHeader* h) {
     if (tid == 0) {
         int bc = -1;
         double best = 0.0;
-        for (int c = 0; c < 2 * kPlanCandidates; ++c) {
-            if (cost[c] < 0) continue;
+        for (int c = h->steps_max_act > 0 ? kPlanCandidates : 0; c < 2 * kPlanCandidates; ++c) {
+            if (cost[c] < 0) continue;   // (with the stepping kernel on, only large steps come here: I = 4)
             const int I = c < kPlanCandidates ? 1 : 4;
             const double w = static_cast<double>(cost[c]) * warps_of(I) / (I == 4 ? 1.0 : 0.86);
             if (bc < 0 || w < best * (1.0 - 1e-9)) { bc = c; best = w; }
@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(256) hd_predict_kernel(const RawJ raw, DynHead
     bool due = false;
     if (j < n_j) {
         predict_one(raw, j, t, o);
-        due = hs.level[j] >= kstar;
+        due = hs.level[j] > kstar;   // level bytes hold k + 1
     }
     const unsigned bal = __ballot_sync(0xffffffffu, due);
     if (lane == 0) wsum[warp] = __popc(bal);
@@ -160,7 +160,7 @@ cudaError_t launch_hd_predict(const RawJ& raw, DynHeader* h, const HermiteState&
 cudaError_t launch_hd_correct(const RawJ& raw, DynHeader* h, const HermiteState& hs, const float* acc,
                               const float* jerk, int n, cudaStream_t st) {
     int grid = (n + 127) / 128;
-    if (grid > 64) grid = 64;   // grid-stride over the due particles; most steps hold a handful
+    if (grid > 592) grid = 592;   // grid-stride over the due particles
     return launch_pdl(hd_correct_kernel, static_cast<unsigned>(grid), 128, 0, st, raw, h, hs, acc, jerk);
 }
 

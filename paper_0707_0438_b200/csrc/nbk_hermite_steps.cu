@@ -171,8 +171,8 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
     // ---- set-up: resident copies of the chunk's raw state, of every particle's level, of the counts
     for (int jl = tid; jl < chunk; jl += kStepsThreads)
         if (j0 + jl < n) fetch_raw(raw, L, chunk, j0 + jl, jl);
-    for (int i = tid; i < a.n_lev; i += kStepsThreads)
-        L.lev[i] = i < n ? static_cast<unsigned char>(hs.level[i] + 1) : static_cast<unsigned char>(0);
+    for (int i = 16 * tid; i < a.n_lev; i += 16 * kStepsThreads)   // level bytes (k + 1; 0 beyond n), 16 per load
+        *reinterpret_cast<uint4*>(L.lev + i) = i < n ? *reinterpret_cast<const uint4*>(hs.level + i) : make_uint4(0u, 0u, 0u, 0u);
     if (tid <= kMaxLevel) S.cnt[tid] = static_cast<int>(h->level_count[tid]);
     if (tid < 32) S.hist[tid] = 0;
     if (tid == 0) S.err = 0;

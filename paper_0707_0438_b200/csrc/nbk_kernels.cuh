@@ -167,7 +167,7 @@ struct HermiteState {        // fp64 integrator state, [n][3] row-major; level[n
     double* v;
     double* a;
     double* j;
-    int* level;
+    unsigned char* level;    // [n rounded up to 16] step level k (dt = 2^-k) of every particle as k + 1, 0 beyond n
     int32_t* act;            // [n] indices of the particles due at T_next, ascending
     int* bc_ge;              // [kMaxLevel + 1][nblk]: particles of index block b (256 indices) with
                              // level >= k; gives each block its offset into act without a scan
