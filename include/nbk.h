@@ -299,7 +299,9 @@ int nbk_get_timing(nbk_ctx* ctx, float ms[4]);
 /* Launch shape of the last firsthalf: out[0] grid (CTAs, one per SM at most), out[1] threads
  * per CTA, out[2] i-particles per thread, out[3] warps splitting each j-tile, out[4] j-tile
  * size, out[5] SM count, out[6] dynamic shared memory bytes, out[7] number of kernels launched
- * by the last firsthalf (2: force + reduce; 1: small block, reduced by the force kernel's last
+ * by the last firsthalf (2: force + reduce; 1: small block -- predicted, summed and reduced by one
+ * launch of 512-thread CTAs, out[3] = 16, out[4] = j-particles per CTA -- or, with external positions or
+ * NBK_NN, reduced by the tiled force kernel's last
  * CTA; 3: force + reduce + neighbour re-scan).  After nbk_calc_batch: out[0] CTAs of 16 warps, out[2]
  * i-particles per lane (1, 2), out[3] ways the lanes of a warp split a j-tile (1, 2, 4), out[4] 128. */
 int nbk_last_launch(const nbk_ctx* ctx, int64_t out[8]);

@@ -163,13 +163,70 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
                   const int32_t* h_inline = nullptr, bool to_host = false,
                   double* sum64 = nullptr) {
     eps2 = flushed_eps2(eps2);
+    float* acc = c->d_result;
+    float* jerk = acc + 3 * n_i;
+    float* pot = acc + 6 * n_i;
+    // A block of <= 32 particles of the j-set: ONE launch that predicts, sums and reduces (nbk_small_kernels.cu)
+    {
+        const int G = c->num_sms < kMaxCtas ? c->num_sms : kMaxCtas;
+        const long long n_pad = round_up(n_j, kTileJMax);
+        const long long chunk = round_up((n_pad + G - 1) / G, 4);
+        bool small = n_i >= 1 && n_i <= kFusedMaxI && n_j >= 1 && !d_xi && !d_vi && !sum64 && c->fused_ok &&
+                     !(flags & NBK_NN) && chunk <= kSmallMaxChunk &&
+                     plan_partial_floats_bound(c->ni_max, c->num_sms) >= static_cast<size_t>(G) * kFusedMaxI * 8;
+        if (small && h_inline)
+            for (long long k = 0; k < n_i; ++k) small = small && h_inline[k] >= 0;
+        if (small) {
+            bool fold = true;
+            for (int k = 0; k < c->pending.n; ++k) fold = fold && c->pending.addr[k] < n_j;
+            if (!fold) {
+                const int rc = flush_pending(c);
+                if (rc != NBK_OK) return rc;
+            }
+            SmallArgs sa;
+            sa.raw = c->raw;
+            sa.t = c->t;
+            sa.n_j = static_cast<int>(n_j);
+            sa.n_pad = static_cast<int>(n_pad);
+            sa.chunk = static_cast<int>(chunk);
+            for (int k = 0; k < 7; ++k) sa.pred[k] = pred_arr(c, k);
+            sa.n_i = static_cast<int>(n_i);
+            sa.inline_index = h_inline ? 1 : 0;
+            std::memset(sa.i_inline, 0, sizeof(sa.i_inline));
+            if (h_inline) std::memcpy(sa.i_inline, h_inline, sizeof(int32_t) * n_i);
+            sa.i_index = d_iidx;
+            sa.eps2 = eps2;
+            sa.partial = c->d_partial;
+            sa.counter = c->d_counter;
+            sa.acc = acc; sa.jerk = jerk; sa.pot = pot;
+            sa.host_out = to_host ? c->h_result_dev : nullptr;
+            sa.upd = c->pending;
+            if (!c->small_ready) {
+                NBK_CUDA(c, small_prepare(kSmallMaxChunk));
+                c->small_ready = true;
+            }
+            c->last_ni = n_i;
+            c->in_flight = true;
+            c->last_nn = false;
+            {
+                TimeScope ts(c, 2);
+                NBK_CUDA(c, launch_small_block(sa, (flags & NBK_JERK) != 0, (flags & NBK_EPS0) != 0 || eps2 == 0.f, G,
+                                               c->stream));
+            }
+            c->pending.n = 0;
+            c->pred_valid = true;
+            c->pred_nj = n_j;
+            c->host_has_result = to_host;
+            c->last_launch[0] = G; c->last_launch[1] = 512; c->last_launch[2] = 1; c->last_launch[3] = 16;
+            c->last_launch[4] = chunk; c->last_launch[5] = c->num_sms;
+            c->last_launch[6] = static_cast<long long>(small_smem_bytes(sa.chunk)); c->last_launch[7] = 1;
+            return NBK_OK;
+        }
+    }
     if (!c->pred_valid || c->pred_nj != n_j) {
         const int rc = do_predict(c, n_j);
         if (rc != NBK_OK) return rc;
     }
-    float* acc = c->d_result;
-    float* jerk = acc + 3 * n_i;
-    float* pot = acc + 6 * n_i;
     c->last_ni = n_i;
     c->in_flight = true;
     c->host_has_result = false;

@@ -65,6 +65,7 @@ struct nbk_ctx {
     unsigned char* d_batch = nullptr;  // batched calls: one growable device arena
     size_t batch_bytes = 0;
     bool batch_ready = false;
+    bool small_ready = false;            // small_block_kernel's shared-memory limit has been raised
     nbk::HermiteState hs{};              // device-resident integrator state (allocated on first use)
     long long hs_cap = 0;
     unsigned hs_seq = 0;                 // steps the stepping kernel has taken in this context (tags of its rows and flags)

@@ -353,6 +353,32 @@ __device__ __forceinline__ void correct_one(const RawJ& raw, const HermiteState&
     store_level(hs, h, i, k0, next_level(a1, j1, a2e, a3, eta, k0, kmin, T_next));
 }
 
+// One ordered pair in scalar fp32 (the formulas of tile_packed with the jerk formed
+// per pair: u = w - 3 (r.w) r / s, jerk += m s^-3/2 u).  nx.. = negated i-state; s7 += acc3, m/sqrt(s), jerk3.
+template <bool JERK, bool EPS0>
+__device__ __forceinline__ void pair_scalar(const float (&jv)[7], const float* ni, bool self, float eps2,
+                                            float (&s7)[7]) {
+    const float dx = jv[0] + ni[0], dy = jv[1] + ni[1], dz = jv[2] + ni[2];
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, eps2)));
+    float rinv = rsq(r2);
+    if (EPS0) rinv = r2 > 0.f ? rinv : 0.f;
+    const float m = self ? 0.f : jv[3];       // L96: the own entry contributes nothing
+    const float rinv2 = rinv * rinv, mrinv = m * rinv, mrinv3 = mrinv * rinv2;
+    s7[0] = fmaf(mrinv3, dx, s7[0]);
+    s7[1] = fmaf(mrinv3, dy, s7[1]);
+    s7[2] = fmaf(mrinv3, dz, s7[2]);
+    s7[3] += mrinv;
+    if (JERK) {
+        const float dvx = jv[4] + ni[3], dvy = jv[5] + ni[4], dvz = jv[6] + ni[5];
+        const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+        const float g3 = -3.f * (rv * rinv2);
+        s7[4] = fmaf(mrinv3, fmaf(g3, dx, dvx), s7[4]);
+        s7[5] = fmaf(mrinv3, fmaf(g3, dy, dvy), s7[5]);
+        s7[6] = fmaf(mrinv3, fmaf(g3, dz, dvz), s7[6]);
+    }
+}
+
+
 // Bookkeeping of one finished block step (one thread).
 __device__ __forceinline__ void step_bookkeeping(DynHeader* h, long long T_next, int n_act) {
     h->T_now = T_next;

@@ -317,6 +317,32 @@ cudaError_t launch_predict(const RawJ& raw, double t, long long n_j, long long n
                            float* py, float* pz, float* pm, float* pvx, float* pvy, float* pvz,
                            const InlineJ* upd, cudaStream_t st);
 
+// ---- a block step of <= kFusedMaxI i-particles in one launch (nbk_small_kernels.cu): predictor for the
+// CTA's own j-particles and for the i-particles, pair sums, reduction by the last CTA.
+constexpr int kSmallMaxChunk = 2048;   // j-particles per CTA at most (shared memory): n_j <= SMs x 2048
+struct SmallArgs {
+    RawJ raw;
+    double t;                 // prediction time
+    int n_j, n_pad;           // j-particles, and the padded count the predicted arrays are filled to
+    int chunk;                // j-particles per CTA, multiple of 4; grid x chunk >= n_pad
+    float* pred[7];           // predicted arrays x y z m vx vy vz (also written: other calls read them)
+    int n_i;
+    int inline_index;         // 1: i-indices are i_inline[], else i_index (nullptr: identity)
+    int32_t i_inline[kFusedMaxI];
+    const int32_t* i_index;
+    float eps2;
+    float* partial;           // [cta][kFusedMaxI][8]
+    unsigned* counter;        // zero between launches (the last CTA resets it)
+    float* acc;               // results [n_i][3], [n_i][3], [n_i]
+    float* jerk;
+    float* pot;
+    float* host_out;          // mapped pinned copy acc|jerk|pot (7 n_i floats) or nullptr
+    InlineJ upd;              // a pending set_j of a few particles (upd.n may be 0), all addresses < n_j
+};
+size_t small_smem_bytes(int chunk);
+cudaError_t small_prepare(int chunk_max);
+cudaError_t launch_small_block(const SmallArgs& a, bool jerk, bool eps0, int grid, cudaStream_t s);
+
 // ---- batched acc + pot calls: many (i-group, j-list) problems in one launch ----
 struct BatchArgs {
     const float* x;            // packed j-lists, SoA, each list padded to a multiple of 128 (m = 0 far away)
