@@ -127,10 +127,11 @@ __device__ __forceinline__ void issue_tile(const JPred& j, int jt, int tj, float
 // The i-state is held negated (r = x_j + (-x_i) is one add).  sl[q] is the position of the
 // i-particle's own j entry inside this tile (anything outside [0, tj) if it is elsewhere);
 // MASK instantiations zero the mass of that entry.
+// POT = false leaves the potential sum out (acc[q][3] stays 0).
 // NN instantiations also keep, per i, the smallest s seen in this tile ("a
 // comparison is added with each force calculation to maintain the particle with the minimum
 // distance"); which j it was is found afterwards by re-scanning the one winning tile (nn_scan).
-template <int I, bool JERK, bool EPS0, bool MASK, bool NN>
+template <int I, bool JERK, bool EPS0, bool MASK, bool NN, bool POT = true>
 __device__ __forceinline__ void tile_packed(const float* __restrict__ sx, int jbeg, int jend,
                                             const float (&ni)[I][6], const int (&sl)[I],
                                             u64 (&acc)[I][Shape<JERK>::nacc], float eps2,
@@ -190,7 +191,7 @@ __device__ __forceinline__ void tile_packed(const float* __restrict__ sx, int jb
                     rinv2 = mul2(rinv, rinv);
                 }
                 const u64 mrinv = mul2(mj, rinv);
-                acc[q][3] = add2(acc[q][3], mrinv);
+                if (POT) acc[q][3] = add2(acc[q][3], mrinv);   // (the integrator's kernels do not need the potential)
                 const u64 mrinv3 = mul2(mrinv, rinv2);
                 acc[q][0] = fma2(mrinv3, dx, acc[q][0]);
                 acc[q][1] = fma2(mrinv3, dy, acc[q][1]);

@@ -184,9 +184,9 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
         // fold below tests once per group of NBK_FOLD tiles; only then the group is redone with
         // the guarded loop.  Common case: no per-pair compare-and-select at all.
         if (__any_sync(0xffffffffu, mine)) {
-            tile_packed<I, JERK, EPS0, true, NN>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2, tmin);
+            tile_packed<I, JERK, EPS0, true, NN, !DYN>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2, tmin);
         } else {
-            tile_packed<I, JERK, false, false, NN>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2, tmin);
+            tile_packed<I, JERK, false, false, NN, !DYN>(sx, jbeg, jbeg + jlen, ni, sl, acc, a.eps2, tmin);
         }
 
         if (NN) {
@@ -215,7 +215,7 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
 #pragma unroll
                 for (int q = 0; q < I; ++q) {
                     float lo, hi;
-                    unpack(acc[q][3], lo, hi);
+                    unpack(acc[q][DYN ? 0 : 3], lo, hi);   // DYN forms keep no potential sum: inf x 0 in acc x
                     bad |= !(fabsf(lo + hi) < __int_as_float(0x7f800000));
                 }
                 if (__any_sync(0xffffffffu, bad)) {   // a coincident pair: redo the group, guarded
@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(warps_of(I) * 32, 1) force_kernel(const ForceA
                         int hl[I];   // the guarded loop with the own-entry mask serves every tile
 #pragma unroll
                         for (int q = 0; q < I; ++q) hl[q] = self[q] - held_jt[h] * d.tj;
-                        tile_packed<I, JERK, true, true, NN>(hx, jbeg, jbeg + jlen, ni, hl, acc, a.eps2, tmin);
+                        tile_packed<I, JERK, true, true, NN, !DYN>(hx, jbeg, jbeg + jlen, ni, hl, acc, a.eps2, tmin);
                         if (NN) {   // the same minima as the first pass found
 #pragma unroll
                             for (int q = 0; q < I; ++q) tmin[q] = __int_as_float(0x7f800000);
