@@ -65,9 +65,7 @@ struct StepsSmem {
     int cnt[kMaxLevel + 1];            // particles per level
     long long hist[32];                // CTA 0: steps by log2(size), written back at the end
     int wsum[kSW];
-    long long T_next;
-    double t_next;
-    int kstar, n_act, stop, err;
+    int err;
 };
 
 // shared memory: tiles | raw chunk (x, t fp64; v, a, k, m fp32) | level bytes | StepsSmem
@@ -153,7 +151,7 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
     if (tid <= kMaxLevel) S.cnt[tid] = static_cast<int>(h->level_count[tid]);
     if (tid < 32) S.hist[tid] = 0;
     if (tid == 0) S.err = 0;
-    int n_prev = 0;
+    int n_prev = 0, stop = 0;
     long long steps_done = 0, psteps = 0;
     __syncthreads();
 
@@ -176,12 +174,15 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
             if (i >= j0 && i < j0 + chunk) fetch_raw(raw, L, chunk, i, i - j0);
         }
         __syncthreads();
-        if (warp == 0) {   // header: finest occupied level -> next block time -> threshold level -> number due
+        // header, by every warp for itself (no broadcast, no barrier): finest occupied level -> next block
+        // time -> threshold level -> number due
+        int kstar, n_act = 0;
+        long long T_next = 0;
+        {
             const int c0 = S.cnt[lane], c1 = lane + 32 <= kMaxLevel ? S.cnt[lane + 32] : 0;
             const unsigned m0 = __ballot_sync(0xffffffffu, c0 > 0), m1 = __ballot_sync(0xffffffffu, c1 > 0);
             const int kf = m1 ? 63 - __clz(m1) : (m0 ? 31 - __clz(m0) : -1);
-            int stop = 0, kstar = kf, n_act = 0;
-            long long T_next = 0;
+            kstar = kf;
             if (kf >= 0) {
                 const int sh = kTickLog2 - kf;
                 T_next = ((T_now >> sh) + 1) << sh;
@@ -199,19 +200,9 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
                 for (int o = 16; o > 0; o >>= 1) n_act += __shfl_xor_sync(0xffffffffu, n_act, o);
                 if (n_act > a.max_act || step >= a.max_steps) stop = 1;
             }
-            if (lane == 0) {
-                S.T_next = T_next;
-                S.t_next = ldexp(static_cast<double>(T_next), -kTickLog2);
-                S.kstar = kstar;
-                S.n_act = n_act;
-                S.stop = stop;
-            }
         }
-        __syncthreads();
-        if (S.stop) break;
-        const int kstar = S.kstar, n_act = S.n_act;
-        const long long T_next = S.T_next;
-        const double t_next = S.t_next;
+        if (stop) break;
+        const double t_next = static_cast<double>(T_next) * 0x1p-52;   // = ldexp(T_next, -kTickLog2), exact scaling
         const unsigned seq = seq0 + static_cast<unsigned>(step) + 1u;   // this step's number (never 0)
         {   // due = level >= kstar.  Level bytes hold level + 1 (0: no particle), all below 128, so
             // (byte + 0x80 - (kstar + 1)) has its top bit set exactly for the due ones.  A warp scans a
@@ -368,8 +359,8 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
                         const float* sx = L.tiles + b * 7 * kTileJMax;
                         int sl[1] = {self - j0 - (b << 8)};
                         const bool own = static_cast<unsigned>(sl[0]) < static_cast<unsigned>(kTileJMax);
-                        if (__any_sync(0xffffffffu, own)) tile_packed<1, true, EPS0, true, false>(sx, lo, hi, ni, sl, acc, a.eps2, tmin);
-                        else tile_packed<1, true, EPS0, false, false>(sx, lo, hi, ni, sl, acc, a.eps2, tmin);
+                        if (__any_sync(0xffffffffu, own)) tile_packed<1, true, EPS0, true, false, false>(sx, lo, hi, ni, sl, acc, a.eps2, tmin);
+                        else tile_packed<1, true, EPS0, false, false, false>(sx, lo, hi, ni, sl, acc, a.eps2, tmin);
 #pragma unroll
                         for (int v = 0; v < 10; ++v) d[v] += static_cast<double>(acc_take(acc[0][v]));
                     }
@@ -455,17 +446,23 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
                     store_corrected(raw, hs, my_i, c, x1, v1, a1, j1);
                     __threadfence();   // each component lane's own stores, before lane 0 sets the flag
                 }
-                // squared norms over the three component lanes, (c0 + c1) + c2 in lane 0
-                double sq[4] = {a1 * a1, j1 * j1, a2e * a2e, a3 * a3};
+                // squared norms over the three component lanes, (c0 + c1) + c2, in every lane; lane e < 4 takes
+                // the root of norm e (|a1|, |j1|, |a2'|, |a3|): four square roots side by side
+                const double sq[4] = {a1 * a1, j1 * j1, a2e * a2e, a3 * a3};
+                double mine = 0.0;
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const double s1 = __shfl_down_sync(0xffffffffu, sq[e], 1), s2 = __shfl_down_sync(0xffffffffu, sq[e], 2);
-                    sq[e] = (sq[e] + s1) + s2;
+                    const double tot = (__shfl_sync(0xffffffffu, sq[e], 0) + __shfl_sync(0xffffffffu, sq[e], 1)) +
+                                       __shfl_sync(0xffffffffu, sq[e], 2);
+                    mine = lane == e ? tot : mine;
                 }
+                mine = sqrt(mine);
+                const double na = __shfl_sync(0xffffffffu, mine, 0), nj = __shfl_sync(0xffffffffu, mine, 1);
+                const double n2 = __shfl_sync(0xffffffffu, mine, 2), n3 = __shfl_sync(0xffffffffu, mine, 3);
                 __syncwarp();   // the component lanes' stores before lane 0's flag
                 if (lane == 0) {
                     raw.t[my_i] = t_next;
-                    const int kn = next_level_norms(sqrt(sq[0]), sqrt(sq[1]), sqrt(sq[2]), sqrt(sq[3]), eta, k0, kmin, T_next);
+                    const int kn = next_level_norms(na, nj, n2, n3, eta, k0, kmin, T_next);
                     store_level(hs, h, my_i, k0, kn);
                     __threadfence();   // state, level tables, then the flag: step number and new level
                     const unsigned long long f = (static_cast<unsigned long long>(seq) << 32) |
@@ -492,8 +489,8 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
             h->block_steps += steps_done;
             h->particle_steps += psteps;
             h->interactions += psteps * n;
-            if (S.stop == 2) { h->done = 1; h->n_act = 0; }
-            if (S.stop == 3) h->error = 1;
+            if (stop == 2) { h->done = 1; h->n_act = 0; }
+            if (stop == 3) h->error = 1;
         }
         if (tid < 32) h->hist[tid] += S.hist[tid];
     }
