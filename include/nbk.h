@@ -230,7 +230,9 @@ int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, double* x, doub
  * step takes the launches.  Same scheme, formulas, arguments and argument limits as nbk_hermite_evolve;
  * results are bitwise repeatable; stats->gpu_call_seconds equals wall_seconds.  NBK_ECUDA with
  * nbk_last_cuda_error() == cudaErrorLaunchTimeout means a wait inside the persistent kernel gave up
- * (another process holding SMs for seconds): the state is then undefined. */
+ * (another process holding SMs for seconds): the state is then undefined.  Test knob: the environment
+ * variable NBK_STEPS_MAX_ACT (0..1024, read at each call) caps the step size the persistent kernel takes;
+ * 0 sends every step through the launches. */
 int nbk_hermite_evolve_dev(nbk_ctx* ctx, int64_t n, const double* m, double* x, double* v,
                            double eps, double t_end, double eta, double dt_max,
                            nbk_hermite_stats* stats);
