@@ -329,8 +329,14 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
             // nit i-tiles of 32 due particles (lane = particle); wj warps split the chunk for one i-tile,
             // kSW / wj i-tiles run side by side, in rounds
             const int nit = (n_act + 31) >> 5;
-            int wj = kSW;
-            while (wj > 1 && kSW / wj < nit) wj >>= 1;
+            // wj warps per i-tile, kSW / wj i-tiles per round: the split with the least (rounds x (chunk / wj + a
+            // round's fixed part, about a tenth of a chunk)); e.g. 24 tiles: 3 rounds of half chunks, not 2 of whole
+            int wj = kSW, best = 1 << 30;
+            for (int w = kSW; w >= 1; w >>= 1) {
+                const int rounds = (nit * w + kSW - 1) / kSW;
+                const int cost = rounds * (160 / w + 16);
+                if (cost < best) { best = cost; wj = w; }
+            }
             const int ng = kSW / wj;
             const int ws = warp % wj, wg = warp / wj;
             const int g4 = chunk >> 2;                        // groups of 4 j-particles in the chunk
@@ -442,10 +448,7 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
                 const double j1 = static_cast<float>(__shfl_sync(0xffffffffu, sv, 4 + c));
                 double x1, v1, a2e, a3;
                 correct_component(x, v, a0, jk0, a1, j1, k0, x1, v1, a2e, a3);
-                if (lane < 3) {
-                    store_corrected(raw, hs, my_i, c, x1, v1, a1, j1);
-                    __threadfence();   // each component lane's own stores, before lane 0 sets the flag
-                }
+                if (lane < 3) store_corrected(raw, hs, my_i, c, x1, v1, a1, j1);
                 // squared norms over the three component lanes, (c0 + c1) + c2, in every lane; lane e < 4 takes
                 // the root of norm e (|a1|, |j1|, |a2'|, |a3|): four square roots side by side
                 const double sq[4] = {a1 * a1, j1 * j1, a2e * a2e, a3 * a3};
@@ -459,7 +462,7 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
                 mine = sqrt(mine);
                 const double na = __shfl_sync(0xffffffffu, mine, 0), nj = __shfl_sync(0xffffffffu, mine, 1);
                 const double n2 = __shfl_sync(0xffffffffu, mine, 2), n3 = __shfl_sync(0xffffffffu, mine, 3);
-                __syncwarp();   // the component lanes' stores before lane 0's flag
+                __syncwarp();   // the component lanes' stores happen before lane 0's fence (cumulative) and flag
                 if (lane == 0) {
                     raw.t[my_i] = t_next;
                     const int kn = next_level_norms(na, nj, n2, n3, eta, k0, kmin, T_next);
