@@ -15,14 +15,13 @@
 //      j-state never goes to global memory), due particles from global raw state (every CTA predicts
 //      them itself: same formula, same bits as their j entries); then the pair sums over the resident
 //      chunk -- lanes over j for steps of a few particles, lanes over i (tile_packed) otherwise -- fp32
-//      inside a warp's share, fp64 above; one partial row per (CTA, due particle).  The warp that will
-//      correct particle q fetches its fp64 state meanwhile.
+//      inside a warp's share, fp64 above; one partial row per (CTA, due particle).
 //      Every value of a row travels in one 8-byte word together with the step number, so a row is
 //      complete as soon as its words carry the current number: no fence, no counter, no barrier.
-//   C  due particle q belongs to one warp of CTA (q mod G): it reads the G rows until they are all of
-//      this step, adds them in CTA order (fp64, fixed tree), rounds once to fp32 and runs the fp64
-//      corrector (one lane per component), the Aarseth step and the block rule; then sets the
-//      particle's flag.
+//   C  due particle q belongs to CTA (q mod G): all its threads fetch the G rows at once and spin until
+//      they are all of this step; the rows are added in CTA order (fp64, lane tree then warps in order),
+//      rounded once to fp32, and warp 0 runs the fp64 corrector (one lane per component), the Aarseth
+//      step and the block rule, then sets the particle's flag.
 // The launch ends when the run is finished, after max_steps steps, or at a step with more than
 // max_act due particles, which the chain of launches (hd_begin -> hd_predict -> force -> reduce ->
 // hd_correct) takes with the planner's launch shape.  Every sum is taken in a fixed order and the due
@@ -30,7 +29,6 @@
 #include "nbk_device.cuh"
 
 namespace nbk {
-
 
 namespace {
 
