@@ -156,6 +156,45 @@ int nbk_calc_lasthalf_f64(nbk_ctx* ctx, int64_t n_i, double* acc, double* jerk, 
 /* Same to DEVICE arrays, asynchronous on the stream, no synchronisation. */
 int nbk_calc_lasthalf_dev(nbk_ctx* ctx, int64_t n_i, float* acc, float* jerk, float* pot);
 
+/* ---- the same force evaluation for callers that must not allocate --------------------------------
+ * nbk_open allocates device and pinned memory, so everything above needs a caller that may call
+ * cudaMalloc.  Not every caller can: a plug-in in a process whose memory pool has already taken the
+ * device's memory (a library-side cudaMalloc then fails or eats what the host application counted
+ * on), a step loop that cannot afford cudaMalloc / cudaFree stalling the device, a code that forbids
+ * allocation after start-up.  nbk_calc_noalloc_dev is the one entry point for them.  It takes no
+ * context and calls no cudaMalloc, cudaFree, cudaHostAlloc or any routine that allocates: inputs
+ * and outputs are the caller's device arrays, and the split-j partial rows and
+ * their arrival counters sit in a fixed array of NBK_NOALLOC_SCRATCH_BYTES that is part of the
+ * library's device image -- each GPU that loads libnbk.so carries it until the process exits.
+ *
+ *   device, cuda_stream   the device the arrays live on and a cudaStream_t of that device to enqueue
+ *                         on (NULL: the legacy default stream).  Asynchronous: nothing waits.
+ *   m[n_j], x[n_j][3], v[n_j][3]   the j-particles' state at the time of the evaluation, fp32, already
+ *                         predicted by the caller (no predictor runs here); v may be NULL without NBK_JERK.
+ *   i_index[n_i]          i-particle k is j-particle i_index[k]; its own j entry is left out of its
+ *                         sums.  NULL: i_index[k] = k.  An entry outside [0, n_j) gets zeros.
+ *   eps2, flags           as nbk_calc_firsthalf; NBK_NN is refused (NBK_EINVAL).
+ *   acc[n_i][3], jerk[n_i][3], pot[n_i]   results (any may be NULL; jerk is zero without NBK_JERK).
+ *   cuda_error            optional HOST int: the cudaError_t behind an NBK_ECUDA return, else 0.
+ * All array pointers are DEVICE pointers.  Sums as defined at the top of this file: fp32 per pair,
+ * fp64 across tiles and splits in a fixed order (repeatable bit for bit), results rounded once.
+ *
+ * Limits, and what sharing one array means:
+ *   - n_i <= NBK_NOALLOC_MAX_NI and n_j <= NBK_NOALLOC_MAX_NJ, else NBK_ERANGE and nothing is enqueued.
+ *   - The first call on a device looks up the array's device address (cudaGetSymbolAddress, with that
+ *     device current; this can make the runtime load the library's device code).  Make that first
+ *     call before starting any stream capture.
+ *   - All calls on a device use the same array.  Calls on one stream are ordered and safe; calls of a
+ *     process that can overlap on the GPU (two streams without an event between them) race on the
+ *     rows and counters and give wrong results.  The counters are zeroed on the stream at the start
+ *     of every call; the rows are written before they are read, so old contents never matter. */
+#define NBK_NOALLOC_MAX_NI 4096
+#define NBK_NOALLOC_MAX_NJ 16777216
+#define NBK_NOALLOC_SCRATCH_BYTES (4194304 + 256)
+int nbk_calc_noalloc_dev(int device, void* cuda_stream, int64_t n_j, const float* m, const float* x,
+                         const float* v, int64_t n_i, const int32_t* i_index, float eps2,
+                         uint32_t flags, float* acc, float* jerk, float* pot, int* cuda_error);
+
 /* ---- nearest neighbour ("the GRAPE hardware also calculates the nearest
  * neighbour of every particle that is being updated ... done as part of the force calculation";
  * SURVEY.md 8(f)-2) ------------------------------------------------------------------------------ */

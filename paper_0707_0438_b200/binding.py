@@ -16,11 +16,13 @@ from . import build as _build
 
 NBK_OK, NBK_EINVAL, NBK_ERANGE, NBK_ENOMEM, NBK_ECUDA, NBK_ESTATE = 0, -1, -2, -3, -4, -5
 NBK_JERK, NBK_POT, NBK_EPS0, NBK_NN = 1, 2, 4, 8
+NBK_NOALLOC_MAX_NI, NBK_NOALLOC_MAX_NJ = 4096, 16777216
 
 EXPORTS = [
     "nbk_open", "nbk_open_ws", "nbk_workspace_bytes", "nbk_close", "nbk_npipes", "nbk_set_j_particles", "nbk_set_j_particles_f64",
     "nbk_set_j_particles_dev", "nbk_set_ti", "nbk_predict", "nbk_get_predicted",
     "nbk_calc_firsthalf", "nbk_calc_firsthalf_dev", "nbk_calc_lasthalf", "nbk_calc_lasthalf_f64", "nbk_calc_lasthalf_dev",
+    "nbk_calc_noalloc_dev",
     "nbk_get_neighbours", "nbk_get_neighbours_dev", "nbk_calc_batch", "nbk_calc_batch_dev",
     "nbk_shard_gather_i_dev", "nbk_shard_calc_partial_dev", "nbk_shard_finish_dev",
     "nbk_shard_fetch_i_dev", "nbk_shard_combine_dev",
@@ -55,6 +57,8 @@ _SIGS = {
     "nbk_calc_lasthalf": (_i32, [_vp, _i64, _vp, _vp, _vp]),
     "nbk_calc_lasthalf_f64": (_i32, [_vp, _i64, _vp, _vp, _vp]),
     "nbk_calc_lasthalf_dev": (_i32, [_vp, _i64, _vp, _vp, _vp]),
+    "nbk_calc_noalloc_dev": (_i32, [_i32, _vp, _i64, _vp, _vp, _vp, _i64, _vp, _f32, _u32, _vp, _vp, _vp,
+                                    ctypes.POINTER(_i32)]),
     "nbk_calc_batch": (_i32, [_vp, _i64, _vp, _vp, _vp, _vp, _vp, _f32, _u32, _vp, _vp]),
     "nbk_calc_batch_dev": (_i32, [_vp, _i64, _vp, _vp, _vp, _vp, _vp, _f32, _u32, _vp, _vp]),
     "nbk_get_neighbours": (_i32, [_vp, _i64, _vp, _vp]),
@@ -249,6 +253,19 @@ def nbk_calc_lasthalf_f64(ctx, n_i):
 def nbk_calc_lasthalf_dev(ctx, n_i, acc=0, jerk=0, pot=0):
     _check("nbk_calc_lasthalf_dev",
            load().nbk_calc_lasthalf_dev(ctx, n_i, acc or None, jerk or None, pot or None), ctx)
+
+
+def nbk_calc_noalloc_dev(device, cuda_stream, n_j, m, x, v, n_i, i_index=0, eps2=0.0, flags=NBK_JERK | NBK_POT,
+                         acc=0, jerk=0, pot=0):
+    """The context-free force call for callers that must not allocate device memory (include/nbk.h).
+    m, x, v, i_index, acc, jerk, pot: device addresses (0 = NULL); cuda_stream: a cudaStream_t value (0 = the
+    legacy default stream).  Enqueues and returns; sizes beyond NBK_NOALLOC_MAX_NI / _NJ raise (NBK_ERANGE)."""
+    err = _i32(0)
+    st = load().nbk_calc_noalloc_dev(device, cuda_stream or None, n_j, m or None, x or None, v or None, n_i,
+                                     i_index or None, float(eps2), flags, acc or None, jerk or None, pot or None,
+                                     ctypes.byref(err))
+    if st != NBK_OK:
+        raise NbkError("nbk_calc_noalloc_dev", st, err.value)
 
 
 def nbk_calc_batch(ctx, i_offset, xi, j_offset, mj, xj, eps2=0.0, flags=NBK_POT):

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 INCLUDE = os.path.join(ROOT, "include")
-SOURCES = ["nbk_force.cu", "nbk_state_kernels.cu", "nbk_batch_kernels.cu", "nbk_hermite_kernels.cu", "nbk_hermite_steps.cu", "nbk_small_kernels.cu", "nbk_shard_kernels.cu", "nbk_api.cu",
+SOURCES = ["nbk_force.cu", "nbk_state_kernels.cu", "nbk_batch_kernels.cu", "nbk_hermite_kernels.cu", "nbk_hermite_steps.cu", "nbk_small_kernels.cu", "nbk_shard_kernels.cu", "nbk_noalloc.cu", "nbk_api.cu",
            "nbk_hermite_dev.cu", "nbk_batch.cu", "nbk_hermite.cpp"]
 HEADERS = [os.path.join(CSRC, h) for h in ("nbk_kernels.cuh", "nbk_device.cuh", "nbk_ctx.cuh", "nbk_hermite_common.h")] + [os.path.join(INCLUDE, "nbk.h")]
 LIB = os.path.join(HERE, "libnbk.so")
