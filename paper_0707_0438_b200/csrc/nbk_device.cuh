@@ -291,8 +291,9 @@ __device__ __forceinline__ void predict_one(const RawJ& raw, long long j, double
     o[3] = ld_state<CG>(raw.m + j);
 }
 
-// Corrector of one component (reading R15; fp64).  dt = 2^-k is a power of two, so the divisions by
-// dt^2 and dt^3 are exact multiplications by 2^2k and 2^3k (same bits as the quotient).
+// Predictor + corrector of one component of a due particle (reading R15; fp64; formulas in
+// nbk_hermite_common.h).  dt = 2^-k is a power of two, so the divisions by dt^2 and dt^3 are exact
+// multiplications by 2^2k and 2^3k (same bits as the quotient).
 __device__ __forceinline__ void correct_component(double x, double v, double a0, double j0, double a1,
                                                   double j1, int k, double& x1, double& v1,
                                                   double& a2e, double& a3) {
@@ -300,15 +301,9 @@ __device__ __forceinline__ void correct_component(double x, double v, double a0,
     const double dt = __longlong_as_double((1023LL - k) << 52);
     const double inv_dt2 = __longlong_as_double((1023LL + 2 * k) << 52);
     const double inv_dt3 = __longlong_as_double((1023LL + 3 * k) << 52);
-    const double xp = x + v * dt + a0 * (dt * dt / 2.0) + j0 * (dt * dt * dt / 6.0);
-    const double vp = v + a0 * dt + j0 * (dt * dt / 2.0);
-    const double da = a0 - a1;
-    const double a2 = (-6.0 * da - dt * (4.0 * j0 + 2.0 * j1)) * inv_dt2;
-    a3 = (12.0 * da + 6.0 * dt * (j0 + j1)) * inv_dt3;
-    const double dt3 = dt * dt * dt, dt4 = dt3 * dt;
-    x1 = xp + a2 * (dt4 / 24.0) + a3 * (dt4 * dt / 120.0);
-    v1 = vp + a2 * (dt3 / 6.0) + a3 * (dt4 / 24.0);
-    a2e = a2 + a3 * dt;
+    double xp, vp;
+    hermite_predict_component(x, v, a0, j0, dt, xp, vp);
+    hermite_correct_component(xp, vp, a0, j0, a1, j1, dt, inv_dt2, inv_dt3, x1, v1, a2e, a3);
 }
 
 // What a corrected particle writes: the fp64 state and the raw j-state the predictor reads.

@@ -143,11 +143,10 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
 #pragma omp parallel for schedule(static) if (ni >= kParallelMin)
         for (int64_t q = 0; q < ni; ++q) {
             const size_t i = static_cast<size_t>(act[q]);
-            const double dt = t_new - tl[i], dt2 = dt * dt / 2.0, dt3 = dt * dt * dt / 6.0;
+            const double dt = t_new - tl[i];
             for (int c = 0; c < 3; ++c) {
                 const size_t k = 3 * i + c;
-                xp[3 * q + c] = x[k] + v[k] * dt + a[k] * dt2 + jk[k] * dt3;
-                vp[3 * q + c] = v[k] + a[k] * dt + jk[k] * dt2;
+                nbk::hermite_predict_component(x[k], v[k], a[k], jk[k], dt, xp[3 * q + c], vp[3 * q + c]);
             }
         }
         slot = 1;
@@ -160,19 +159,15 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
         for (int64_t q = 0; q < ni; ++q) {
             const int32_t ii = act[q];
             const size_t i = static_cast<size_t>(ii);
-            const double dt = t_new - tl[i];
+            const double dt = t_new - tl[i];  // the particle's own step: an exact power of two
+            const double inv_dt2 = 1.0 / (dt * dt), inv_dt3 = 1.0 / (dt * dt * dt);
             double a1[3], j1[3], a2e[3], a3[3];
             for (int c = 0; c < 3; ++c) {
                 const size_t k = 3 * i + c;
                 a1[c] = fa[3 * q + c];
                 j1[c] = fj[3 * q + c];
-                const double da = a[k] - a1[c];
-                const double a2 = (-6.0 * da - dt * (4.0 * jk[k] + 2.0 * j1[c])) / (dt * dt);
-                a3[c] = (12.0 * da + 6.0 * dt * (jk[k] + j1[c])) / (dt * dt * dt);
-                const double dt3 = dt * dt * dt, dt4 = dt3 * dt;
-                x[k] = xp[3 * q + c] + a2 * (dt4 / 24.0) + a3[c] * (dt4 * dt / 120.0);
-                v[k] = vp[3 * q + c] + a2 * (dt3 / 6.0) + a3[c] * (dt4 / 24.0);
-                a2e[c] = a2 + a3[c] * dt;
+                nbk::hermite_correct_component(xp[3 * q + c], vp[3 * q + c], a[k], jk[k], a1[c], j1[c], dt,
+                                               inv_dt2, inv_dt3, x[k], v[k], a2e[c], a3[c]);
                 a[k] = a1[c];
                 jk[k] = j1[c];
             }
@@ -211,9 +206,6 @@ extern "C" int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, doub
     st.t_reached = std::ldexp(static_cast<double>(T), -kTickLog2);
     st.wall_seconds = wall.seconds();
     st.gpu_call_seconds = gpu_s;
-    if (std::getenv("NBK_TRACE"))
-        std::fprintf(stderr, "nbk_hermite_evolve: firsthalf %.3f s  lasthalf %.3f s  set_j %.3f s  wall %.3f s\n",
-                     prof[0], prof[1], prof[2], st.wall_seconds);
     if (stats) *stats = st;
     return NBK_OK;
 }

@@ -1,5 +1,6 @@
 // nbk_hermite_common.h -- the pieces of reading R15 that both Hermite drivers share:
-// the power-of-two level of a wanted step and the start-up step.  One copy, used by the host driver
+// the power-of-two level of a wanted step, the start-up step, the fp64 predictor of a due particle and
+// the corrector.  One copy, used by the host driver
 // (nbk_hermite.cpp), the device-resident driver's set-up (nbk_hermite_dev.cu) and its kernels
 // (nbk_hermite_kernels.cu).  Plain C++ usable from host and device code; internal to the CUDA path.
 //
@@ -19,7 +20,8 @@ namespace nbk {
 constexpr int kTickLog2 = 52;   // time unit 2^-52: exact integer block times up to t = 2048
 constexpr int kMaxLevel = 48;   // finest step 2^-48
 
-// Level k of the largest step 2^-k <= want, clamped to [kmin, kMaxLevel] (kmin >= 0: dt_max <= 1).
+// Level k of the largest step 2^-k <= want, clamped to [kmin, kMaxLevel] (kmin >= 0; dt_max itself may
+// lie in [2^-48, 2) and is rounded down to a power of two first, see level_of_dt_max).
 NBK_HD inline int level_for(double want, int kmin) {
     if (!(want > 0.0)) return kMaxLevel;
     int e;
@@ -75,6 +77,33 @@ NBK_HD inline int next_level_norms(double na, double nj, double n2, double n3, d
 NBK_HD inline int next_level(const double* a1, const double* j1, const double* a2e, const double* a3,
                              double eta, int k_old, int kmin, long long T_new) {
     return next_level_norms(norm3(a1), norm3(j1), norm3(a2e), norm3(a3), eta, k_old, kmin, T_new);
+}
+
+
+// fp64 predictor of one component of a due particle over its own step dt (reading R8 / R15):
+//   x_p = x + v dt + a0 dt^2/2 + j0 dt^3/6,  v_p = v + a0 dt + j0 dt^2/2.
+NBK_HD inline void hermite_predict_component(double x, double v, double a0, double j0, double dt,
+                                             double& xp, double& vp) {
+    xp = x + v * dt + a0 * (dt * dt / 2.0) + j0 * (dt * dt * dt / 6.0);
+    vp = v + a0 * dt + j0 * (dt * dt / 2.0);
+}
+
+// Corrector of one component (reading R15; fp64) -- the ONE copy of these coefficients in the product
+// (host driver nbk_hermite.cpp, hd_correct_kernel and hd_steps_kernel through nbk_device.cuh):
+//   a2 = [-6 (a0 - a1) - dt (4 j0 + 2 j1)] / dt^2,   a3 = [12 (a0 - a1) + 6 dt (j0 + j1)] / dt^3,
+//   x1 = x_p + a2 dt^4/24 + a3 dt^5/120,  v1 = v_p + a2 dt^3/6 + a3 dt^4/24,  a2e = a2 + a3 dt.
+// dt is a block step 2^-k, so 1/dt^2 and 1/dt^3 are exact powers of two and multiplying by them gives
+// the bits of the division; the callers pass them (the device builds them from k's bit pattern).
+NBK_HD inline void hermite_correct_component(double xp, double vp, double a0, double j0, double a1,
+                                             double j1, double dt, double inv_dt2, double inv_dt3,
+                                             double& x1, double& v1, double& a2e, double& a3) {
+    const double da = a0 - a1;
+    const double a2 = (-6.0 * da - dt * (4.0 * j0 + 2.0 * j1)) * inv_dt2;
+    a3 = (12.0 * da + 6.0 * dt * (j0 + j1)) * inv_dt3;
+    const double dt3 = dt * dt * dt, dt4 = dt3 * dt;
+    x1 = xp + a2 * (dt4 / 24.0) + a3 * (dt4 * dt / 120.0);
+    v1 = vp + a2 * (dt3 / 6.0) + a3 * (dt4 / 24.0);
+    a2e = a2 + a3 * dt;
 }
 
 }  // namespace nbk

@@ -782,6 +782,49 @@ def test_device_resident_paths_agree(gpu, monkeypatch, eps):
             assert np.median(np.linalg.norm(gx - hx, axis=1)) < 1e-4, max_act
 
 
+@pytest.mark.parametrize("n", [40000, 70001])
+def test_device_resident_stepping_kernel_at_bench_sizes(gpu, c_oracle, monkeypatch, n):
+    """The stepping kernel at the sizes the C5 number is measured at, which the N = 1500 test above never
+    reaches: a j-chunk of several hundred particles per CTA (multi-block loop over 256-particle blocks),
+    more than one 16-byte vector of level bytes per thread in the due-list scan (n > 65536: more than four),
+    and due lists of 513..1024 particles that take the three-round split of the tiled pair sums.  Integrated
+    to t = 1/16 with all steps of <= 1024 particles in hd_steps_kernel, twice (bitwise repeatable), against the
+    launch-chain route and the host driver: same particle steps to 0.1 %, nearby end states, energy."""
+    m, x, v = inputs.plummer(n, seed=77)
+    t_end = 1.0 / 16.0
+    e0 = _energy(c_oracle, m, x, v, EPS)
+    with Ctx(n) as ctx:
+        hx, hv = x.copy(), v.copy()
+        sh = nb.nbk_hermite_evolve(ctx, m, hx, hv, EPS, t_end)
+        out = {}
+        for max_act in ("1024", "0"):
+            monkeypatch.setenv("NBK_STEPS_MAX_ACT", max_act)
+            runs = []
+            for _ in range(2 if max_act == "1024" else 1):
+                gx, gv = x.copy(), v.copy()
+                st = nb.nbk_hermite_evolve_dev(ctx, m, gx, gv, EPS, t_end)
+                runs.append((gx, gv, st))
+            if len(runs) == 2:
+                assert np.array_equal(runs[0][0], runs[1][0]) and np.array_equal(runs[0][1], runs[1][1])
+                assert runs[0][2]["particle_steps"] == runs[1][2]["particle_steps"]
+            out[max_act] = runs[0]
+    gx, gv, st = out["1024"]
+    cx, cv, sc = out["0"]
+    hist = st["ni_histogram"]
+    assert sum(hist[:10]) > 100 and hist[9] > 0, hist        # steps the stepping kernel takes, incl. 512..1023
+    for what, (ox, ov, so) in (("launch chain", (cx, cv, sc)), ("host driver", (hx, hv, sh))):
+        dx = np.linalg.norm(gx - ox, axis=1)
+        print(f"n={n} stepping kernel vs {what}: particle_steps {st['particle_steps']} / {so['particle_steps']}, "
+              f"block_steps {st['block_steps']} / {so['block_steps']}, |dx| median {np.median(dx):.2e} "
+              f"p99 {np.percentile(dx, 99):.2e} max {dx.max():.2e}")
+        assert st["t_reached"] == so["t_reached"] == t_end
+        # measured: particle steps within 1.1e-4 relative, |dx| median <= 9.2e-12, p99 <= 4.1e-11
+        assert abs(st["particle_steps"] - so["particle_steps"]) <= 1e-3 * so["particle_steps"], what
+        assert np.median(dx) < 1e-10 and np.percentile(dx, 99) < 1e-9, what
+    e1 = _energy(c_oracle, m, gx, gv, EPS)
+    assert abs((e1 - e0) / e0) < 1e-6
+
+
 def test_batched_calls_small_groups_split_lanes(gpu, c_oracle):
     """Batched calls with the lanes of a warp split 2 and 4 ways over each j-tile (mean group size
     12-23 and below 12): every group against the oracle, bitwise repeatable."""
