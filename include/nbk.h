@@ -269,9 +269,14 @@ int nbk_hermite_evolve(nbk_ctx* ctx, int64_t n, const double* m, double* x, doub
  * step takes the launches.  Same scheme, formulas, arguments and argument limits as nbk_hermite_evolve;
  * results are bitwise repeatable; stats->gpu_call_seconds equals wall_seconds.  NBK_ECUDA with
  * nbk_last_cuda_error() == cudaErrorLaunchTimeout means a wait inside the persistent kernel gave up
- * (another process holding SMs for seconds): the state is then undefined.  Test knob: the environment
- * variable NBK_STEPS_MAX_ACT (0..1024, read at each call) caps the step size the persistent kernel takes;
- * 0 sends every step through the launches. */
+ * (another process holding SMs for seconds; the first CTA to give up raises an abort word and the others
+ * leave within milliseconds): the state is then undefined.  NBK_ERANGE after the forces at t = 0 means no
+ * launch plan of a large step fits the context's partial-row buffer (open it with a larger ni_max).  Test
+ * knob: the environment variable NBK_STEPS_MAX_ACT (a whole number 0..1024, read at each call; anything else
+ * is NBK_EINVAL) caps the step size the persistent kernel takes; 0 sends every step through the launches.
+ * After the call nbk_last_launch reports the persistent kernel: out[0] its CTAs (0: not used), out[1] its
+ * threads, out[4] the step-size cap, out[7] 2 if it was captured as a cooperative launch (the driver checks
+ * that all CTAs are co-resident), 1 if as a plain launch (co-residency by construction: one CTA per SM). */
 int nbk_hermite_evolve_dev(nbk_ctx* ctx, int64_t n, const double* m, double* x, double* v,
                            double eps, double t_end, double eta, double dt_max,
                            nbk_hermite_stats* stats);

@@ -57,6 +57,14 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     if (!c->d_hdr) NBK_CUDA(c, cudaMalloc(&c->d_hdr, sizeof(DynHeader)));
     if (!c->h_hdr) NBK_CUDA(c, cudaMallocHost(&c->h_hdr, sizeof(DynHeader)));
 
+    int env_max_act = -1;   // test knob NBK_STEPS_MAX_ACT (include/nbk.h): a whole number 0..kStepsMaxAct, else NBK_EINVAL
+    if (const char* e = std::getenv("NBK_STEPS_MAX_ACT")) {
+        char* end = nullptr;
+        const long val = std::strtol(e, &end, 10);
+        if (end == e || *end != '\0' || val < 0 || val > kStepsMaxAct) return NBK_EINVAL;
+        env_max_act = static_cast<int>(val);
+    }
+
     // t = 0 through the ordinary entry points: forces on everybody, first steps (reading R15)
     std::vector<float> fa(3 * N), fj(3 * N);
     std::vector<double> a(3 * N), jk(3 * N), tl(N, 0.0);
@@ -108,7 +116,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     // in batches with no host synchronisation inside a batch, and rounds past t_end return at once.
     const int G = H.num_sms;
     int max_act = kStepsMaxAct;
-    if (const char* e = std::getenv("NBK_STEPS_MAX_ACT")) max_act = std::atoi(e);
+    if (env_max_act >= 0) max_act = env_max_act;
     if (max_act > kStepsMaxAct) max_act = kStepsMaxAct;
     if (max_act > G * (kStepsThreads / 32)) max_act = G * (kStepsThreads / 32);   // one due particle per warp
     const int chunk = static_cast<int>(round_up_ll((n + G - 1) / G, 4));
@@ -129,6 +137,12 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
             NBK_CUDA(c, cudaMemsetAsync(c->hs.rows, 0, need, c->stream));
             c->hs_rows_bytes = need;
         }
+    }
+    if (c->hs_seq >= (1u << 31)) {   // 32-bit tags: start over long before they wrap (a zeroed word = no step yet;
+                                     // one call would need more than 2^31 steps to wrap by itself)
+        if (c->hs.rows) NBK_CUDA(c, cudaMemsetAsync(c->hs.rows, 0, c->hs_rows_bytes, c->stream));
+        NBK_CUDA(c, cudaMemsetAsync(c->hs.flag, 0, sizeof(unsigned long long) * kStepsMaxAct, c->stream));
+        c->hs_seq = 0;
     }
     H.steps_max_act = max_act;
     H.seq = c->hs_seq;
@@ -195,7 +209,17 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
         cudaError_t ce2 = cudaStreamEndCapture(c->stream, &graph);
         if (ce == cudaSuccess) ce = ce2;
         if (ce == cudaSuccess) ce = cudaGraphInstantiate(&gexec, graph, 0);
-        if (ce == cudaSuccess) break;
+        if (ce == cudaSuccess) {
+            // nbk_last_launch after this call: out[0] CTAs of the stepping kernel (0: off), out[1] its threads,
+            // out[7] 2 = captured as a cooperative launch (co-residency checked by the driver), 1 = plain launch
+            // (co-residency by construction: one CTA per SM, occupancy checked in steps_prepare), 0 = no stepping kernel
+            c->last_launch[0] = max_act > 0 ? G : 0;
+            c->last_launch[1] = max_act > 0 ? kStepsThreads : 0;
+            c->last_launch[2] = 0; c->last_launch[3] = 0; c->last_launch[4] = max_act;
+            c->last_launch[5] = G; c->last_launch[6] = 0;
+            c->last_launch[7] = max_act > 0 ? (cooperative ? 2 : 1) : 0;
+            break;
+        }
         if (graph) cudaGraphDestroy(graph);
         graph = nullptr;
         gexec = nullptr;
@@ -216,6 +240,7 @@ int nbk_hermite_evolve_dev(nbk_ctx* c, int64_t n, const double* m, double* x, do
     if (ce != cudaSuccess) return cuda_fail(c, ce);
     if (c->h_hdr->error) {   // a wait inside the stepping kernel gave up: its tags are not to be trusted again
         c->hs_seq = c->h_hdr->seq + (1u << 24);
+        if (c->h_hdr->error == 2) return NBK_ERANGE;   // no launch plan fits this context's partial rows
         return cuda_fail(c, cudaErrorLaunchTimeout);
     }
     NBK_CUDA(c, cudaMemcpyAsync(x, c->hs.x, sizeof(double) * 3 * N, cudaMemcpyDeviceToHost, c->stream));

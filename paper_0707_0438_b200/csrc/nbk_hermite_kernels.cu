@@ -24,6 +24,10 @@ __global__ void hd_begin_kernel(DynHeader* h) {
     pdl_wait();
     const int tid = threadIdx.x;
     if (h->done) return;
+    if (h->error) {   // the stepping kernel gave up a wait: the state is undefined, run nothing more on it
+        if (tid == 0) h->done = 1;
+        return;
+    }
     if (tid <= kMaxLevel) cnt[tid] = h->level_count[tid];
     __syncthreads();
     if (tid == 0) {
@@ -74,6 +78,11 @@ __global__ void hd_begin_kernel(DynHeader* h) {
             const int I = c < kPlanCandidates ? 1 : 4;
             const double w = static_cast<double>(cost[c]) * warps_of(I) / (I == 4 ? 1.0 : 0.86);
             if (bc < 0 || w < best * (1.0 - 1e-9)) { bc = c; best = w; }
+        }
+        if (bc < 0) {   // no candidate fits the partial-row buffer: stop here rather than launch a garbage plan
+            h->error = 2;
+            h->done = 1;
+            return;
         }
         h->plan = cand[bc];
         h->plan_I = bc < kPlanCandidates ? 1 : 4;

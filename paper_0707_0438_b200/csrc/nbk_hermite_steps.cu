@@ -36,6 +36,16 @@ constexpr int kSW = kStepsThreads / 32;   // warps per CTA
 constexpr int kLaneJMax = 4;              // steps of up to this many particles: lanes run over j
 constexpr long long kSpinLimit = 1LL << 26;
 
+// One failed poll of a wait on another CTA's tagged word.  Every 4096 polls the waiter looks at the launch's
+// abort word (DynHeader::error); the waiter that runs out of polls raises it, so that all other CTAs leave
+// within a few thousand polls of the first one giving up instead of each running out its own limit.
+__device__ __forceinline__ bool spin_abort(long long& spins, DynHeader* h) {
+    if ((++spins & 4095) != 0) return false;
+    if (spins <= kSpinLimit && *reinterpret_cast<volatile int*>(&h->error) == 0) return false;
+    atomicExch(&h->error, 1);
+    return true;
+}
+
 
 // one value of a partial row and the number of the step it belongs to, in one 8-byte word
 __device__ __forceinline__ unsigned long long row_word(float v, unsigned seq) {
@@ -161,7 +171,7 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
             unsigned long long f;
             long long spins = 0;
             while (static_cast<unsigned>((f = ld_acquire64(hs.flag + q)) >> 32) != want) {
-                if (++spins > kSpinLimit) { S.err = 1; break; }   // never hang the device
+                if (spin_abort(spins, h)) { S.err = 1; break; }   // never hang the device
             }
             const int nl = static_cast<int>(f & 0xffu), ol = L.lev[i] - 1;
             if (nl != ol) {
@@ -417,7 +427,7 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
                                     static_cast<unsigned>(w1.x >> 32) == seq &&
                                     (hf || static_cast<unsigned>(w1.y >> 32) == seq);   // word 7 is not used
                     if (ok) break;
-                    if (++spins > kSpinLimit) { S.err = 1; break; }   // never hang the device
+                    if (spin_abort(spins, h)) { S.err = 1; break; }   // never hang the device
                 }
                 v4[0] = __uint_as_float(static_cast<unsigned>(w0.x)); v4[1] = __uint_as_float(static_cast<unsigned>(w0.y));
                 v4[2] = __uint_as_float(static_cast<unsigned>(w1.x)); v4[3] = hf ? 0.0 : __uint_as_float(static_cast<unsigned>(w1.y));
@@ -432,7 +442,7 @@ __global__ void __launch_bounds__(kStepsThreads, 1) hd_steps_kernel(const StepsA
                 for (int e = 0; e < 4; ++e) S.scratch[warp][lane][e] = v4[e];
             }
             __syncthreads();
-            if (warp == 0) {
+            if (warp == 0 && !S.err) {   // (a wait gave up: the rows are not this step's -- correct nothing, publish no flag)
                 double sv = 0.0;   // lane v < 7: sum v (acc3, m/sqrt(s), jerk3)
                 if (lane < 8) {
 #pragma unroll

@@ -159,7 +159,7 @@ struct DynHeader {
     int fused;                          // the force kernel's last CTA reduces (small block)
     int skip;                           // this step is left to hd_steps_kernel: the launched chain returns
     int steps_max_act;                  // hd_steps_kernel takes steps of up to this many due particles (0: off)
-    int error;                          // a grid barrier of hd_steps_kernel gave up waiting
+    int error;                          // 1: a wait of hd_steps_kernel on another CTA's tagged rows / flags gave up; 2: hd_begin_kernel found no launch plan that fits
     unsigned seq;                       // hd_steps_kernel: steps it has taken so far
 };
 struct HermiteState {        // fp64 integrator state, [n][3] row-major; level[n]

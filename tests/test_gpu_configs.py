@@ -825,6 +825,50 @@ def test_device_resident_stepping_kernel_at_bench_sizes(gpu, c_oracle, monkeypat
     assert abs((e1 - e0) / e0) < 1e-6
 
 
+def test_device_resident_reports_its_launch_form_and_validates_the_knob(gpu, monkeypatch):
+    """nbk_last_launch after nbk_hermite_evolve_dev says whether the persistent stepping kernel ran and how it
+    was captured (2: cooperative launch, 1: plain launch, 0: not used), so a silent fall-back from the
+    cooperative form is visible; NBK_STEPS_MAX_ACT must be a whole number in 0..1024."""
+    m, x, v = inputs.plummer(600, seed=3)
+    with Ctx(600) as ctx:
+        monkeypatch.setenv("NBK_STEPS_MAX_ACT", "1024")
+        nb.nbk_hermite_evolve_dev(ctx, m, x.copy(), v.copy(), EPS, 1.0 / 64.0, dt_max=1.0 / 64.0)
+        shape = nb.nbk_last_launch(ctx)
+        assert shape["launches"] == 2, shape          # the B200 box captures the cooperative form
+        assert shape["grid"] == shape["sms"] and shape["threads"] == 512 and shape["j_tile"] == 1024
+        monkeypatch.setenv("NBK_STEPS_MAX_ACT", "0")
+        nb.nbk_hermite_evolve_dev(ctx, m, x.copy(), v.copy(), EPS, 1.0 / 64.0, dt_max=1.0 / 64.0)
+        shape = nb.nbk_last_launch(ctx)
+        assert shape["launches"] == 0 and shape["grid"] == 0, shape
+        for bad in ("-1", "1025", "12x", "", "4.5"):
+            monkeypatch.setenv("NBK_STEPS_MAX_ACT", bad)
+            with pytest.raises(nb.NbkError) as e:
+                nb.nbk_hermite_evolve_dev(ctx, m, x.copy(), v.copy(), EPS, 1.0 / 64.0, dt_max=1.0 / 64.0)
+            assert e.value.status == nb.NBK_EINVAL, bad
+
+
+def test_stepping_kernel_200_repeats_bitwise(gpu, monkeypatch):
+    """hd_steps_kernel hands partial rows and per-particle flags from CTA to CTA through global memory
+    (tagged 8-byte words, st.relaxed / ld.acquire, no grid barrier) -- traffic compute-sanitizer's racecheck
+    does not look at (it checks shared memory only; profiles/r03_sanitizer.md).  A missed wait would show as a
+    run that read a stale row: 200 runs of N = 1500 to t = 1/32 (~400 block steps each) must all end in the
+    bits of the first, for eps > 0 and eps = 0."""
+    m, x, v = inputs.plummer(1500, seed=23)
+    monkeypatch.setenv("NBK_STEPS_MAX_ACT", "1024")
+    with Ctx(1500) as ctx:
+        for eps in (EPS, 0.0):
+            first = None
+            for rep in range(200):
+                gx, gv = x.copy(), v.copy()
+                st = nb.nbk_hermite_evolve_dev(ctx, m, gx, gv, eps, 1.0 / 32.0, dt_max=1.0 / 32.0)
+                if first is None:
+                    first = (gx, gv, st["block_steps"], st["particle_steps"])
+                    assert st["t_reached"] == 1.0 / 32.0 and st["block_steps"] > 100
+                    continue
+                assert (st["block_steps"], st["particle_steps"]) == first[2:], (eps, rep)
+                assert np.array_equal(gx, first[0]) and np.array_equal(gv, first[1]), (eps, rep)
+
+
 def test_batched_calls_small_groups_split_lanes(gpu, c_oracle):
     """Batched calls with the lanes of a warp split 2 and 4 ways over each j-tile (mean group size
     12-23 and below 12): every group against the oracle, bitwise repeatable."""
