@@ -753,9 +753,9 @@ def run_sweep(args):
     print()
     print("| N | n_i (block) | force+reduce kernels us | interactions/s | firsthalf+lasthalf wall us (host API) |")
     print("|---|---|---|---|---|")
-    for n, seed in ((16384, 2), (65536, 5)):
+    for n, seed in ((16384, 2), (65536, 5), (131072, 3), (1048576, 4)):   # north_star: N from 1K to 1M, block-step i-sets
         m, x, v = inputs.plummer_f32(n, seed)
-        ctx = nb.nbk_open(0, n, n)
+        ctx = nb.nbk_open(0, n, 16384)
         try:
             nb.nbk_set_j_particles(ctx, None, None, m, x, v)
             for n_i in (1, 32, 256, 2048, 16384):

@@ -18,8 +18,10 @@
  *     pot_i  = -sum_j m_j s^(-1/2)
  *
  * over all j in [0, n_j) except the i-particle's own j entry; with NBK_EPS0 pairs with
- * s == 0 contribute nothing.  Pairwise arithmetic is fp32 (FMA + rsqrt.approx), partial
- * sums are folded in fp64 on the device, results are returned in fp32.
+ * s == 0 contribute nothing.  Pairwise arithmetic is fp32 (FMA + rsqrt.approx); the sums over
+ * one j-tile are fp32, a CTA adds its tiles in fp64 and rounds its share once to an fp32 partial
+ * row, the partial rows of an i-particle (at most one per CTA) are added in fp64 in a fixed order;
+ * results are returned in fp32.
  *
  * Conventions
  *   - Every function returns NBK_OK (0) or a negative nbk_status; nothing throws or aborts.
@@ -301,7 +303,8 @@ int nbk_hermite_evolve_dev(nbk_ctx* ctx, int64_t n, const double* m, double* x, 
  * 2. nbk_shard_calc_partial_dev: the force kernel and split-j reduction of i-particles with the
  *    state xv (after the exchange) against local j-particles [0, n_local), the own entry of an
  *    owned i-particle (i_local[k] >= 0) left out; writes sum64[k][0..7] = (acc(3), -pot, jerk(3),
- *    0) as the fp64 sums BEFORE the rounding to fp32 (the fp32 results of this rank alone remain
+ *    0): the fp64 sum of this rank's fp32 partial rows (each CTA's share is rounded to fp32 once, as
+ *    on one GPU), NOT yet rounded to the fp32 result (the fp32 results of this rank alone remain
  *    readable with nbk_calc_lasthalf*).  flags as nbk_calc_firsthalf; NBK_NN is refused
  *    (NBK_EINVAL).  n_local == 0 is allowed (sums are zero).
  * 3. nbk_shard_finish_dev: after all-reduce(sum) of sum64: acc, jerk, pot in fp32 (one rounding;

@@ -386,7 +386,8 @@ cudaError_t launch_batch_reduce(const BatchArgs& a, cudaStream_t s);
 
 // device-resident integrator kernels (one block step = begin, predict+select, force, reduce, correct)
 // hd_steps_kernel (nbk_hermite_steps.cu): whole block steps of up to max_act due particles inside one
-// persistent kernel, one CTA per SM, grid barriers between the phases of a step.
+// persistent kernel, one CTA per SM; the phases of a step are ordered by per-word step tags on the partial
+// rows and per-particle flags (no grid barrier, no counter).
 constexpr int kStepsThreads = 512;     // 16 warps per CTA
 constexpr int kStepsMaxAct = 1024;     // largest step the stepping kernel can hold (due list in shared memory)
 constexpr int kStepsMaxVec = 16;       // 16-byte loads of level bytes per thread at most: n <= 131072

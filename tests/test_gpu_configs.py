@@ -4,6 +4,8 @@ expected values come from oracle/ on the same seeded inputs.  Tolerances: tests/
 
 Run on the B200 box:  python -m pytest tests -m gpu -x -q
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -419,9 +421,18 @@ def test_nearest_neighbour_matches_oracle(gpu, c_oracle, n, n_i, eps):
     if n_i > 32:
         for a, b in zip(plain, withnn):
             assert np.array_equal(a, b)
-    else:   # small blocks: the plain call is the one-launch kernel, the neighbour search rides in the tiled one
-        assert np.abs(plain[0] - withnn[0]).max() <= 2e-6 * np.abs(plain[0]).max()
-        assert scalar_rel_err(plain[2], withnn[2]).max() < 1e-6
+    else:   # small blocks: the plain call is the one-launch kernel, the neighbour search rides in the tiled one.
+        # Different summation orders, so not the same bits: each form must sit within a few fp32 ulps of the
+        # fp64 oracle sum (ulp of the vector's norm; measured on a B200: acc <= 0.86, jerk <= 4.2, pot <= 0.51), hence within a
+        # few ulps of the other.
+        ref = c_oracle.force(m, x, v, eps, i_index=idx)
+        ulp = 2.0 ** -23
+        for name, got in (("one-launch", plain), ("tiled+nn", withnn)):
+            ea = vec_rel_err(got[0], ref[0]).max() / ulp
+            ej = vec_rel_err(got[1], ref[1]).max() / ulp
+            ep = scalar_rel_err(got[2], ref[2]).max() / ulp
+            print(f"nn small block n_i={n_i} eps={eps} {name}: acc {ea:.2f} jerk {ej:.2f} pot {ep:.2f} ulp")
+            assert ea <= 4.0 and ej <= 16.0 and ep <= 2.0, (name, ea, ej, ep)
     _check_nn(nn, r2, ref_nn, ref_r2, x, idx, what=f"nn n={n} n_i={n_i} eps={eps}")
     if n == 300:
         pos = {int(i): k for k, i in enumerate(idx)}
@@ -845,6 +856,48 @@ def test_device_resident_reports_its_launch_form_and_validates_the_knob(gpu, mon
             with pytest.raises(nb.NbkError) as e:
                 nb.nbk_hermite_evolve_dev(ctx, m, x.copy(), v.copy(), EPS, 1.0 / 64.0, dt_max=1.0 / 64.0)
             assert e.value.status == nb.NBK_EINVAL, bad
+
+
+_PDL_SCRIPT = """
+import sys, numpy as np
+sys.path.insert(0, {root!r})
+from paper_0707_0438_b200 import binding as nb, inputs
+m, x, v = inputs.plummer_f32(3000, seed=8)
+ctx = nb.nbk_open(0, 3000, 3000)
+out = []
+nb.nbk_set_j_particles(ctx, None, None, m, x, v)
+for n_i, t in ((3000, 0.0), (200, 0.01), (7, 0.02)):
+    nb.nbk_set_ti(ctx, t)
+    idx = inputs.active_block(3000, n_i, seed=n_i)
+    nb.nbk_calc_firsthalf(ctx, 3000, n_i, idx, None, None, np.float32(1 / 256) ** 2, 3)
+    out += list(nb.nbk_calc_lasthalf(ctx, n_i))
+md, xd, vd = inputs.plummer(400, seed=9)
+nb.nbk_hermite_evolve_dev(ctx, md, xd, vd, 1 / 256, 1 / 32, dt_max=1 / 32)
+nb.nbk_close(ctx)
+np.savez({path!r}, *out, xd, vd)
+"""
+
+
+def test_programmatic_dependent_launch_switch_changes_no_bits(gpu, tmp_path):
+    """NBK_PDL=0 (read once per process, csrc/nbk_api.cu) launches the block-step kernel chain without the
+    programmatic-dependent-launch attribute: griddepcontrol.wait / launch_dependents then do nothing and the
+    stream orders the kernels fully.  Same kernels, same data, so the same bits as with the attribute on -- a
+    kernel that touched global memory before its pdl_wait would differ with it on.  Two child processes."""
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    res = {}
+    for pdl in ("1", "0"):
+        path = str(tmp_path / f"pdl{pdl}.npz")
+        env = dict(os.environ, NBK_PDL=pdl)
+        env.pop("NBK_STEPS_MAX_ACT", None)
+        subprocess.run([sys.executable, "-c", _PDL_SCRIPT.format(root=root, path=path)], check=True, env=env,
+                       timeout=600)
+        with np.load(path) as z:
+            res[pdl] = [z[k] for k in z.files]
+    assert len(res["1"]) == len(res["0"]) == 11
+    for a, b in zip(res["1"], res["0"]):
+        assert np.array_equal(a, b)
 
 
 def test_stepping_kernel_200_repeats_bitwise(gpu, monkeypatch):
