@@ -151,7 +151,11 @@ int nbk_calc_firsthalf_dev(nbk_ctx* ctx, int64_t n_j, int64_t n_i, const int32_t
 /* ---- a7: read back (GPUcalc_lasthalf, L430) ----------------------------------------------- */
 
 /* Wait for the last firsthalf and copy acc[n_i][3], jerk[n_i][3], pot[n_i] to HOST arrays
- * (any may be NULL; jerk is zero if NBK_JERK was not set).  n_i must equal firsthalf's. */
+ * (any may be NULL; jerk is zero if NBK_JERK was not set).  n_i must equal firsthalf's.
+ * After a one-launch small block (n_i <= 32 particles of the j-set) the wait is a poll of a word in
+ * mapped host memory that the kernel writes after the results, not a stream synchronisation: the call
+ * returns as soon as the results are in host memory; the stream itself may take a microsecond longer to
+ * drain (nbk_sync waits for that). */
 int nbk_calc_lasthalf(nbk_ctx* ctx, int64_t n_i, float* acc, float* jerk, float* pot);
 /* Same into double arrays (GRAPE-style callers keep doubles); the values are the fp32 results. */
 int nbk_calc_lasthalf_f64(nbk_ctx* ctx, int64_t n_i, double* acc, double* jerk, double* pot);

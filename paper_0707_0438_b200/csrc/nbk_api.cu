@@ -8,6 +8,7 @@
 #include <climits>
 #include <cmath>
 #include <cstdlib>
+#include <atomic>
 #include <cstring>
 #include <functional>
 #include <new>
@@ -200,6 +201,9 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
             sa.counter = c->d_counter;
             sa.acc = acc; sa.jerk = jerk; sa.pot = pot;
             sa.host_out = to_host ? c->h_result_dev : nullptr;
+            sa.host_seq = to_host ? c->h_seq_dev : nullptr;
+            sa.seq = ++c->small_seq;
+            if (sa.seq == 0) sa.seq = ++c->small_seq;   // 0 is the word's initial value
             sa.upd = c->pending;
             if (!c->small_ready) {
                 NBK_CUDA(c, small_prepare(kSmallMaxChunk));
@@ -217,6 +221,7 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
             c->pred_valid = true;
             c->pred_nj = n_j;
             c->host_has_result = to_host;
+            c->poll_result = to_host;
             c->last_launch[0] = G; c->last_launch[1] = 512; c->last_launch[2] = 1; c->last_launch[3] = 16;
             c->last_launch[4] = chunk; c->last_launch[5] = c->num_sms;
             c->last_launch[6] = static_cast<long long>(small_smem_bytes(sa.chunk)); c->last_launch[7] = 1;
@@ -230,6 +235,7 @@ int enqueue_force(nbk_ctx* c, long long n_j, long long n_i, const int32_t* d_iid
     c->last_ni = n_i;
     c->in_flight = true;
     c->host_has_result = false;
+    c->poll_result = false;
     if (n_i == 0) return NBK_OK;
     if (n_j == 0) {
         NBK_CUDA(c, cudaMemsetAsync(acc, 0, sizeof(float) * 7 * n_i, c->stream));
@@ -523,8 +529,12 @@ int open_impl(nbk_ctx** out, int device, int64_t n_max, int64_t ni_max, void* cu
         if ((e = dalloc(reinterpret_cast<void**>(&c->d_xi), sizeof(float) * 3 * ni)) != cudaSuccess) break;
         if ((e = dalloc(reinterpret_cast<void**>(&c->d_vi), sizeof(float) * 3 * ni)) != cudaSuccess) break;
         if ((e = dalloc(reinterpret_cast<void**>(&c->d_result), sizeof(float) * 7 * ni)) != cudaSuccess) break;
-        if ((e = cudaHostAlloc(&c->h_result, sizeof(float) * 9 * ni, cudaHostAllocMapped)) != cudaSuccess) break;
+        const size_t seq_at = (9 * ni + 15) / 16 * 16;   // the sequence word on a 64-byte line of its own behind the results
+        if ((e = cudaHostAlloc(&c->h_result, sizeof(float) * (seq_at + 16), cudaHostAllocMapped)) != cudaSuccess) break;
         if ((e = cudaHostGetDevicePointer(&c->h_result_dev, c->h_result, 0)) != cudaSuccess) break;
+        std::memset(c->h_result + seq_at, 0, sizeof(float) * 16);
+        c->h_seq = reinterpret_cast<volatile unsigned*>(c->h_result + seq_at);
+        c->h_seq_dev = reinterpret_cast<unsigned*>(c->h_result_dev + seq_at);
         if ((e = dalloc(reinterpret_cast<void**>(&c->d_counter), sizeof(unsigned))) != cudaSuccess) break;
         if ((e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned), c->stream)) != cudaSuccess) break;
         c->partial_bytes = sizeof(float) * plan_partial_floats_bound(ni_max, c->num_sms);
@@ -747,7 +757,26 @@ int nbk_calc_lasthalf(nbk_ctx* c, int64_t n_i, float* acc, float* jerk, float* p
     if (!c->host_has_result)
         NBK_CUDA(c, cudaMemcpyAsync(c->h_result, c->d_result, sizeof(float) * 7 * ni,
                                     cudaMemcpyDeviceToHost, c->stream));
-    NBK_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->host_has_result && c->poll_result && !c->timing) {
+        // One-launch small block: its last CTA wrote the results into h_result (mapped) and then the sequence
+        // word.  Seeing the word is enough -- no need to wait for the kernel to retire and the driver to notice
+        // (the per-call overhead is what a block step of a few particles costs).  The stream
+        // is asked now and then so that a failed launch ends the wait.
+        const unsigned want = c->small_seq;
+        for (unsigned spins = 1; *c->h_seq != want; ++spins) {
+            if ((spins & 2047u) == 0) {
+                const cudaError_t q = cudaStreamQuery(c->stream);
+                if (q == cudaSuccess) {
+                    if (*c->h_seq == want) break;
+                    return cuda_fail(c, cudaErrorUnknown);   // the kernel retired without writing the word
+                }
+                if (q != cudaErrorNotReady) return cuda_fail(c, q);
+            }
+        }
+        std::atomic_thread_fence(std::memory_order_acquire);
+    } else {
+        NBK_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
     if (acc) std::memcpy(acc, c->h_result, sizeof(float) * 3 * ni);
     if (jerk) std::memcpy(jerk, c->h_result + 3 * ni, sizeof(float) * 3 * ni);
     if (pot) std::memcpy(pot, c->h_result + 6 * ni, sizeof(float) * ni);

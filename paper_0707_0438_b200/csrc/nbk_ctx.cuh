@@ -73,6 +73,10 @@ struct nbk_ctx {
     nbk::DynHeader* d_hdr = nullptr;
     nbk::DynHeader* h_hdr = nullptr;     // pinned
     bool host_has_result = false;   // the last firsthalf wrote h_result itself (no D2H needed)
+    volatile unsigned* h_seq = nullptr;  // mapped word behind h_result: small_block_kernel's "results are in host memory" mark
+    unsigned* h_seq_dev = nullptr;
+    unsigned small_seq = 0;              // value the last small-block launch writes there
+    bool poll_result = false;            // lasthalf may poll h_seq instead of synchronising the stream
     nbk::InlineJ pending;                // a small set_j not yet on the device (pending.n == 0: none)
 
     unsigned char* h_stage = nullptr;  // pinned staging for set_j

@@ -337,6 +337,8 @@ struct SmallArgs {
     float* jerk;
     float* pot;
     float* host_out;          // mapped pinned copy acc|jerk|pot (7 n_i floats) or nullptr
+    unsigned* host_seq;       // mapped pinned word: set to `seq` after host_out is complete (nullptr: not wanted)
+    unsigned seq;
     InlineJ upd;              // a pending set_j of a few particles (upd.n may be 0), all addresses < n_j
 };
 size_t small_smem_bytes(int chunk);

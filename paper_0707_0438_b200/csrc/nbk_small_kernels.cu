@@ -265,7 +265,14 @@ __global__ void __launch_bounds__(kST, 1) small_block_kernel(const SmallArgs a) 
                 a.host_out[3 * n + 3 * tx + c] = r[3 + c];
             }
             a.host_out[6 * n + tx] = r[6];
+            __threadfence_system();   // the results are in host memory before the sequence word below
         }
+    }
+    // The host may wait for the results by polling one mapped word instead of waiting for the kernel to retire
+    // (nbk_calc_lasthalf): written last, by one thread, after every result-writing thread's system fence.
+    if (a.host_seq) {
+        __syncthreads();
+        if (tid == 0) *reinterpret_cast<volatile unsigned*>(a.host_seq) = a.seq;
     }
 }
 
